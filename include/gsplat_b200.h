@@ -1,0 +1,151 @@
+/* gsplat_b200.h -- C ABI of the single-GPU (sm_100a) differentiable 3D Gaussian splatting hot path.
+ *
+ * What this library computes is the data-parallel hot path inside the custom splatting
+ * operators that arxiv/paper_2606_11390 distributes across GPUs (section 4:
+ * "Gaussian spherical harmonics [10] and Gaussian projection operators ... each GPU processes
+ * a segment of the input Gaussians and outputs colors and projected geometric quantities for
+ * all cameras in the batch"; "the GPU sorts the Gaussians by depth, rasterizes them to obtain
+ * the rendered image"; "atomics are needed to accumulate gradients in the backward
+ * pass"; "per-pixel/tile intersection records").  The paper states no formula and
+ * defers to its reference [10]; the mathematics is written out in SURVEY.md
+ * section 8(c) (steps O-P1, O-B, O-R1, O-R2, O-P5) and restated in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *   - Every pointer is a DEVICE pointer owned by the caller unless its comment says "host".
+ *     The library never allocates or frees device memory and keeps no global state.
+ *   - Arrays are dense, row-major, fp32 unless stated; counts are int64_t.
+ *   - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default
+ *     stream).  The only host synchronisation is in gs_bin_tiles when `M_out` is non-NULL.
+ *   - Views of one call share width, height and the tile size; a "batch" is C >= 1 views.
+ *     Per-(view, Gaussian) arrays are laid out [C, N, *]; entry e = c*N + i.
+ *   - Return value: GS_OK (0) or a negative gs_status.  No exception crosses the ABI.
+ *   - Culled (view, Gaussian) entries have radii == 0 and tiles_touched == 0; their other
+ *     per-view fields are unspecified and are never read by later stages.
+ */
+#ifndef GSPLAT_B200_H_
+#define GSPLAT_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GS_MAX_VIEWS 64 /* upper bound on C per call */
+
+typedef enum gs_status {
+    GS_OK = 0,
+    GS_ERR_INVALID_ARGUMENT = -1, /* null / misaligned pointer, N < 0, C out of range, bad config, views differ in size */
+    GS_ERR_CAPACITY = -2,         /* gs_bin_tiles: capacity_M too small; needed M is in *M_out */
+    GS_ERR_CUDA = -3,             /* a CUDA runtime call or launch failed (cudaGetLastError) */
+    GS_ERR_UNSUPPORTED = -4       /* tile != 16, C*N >= 2^31, M >= 2^30 */
+} gs_status;
+
+/* Pinhole camera (host struct).  Pixel (row i, col j) samples the image plane at (j+0.5, i+0.5).
+ * viewmat = world->camera [W | tau], row-major 3x4; camera axes +x right, +y down, +z forward
+ * (SURVEY.md 8(c) reading A3). */
+typedef struct gs_camera {
+    int32_t width, height;
+    float fx, fy, cx, cy;
+    float viewmat[12];
+    float near_plane, far_plane; /* cull t_z <= near or t_z >= far (reading A4) */
+} gs_camera;
+
+/* Constants of the method (host struct); gs_config_default fills the 3DGS values:
+ * dilation 0.3, alpha_min 1/255, alpha_max 0.99, t_min 1e-4, extent 3, tile 16, sh_degree 3
+ * (readings A6, A7, A11). */
+typedef struct gs_config {
+    float dilation, alpha_min, alpha_max, t_min, extent;
+    int32_t tile;      /* only 16 is supported */
+    int32_t sh_degree; /* 0..3; K = (sh_degree+1)^2 bases */
+} gs_config;
+
+int gs_config_default(gs_config* cfg /*host, out*/);
+const char* gs_status_string(int status);
+
+/* P1 -- per-Gaussian forward.
+ * exp(log-scale), normalised quaternion (w,x,y,z) -> Sigma = R S S^T R^T; t = W p + tau; near/far
+ * cull; EWA Jacobian with the 1.3x field-of-view clamp -> 2-D covariance + dilation -> conic and
+ * det cull; radius = ceil(extent*sqrt(lambda_max)); mean2d, depth; fp32 tile rectangle and
+ * tiles_touched; SH colour (+0.5, clamp >= 0) along the camera->Gaussian direction; sigmoid opacity.
+ * in : means[N,3] log_scales[N,3] quats[N,4] opacity_logits[N] sh[N,K,3]; cams: host array of C.
+ * out: means2d[C,N,2] depths[C,N] conics[C,N,3] (A,B,C) opacities[C,N] rgbs[C,N,3]
+ *      radii[C,N] (int32, 0 = culled) tiles_touched[C,N] (uint32). */
+int gs_project_fwd(const gs_config* cfg /*host*/, int64_t N, const float* means, const float* log_scales,
+                   const float* quats, const float* opacity_logits, const float* sh, int32_t C,
+                   const gs_camera* cams /*host*/, float* means2d, float* depths, float* conics,
+                   float* opacities, float* rgbs, int32_t* radii, uint32_t* tiles_touched, void* stream);
+
+/* B1..B4 -- tile binning for a batch of views.
+ * For every entry e = c*N + i with radii[e] > 0, in ascending e, one record per overlapped 16x16
+ * tile (tile rectangle recomputed in fp32 from means2d and radii exactly as in P1 step 8):
+ *   key = (uint64)(c*tiles + ty*Gx + tx) << 32 | bit pattern of depths[e],  value = e.
+ * Records are stably radix-sorted by key (equal keys keep ascending e), and tile_ranges[t] =
+ * [first, last+1) of the records whose key >> 32 == t ([0,0) when none), t in [0, C*tiles).
+ * workspace == NULL: only *workspace_bytes (host) is written (size query for N, C, capacity_M).
+ * capacity_M: number of records isect_keys / isect_vals can hold.
+ * M_dev (device, optional): receives the total record count M.
+ * M_out (host, optional): if non-NULL the call synchronises `stream`, writes M, and returns
+ *   GS_ERR_CAPACITY when M > capacity_M (outputs are then incomplete but nothing is written
+ *   out of bounds).  With M_out == NULL the call never synchronises; overflow is reported only
+ *   through M_dev.
+ * isect_keys[capacity_M] (uint64), isect_vals[capacity_M] (int32), tile_ranges[C*tiles,2] (int64). */
+int gs_bin_tiles(const gs_config* cfg /*host*/, int64_t N, int32_t C, const gs_camera* cams /*host*/,
+                 const float* means2d, const float* depths, const int32_t* radii, void* workspace,
+                 size_t* workspace_bytes /*host*/, int64_t capacity_M, uint64_t* isect_keys,
+                 int32_t* isect_vals, int64_t* tile_ranges, int64_t* M_dev, int64_t* M_out /*host*/,
+                 void* stream);
+
+/* Stand-alone stable LSD radix sort used by gs_bin_tiles (step B3), exported for testing and
+ * measurement: sorts n (key, value) pairs on key bits [0, end_bit) -- bit 31 is skipped when
+ * skip_bit31 != 0 (positive fp32 depth patterns).  keys/vals are overwritten with the result;
+ * workspace as in gs_bin_tiles (NULL -> size query). */
+int gs_sort_pairs(int64_t n, int32_t end_bit, int32_t skip_bit31, uint64_t* keys, int32_t* vals, void* workspace,
+                  size_t* workspace_bytes /*host*/, void* stream);
+
+/* R1 -- rasterisation forward.  Per pixel, front to back over
+ * its tile's range: power = -1/2 d^T K d; skip power > 0; alpha = min(alpha_max, o*exp(power));
+ * skip alpha < alpha_min; stop before T(1-alpha) < t_min; C += rgb*alpha*T.  image = C + T*bg.
+ * out: image[C,H,W,3] final_T[C,H,W] n_contrib[C,H,W] (index+1 of the last composited record). */
+int gs_raster_fwd(const gs_config* cfg /*host*/, int32_t C, const gs_camera* cams /*host*/,
+                  const int32_t* isect_vals, const int64_t* tile_ranges, const float* means2d,
+                  const float* conics, const float* opacities, const float* rgbs, const float* bg /*host[3]*/,
+                  float* image, float* final_T, int32_t* n_contrib, void* stream);
+
+/* R2 -- rasterisation backward.  Per pixel, back to front over
+ * the first n_contrib records, recomputing alpha and recovering T by division; gradients are summed
+ * per (view, Gaussian) entry with warp-shuffle + shared-memory reduction and device-scope atomics.
+ * radii (optional): when given, only rows with radii > 0 are zero-filled before accumulation (rows of
+ * culled entries are left untouched and are never read by gs_project_bwd); when NULL all C*N rows
+ * are zero-filled.  N_total = C*N.
+ * out: dL_dmeans2d[C,N,2] dL_dconics[C,N,3] dL_dopacities[C,N] dL_drgbs[C,N,3]. */
+int gs_raster_bwd(const gs_config* cfg /*host*/, int32_t C, const gs_camera* cams /*host*/, int64_t N_total,
+                  const int32_t* isect_vals, const int64_t* tile_ranges, const float* means2d,
+                  const float* conics, const float* opacities, const float* rgbs, const float* bg /*host[3]*/,
+                  const float* final_T, const int32_t* n_contrib, const float* dL_dimage /*[C,H,W,3]*/,
+                  const int32_t* radii /*optional*/, float* dL_dmeans2d, float* dL_dconics, float* dL_dopacities,
+                  float* dL_drgbs, void* stream);
+
+/* P5 -- per-Gaussian backward.  Chain rule through conic ->
+ * 2-D covariance -> (J, Sigma) -> (mean, log-scale, quaternion), mean2d -> mean, rgb -> SH
+ * coefficients and view direction -> mean, opacity -> logit; summed over the C views.  Gradients
+ * are with respect to the RAW parameters (reading A1).
+ * accumulate == 0: every row of every output is overwritten (zeros for Gaussians visible nowhere);
+ * accumulate != 0: rows of Gaussians visible in >= 1 view are added to, other rows untouched.
+ * out: dL_dmeans[N,3] dL_dlog_scales[N,3] dL_dquats[N,4] dL_dopacity_logits[N] dL_dsh[N,K,3]. */
+int gs_project_bwd(const gs_config* cfg /*host*/, int64_t N, const float* means, const float* log_scales,
+                   const float* quats, const float* opacity_logits, const float* sh, int32_t C,
+                   const gs_camera* cams /*host*/, const int32_t* radii, const float* dL_dmeans2d,
+                   const float* dL_dconics, const float* dL_dopacities, const float* dL_drgbs,
+                   float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats, float* dL_dopacity_logits,
+                   float* dL_dsh, int32_t accumulate, void* stream);
+
+/* Harness loss (SURVEY.md 8(c) reading A18): mean-reduced L1 against a target image.
+ * dL_dimage[n] = sign(image - target) / n; *loss_sum (device, float, caller-zeroed) += sum |image - target| / n. */
+int gs_l1_loss(int64_t n, const float* image, const float* target, float* dL_dimage, float* loss_sum, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSPLAT_B200_H_ */

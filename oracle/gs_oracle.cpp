@@ -331,7 +331,7 @@ void project_fwd(const double* cfg_, int64_t N, const R* means, const R* log_sca
 template <class R>
 void raster_fwd(const double* cfg_, int C, int width, int height, const int32_t* vals, const int64_t* ranges,
                 const R* means2d, const R* conics, const R* opacities, const R* rgbs, const R* bg, R* image,
-                R* final_T, int32_t* n_contrib, uint8_t* ambiguous, double rel_eps) {
+                R* final_T, int32_t* n_contrib, uint8_t* ambiguous, double rel_eps, const uint8_t* tile_mask) {
     const Cfg cfg = load_cfg(cfg_);
     const int Gx = (width + cfg.tile - 1) / cfg.tile, Gy = (height + cfg.tile - 1) / cfg.tile;
     const int64_t tiles = (int64_t)Gx * Gy;
@@ -339,6 +339,7 @@ void raster_fwd(const double* cfg_, int C, int width, int height, const int32_t*
         for (int i = 0; i < height; ++i)
             for (int j = 0; j < width; ++j) {
                 const int64_t t = (int64_t)c * tiles + (int64_t)(i / cfg.tile) * Gx + (j / cfg.tile);
+                if (tile_mask && !tile_mask[t]) continue;   // sampled evaluation: pixels of unselected tiles are left untouched
                 const R px = (R)j + (R)0.5, py = (R)i + (R)0.5;
                 R T = 1, Cacc[3] = {0, 0, 0};
                 int32_t n = 0, last = 0;
@@ -383,7 +384,7 @@ template <class R>
 void raster_bwd(const double* cfg_, int C, int width, int height, int64_t Ntot, const int32_t* vals,
                 const int64_t* ranges, const R* means2d, const R* conics, const R* opacities, const R* rgbs,
                 const R* bg, const R* final_T, const int32_t* n_contrib, const R* dL_dimage, R* dL_dmeans2d,
-                R* dL_dconics, R* dL_dopacities, R* dL_drgbs) {
+                R* dL_dconics, R* dL_dopacities, R* dL_drgbs, const uint8_t* tile_mask) {
     const Cfg cfg = load_cfg(cfg_);
     const int Gx = (width + cfg.tile - 1) / cfg.tile, Gy = (height + cfg.tile - 1) / cfg.tile;
     const int64_t tiles = (int64_t)Gx * Gy;
@@ -395,6 +396,7 @@ void raster_bwd(const double* cfg_, int C, int width, int height, int64_t Ntot, 
         for (int i = 0; i < height; ++i)
             for (int j = 0; j < width; ++j) {
                 const int64_t t = (int64_t)c * tiles + (int64_t)(i / cfg.tile) * Gx + (j / cfg.tile);
+                if (tile_mask && !tile_mask[t]) continue;   // sampled evaluation (caller zeroes dL_dimage there)
                 const int64_t pix = ((int64_t)c * height + i) * width + j;
                 const R px = (R)j + (R)0.5, py = (R)i + (R)0.5;
                 const R* g3 = dL_dimage + 3 * pix;
@@ -596,17 +598,19 @@ void project_bwd(const double* cfg_, int64_t N, const R* means, const R* log_sca
                                             const int32_t* vals, const int64_t* ranges, const R* means2d,       \
                                             const R* conics, const R* opacities, const R* rgbs, const R* bg,    \
                                             R* image, R* final_T, int32_t* n_contrib, uint8_t* ambiguous,       \
-                                            double rel_eps) {                                                   \
+                                            double rel_eps, const uint8_t* tile_mask) {                         \
         raster_fwd<R>(cfg, C, width, height, vals, ranges, means2d, conics, opacities, rgbs, bg, image,         \
-                      final_T, n_contrib, ambiguous, rel_eps);                                                  \
+                      final_T, n_contrib, ambiguous, rel_eps, tile_mask);                                       \
     }                                                                                                           \
     extern "C" void oracle_raster_bwd_##SUF(const double* cfg, int C, int width, int height, int64_t Ntot,      \
                                             const int32_t* vals, const int64_t* ranges, const R* means2d,       \
                                             const R* conics, const R* opacities, const R* rgbs, const R* bg,    \
                                             const R* final_T, const int32_t* n_contrib, const R* dL_dimage,     \
-                                            R* dL_dmeans2d, R* dL_dconics, R* dL_dopacities, R* dL_drgbs) {     \
+                                            R* dL_dmeans2d, R* dL_dconics, R* dL_dopacities, R* dL_drgbs,       \
+                                            const uint8_t* tile_mask) {                                         \
         raster_bwd<R>(cfg, C, width, height, Ntot, vals, ranges, means2d, conics, opacities, rgbs, bg,          \
-                      final_T, n_contrib, dL_dimage, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs);         \
+                      final_T, n_contrib, dL_dimage, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs,          \
+                      tile_mask);                                                                               \
     }                                                                                                           \
     extern "C" void oracle_project_bwd_##SUF(const double* cfg, int64_t N, const R* means,                      \
                                              const R* log_scales, const R* quats, const R* logits,              \

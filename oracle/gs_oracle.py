@@ -59,6 +59,15 @@ def _p(a):
     return a.ctypes.data_as(C.c_void_p)
 
 
+def _mask(tile_mask):
+    """Optional uint8 [C*tiles] selection of tiles to evaluate (sampled checks at full size)."""
+    if tile_mask is None:
+        return None
+    m = np.ascontiguousarray(tile_mask, dtype=np.uint8)
+    _mask.keep = m
+    return _p(m)
+
+
 def _suffix(dtype):
     dtype = np.dtype(dtype)
     if dtype == np.float64:
@@ -122,7 +131,7 @@ def bin_tiles(cfg, cams, means2d, depths, radii):
 
 
 def raster_fwd(cfg, cams, vals, ranges, means2d, conics, opacities, rgbs, bg, dtype=np.float64,
-               ambiguity_eps=None):
+               ambiguity_eps=None, tile_mask=None):
     """O-R1.  Returns (image [C,H,W,3], final_T [C,H,W], n_contrib [C,H,W] i32[, ambiguous u8])."""
     nc = len(cams)
     W, H = cams[0]["width"], cams[0]["height"]
@@ -137,14 +146,14 @@ def raster_fwd(cfg, cams, vals, ranges, means2d, conics, opacities, rgbs, bg, dt
     fn = getattr(lib(), "oracle_raster_fwd_" + _suffix(dtype))
     fn(_p(ca), C.c_int(nc), C.c_int(W), C.c_int(H), _p(vals), _p(ranges), _p(means2d), _p(conics), _p(opacities),
        _p(rgbs), _p(bg), _p(image), _p(final_T), _p(n_contrib), _p(amb) if amb is not None else None,
-       C.c_double(0.0 if ambiguity_eps is None else ambiguity_eps))
+       C.c_double(0.0 if ambiguity_eps is None else ambiguity_eps), _mask(tile_mask))
     if amb is not None:
         return image, final_T, n_contrib, amb
     return image, final_T, n_contrib
 
 
 def raster_bwd(cfg, cams, vals, ranges, means2d, conics, opacities, rgbs, bg, final_T, n_contrib, dL_dimage,
-               dtype=np.float64):
+               dtype=np.float64, tile_mask=None):
     """O-R2.  Returns dict of per-(view,Gaussian) 2-D gradients shaped like the inputs."""
     nc = len(cams)
     W, H = cams[0]["width"], cams[0]["height"]
@@ -159,7 +168,7 @@ def raster_bwd(cfg, cams, vals, ranges, means2d, conics, opacities, rgbs, bg, fi
     fn = getattr(lib(), "oracle_raster_bwd_" + _suffix(dtype))
     fn(_p(ca), C.c_int(nc), C.c_int(W), C.c_int(H), C.c_int64(ntot), _p(vals), _p(ranges), _p(means2d), _p(conics),
        _p(opacities), _p(rgbs), _p(bg), _p(final_T), _p(n_contrib), _p(dL_dimage), _p(out["means2d"]),
-       _p(out["conics"]), _p(out["opacities"]), _p(out["rgbs"]))
+       _p(out["conics"]), _p(out["opacities"]), _p(out["rgbs"]), _mask(tile_mask))
     return out
 
 

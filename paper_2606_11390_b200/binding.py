@@ -1,0 +1,219 @@
+"""Thin ctypes binding of ``libgsplat_b200.so`` (C ABI in ``include/gsplat_b200.h``).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels behind the C
+entry points.  PyTorch is used for device memory and streams.  Function names match the C
+names.  There is NO CPU fallback: if the library is missing the import of a function raises,
+and the functions refuse non-CUDA tensors.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgsplat_b200.so")
+
+GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+
+EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
+           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss"]
+
+
+class gs_camera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("viewmat", C.c_float * 12),
+                ("near_plane", C.c_float), ("far_plane", C.c_float)]
+
+
+class gs_config(C.Structure):
+    _fields_ = [("dilation", C.c_float), ("alpha_min", C.c_float), ("alpha_max", C.c_float),
+                ("t_min", C.c_float), ("extent", C.c_float), ("tile", C.c_int32), ("sh_degree", C.c_int32)]
+
+
+class GsError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)} ({status})")
+
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA library; raises if it has not been built (no fallback exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_11390_b200.build` "
+                               "(there is no CPU fallback)")
+        _lib = C.CDLL(LIB_PATH)
+        _lib.gs_status_string.restype = C.c_char_p
+        _lib.gs_status_string.argtypes = [C.c_int]
+        for name in EXPORTS:
+            if name != "gs_status_string":
+                getattr(_lib, name).restype = C.c_int
+    return _lib
+
+
+def status_string(status):
+    return lib().gs_status_string(int(status)).decode()
+
+
+def default_config(**kw):
+    cfg = gs_config()
+    rc = lib().gs_config_default(C.byref(cfg))
+    if rc:
+        raise GsError(rc, "gs_config_default")
+    for k, v in kw.items():
+        setattr(cfg, k, v)
+    return cfg
+
+
+def make_cameras(cams):
+    """Sequence of camera dicts (see ``scenes.make_camera``) -> ctypes array of gs_camera."""
+    arr = (gs_camera * len(cams))()
+    for k, c in enumerate(cams):
+        a = arr[k]
+        a.width, a.height = int(c["width"]), int(c["height"])
+        a.fx, a.fy, a.cx, a.cy = float(c["fx"]), float(c["fy"]), float(c["cx"]), float(c["cy"])
+        vm = np.asarray(c["viewmat"], dtype=np.float32).reshape(12)
+        for j in range(12):
+            a.viewmat[j] = float(vm[j])
+        a.near_plane, a.far_plane = float(c["near"]), float(c["far"])
+    return arr
+
+
+def grid_of(cams_arr):
+    return (cams_arr[0].width + 15) // 16, (cams_arr[0].height + 15) // 16
+
+
+def _ptr(t, dtype=None):
+    import torch
+    if t is None:
+        return C.c_void_p(0)
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("expected a CUDA tensor (the library has no CPU path)")
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check(rc, where):
+    if rc != GS_OK:
+        raise GsError(rc, where)
+
+
+def gs_project_fwd(cfg, means, log_scales, quats, opacity_logits, sh, cams, means2d, depths, conics, opacities, rgbs,
+                   radii, tiles_touched, stream=None):
+    import torch
+    N = means.shape[0]
+    rc = lib().gs_project_fwd(C.byref(cfg), C.c_int64(N), _ptr(means, torch.float32), _ptr(log_scales, torch.float32),
+                              _ptr(quats, torch.float32), _ptr(opacity_logits, torch.float32), _ptr(sh, torch.float32),
+                              C.c_int32(len(cams)), cams, _ptr(means2d, torch.float32), _ptr(depths, torch.float32),
+                              _ptr(conics, torch.float32), _ptr(opacities, torch.float32), _ptr(rgbs, torch.float32),
+                              _ptr(radii, torch.int32), _ptr(tiles_touched), _stream(stream))
+    _check(rc, "gs_project_fwd")
+
+
+def gs_bin_tiles_workspace_bytes(cfg, N, cams, capacity_M):
+    n = C.c_size_t(0)
+    rc = lib().gs_bin_tiles(C.byref(cfg), C.c_int64(N), C.c_int32(len(cams)), cams, None, None, None, None, C.byref(n),
+                            C.c_int64(capacity_M), None, None, None, None, None, None)
+    _check(rc, "gs_bin_tiles(size query)")
+    return int(n.value)
+
+
+def gs_bin_tiles(cfg, N, cams, means2d, depths, radii, workspace, capacity_M, isect_keys, isect_vals, tile_ranges,
+                 M_dev=None, sync=True, stream=None):
+    """Returns M (host int) when ``sync`` is true, else None (M is then only in ``M_dev``).
+    Raises GsError(GS_ERR_CAPACITY) with ``.needed`` set when capacity_M is too small."""
+    import torch
+    wb = C.c_size_t(workspace.numel() * workspace.element_size())
+    m = C.c_int64(0)
+    rc = lib().gs_bin_tiles(C.byref(cfg), C.c_int64(N), C.c_int32(len(cams)), cams, _ptr(means2d, torch.float32),
+                            _ptr(depths, torch.float32), _ptr(radii, torch.int32), _ptr(workspace), C.byref(wb),
+                            C.c_int64(capacity_M), _ptr(isect_keys), _ptr(isect_vals, torch.int32),
+                            _ptr(tile_ranges, torch.int64), _ptr(M_dev, torch.int64) if M_dev is not None else None,
+                            C.byref(m) if sync else None, _stream(stream))
+    if rc == GS_ERR_CAPACITY:
+        err = GsError(rc, "gs_bin_tiles")
+        err.needed = int(m.value)
+        raise err
+    _check(rc, "gs_bin_tiles")
+    return int(m.value) if sync else None
+
+
+def gs_sort_pairs_workspace_bytes(n):
+    b = C.c_size_t(0)
+    rc = lib().gs_sort_pairs(C.c_int64(n), C.c_int32(64), C.c_int32(0), None, None, None, C.byref(b), None)
+    _check(rc, "gs_sort_pairs(size query)")
+    return int(b.value)
+
+
+def gs_sort_pairs(n, end_bit, skip_bit31, keys, vals, workspace, stream=None):
+    import torch
+    wb = C.c_size_t(workspace.numel() * workspace.element_size())
+    rc = lib().gs_sort_pairs(C.c_int64(n), C.c_int32(end_bit), C.c_int32(1 if skip_bit31 else 0), _ptr(keys),
+                             _ptr(vals, torch.int32), _ptr(workspace), C.byref(wb), _stream(stream))
+    _check(rc, "gs_sort_pairs")
+
+
+def _bg(bg):
+    return (C.c_float * 3)(float(bg[0]), float(bg[1]), float(bg[2]))
+
+
+def gs_raster_fwd(cfg, cams, isect_vals, tile_ranges, means2d, conics, opacities, rgbs, bg, image, final_T, n_contrib,
+                  stream=None):
+    import torch
+    rc = lib().gs_raster_fwd(C.byref(cfg), C.c_int32(len(cams)), cams, _ptr(isect_vals, torch.int32),
+                             _ptr(tile_ranges, torch.int64), _ptr(means2d, torch.float32), _ptr(conics, torch.float32),
+                             _ptr(opacities, torch.float32), _ptr(rgbs, torch.float32), _bg(bg),
+                             _ptr(image, torch.float32), _ptr(final_T, torch.float32), _ptr(n_contrib, torch.int32),
+                             _stream(stream))
+    _check(rc, "gs_raster_fwd")
+
+
+def gs_raster_bwd(cfg, cams, N_total, isect_vals, tile_ranges, means2d, conics, opacities, rgbs, bg, final_T, n_contrib,
+                  dL_dimage, radii, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs, stream=None):
+    import torch
+    rc = lib().gs_raster_bwd(C.byref(cfg), C.c_int32(len(cams)), cams, C.c_int64(N_total), _ptr(isect_vals, torch.int32),
+                             _ptr(tile_ranges, torch.int64), _ptr(means2d, torch.float32), _ptr(conics, torch.float32),
+                             _ptr(opacities, torch.float32), _ptr(rgbs, torch.float32), _bg(bg),
+                             _ptr(final_T, torch.float32), _ptr(n_contrib, torch.int32), _ptr(dL_dimage, torch.float32),
+                             _ptr(radii, torch.int32) if radii is not None else None, _ptr(dL_dmeans2d, torch.float32),
+                             _ptr(dL_dconics, torch.float32), _ptr(dL_dopacities, torch.float32),
+                             _ptr(dL_drgbs, torch.float32), _stream(stream))
+    _check(rc, "gs_raster_bwd")
+
+
+def gs_project_bwd(cfg, means, log_scales, quats, opacity_logits, sh, cams, radii, dL_dmeans2d, dL_dconics,
+                   dL_dopacities, dL_drgbs, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh,
+                   accumulate=False, stream=None):
+    import torch
+    N = means.shape[0]
+    rc = lib().gs_project_bwd(C.byref(cfg), C.c_int64(N), _ptr(means, torch.float32), _ptr(log_scales, torch.float32),
+                              _ptr(quats, torch.float32), _ptr(opacity_logits, torch.float32), _ptr(sh, torch.float32),
+                              C.c_int32(len(cams)), cams, _ptr(radii, torch.int32), _ptr(dL_dmeans2d, torch.float32),
+                              _ptr(dL_dconics, torch.float32), _ptr(dL_dopacities, torch.float32),
+                              _ptr(dL_drgbs, torch.float32), _ptr(dL_dmeans, torch.float32),
+                              _ptr(dL_dlog_scales, torch.float32), _ptr(dL_dquats, torch.float32),
+                              _ptr(dL_dopacity_logits, torch.float32), _ptr(dL_dsh, torch.float32),
+                              C.c_int32(1 if accumulate else 0), _stream(stream))
+    _check(rc, "gs_project_bwd")
+
+
+def gs_l1_loss(image, target, dL_dimage, loss_sum, stream=None):
+    import torch
+    rc = lib().gs_l1_loss(C.c_int64(image.numel()), _ptr(image, torch.float32), _ptr(target, torch.float32),
+                          _ptr(dL_dimage, torch.float32), _ptr(loss_sum, torch.float32), _stream(stream))
+    _check(rc, "gs_l1_loss")

@@ -1,0 +1,113 @@
+// common.cuh -- shared device/host helpers of the sm_100a splatting library (CUDA path only;
+// nothing here is used by, or derived from, the CPU oracle under oracle/).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "../../include/gsplat_b200.h"
+
+namespace gs {
+
+constexpr int kTile = 16;
+constexpr int kMaxCamsPerLaunch = 16;
+
+// Device-side camera: the host gs_camera plus derived constants (Jacobian clamp limits, camera
+// centre o = -W^T tau, tile grid).  Passed by value in kernel parameters (constant bank).
+struct DevCam {
+    float W[9];
+    float tau[3];
+    float fx, fy, cx, cy;
+    float near_plane, far_plane;
+    float lim_x, lim_y;
+    float ox, oy, oz;
+    int32_t width, height, gx, gy;
+};
+
+struct CamBatch {
+    DevCam cam[kMaxCamsPerLaunch];
+};
+
+inline DevCam make_devcam(const gs_camera& c) {
+    DevCam d;
+    for (int r = 0; r < 3; ++r) {
+        for (int j = 0; j < 3; ++j) d.W[3 * r + j] = c.viewmat[4 * r + j];
+        d.tau[r] = c.viewmat[4 * r + 3];
+    }
+    d.fx = c.fx; d.fy = c.fy; d.cx = c.cx; d.cy = c.cy;
+    d.near_plane = c.near_plane; d.far_plane = c.far_plane;
+    d.lim_x = 1.3f * (float)c.width / (2.0f * c.fx);
+    d.lim_y = 1.3f * (float)c.height / (2.0f * c.fy);
+    d.ox = -(d.W[0] * d.tau[0] + d.W[3] * d.tau[1] + d.W[6] * d.tau[2]);
+    d.oy = -(d.W[1] * d.tau[0] + d.W[4] * d.tau[1] + d.W[7] * d.tau[2]);
+    d.oz = -(d.W[2] * d.tau[0] + d.W[5] * d.tau[1] + d.W[8] * d.tau[2]);
+    d.width = c.width; d.height = c.height;
+    d.gx = (c.width + kTile - 1) / kTile;
+    d.gy = (c.height + kTile - 1) / kTile;
+    return d;
+}
+
+inline bool finite_f(float x) { return x == x && x - x == 0.0f; }
+
+// Validation shared by the entry points.
+inline int check_cfg(const gs_config* cfg) {
+    if (!cfg) return GS_ERR_INVALID_ARGUMENT;
+    if (cfg->sh_degree < 0 || cfg->sh_degree > 3) return GS_ERR_INVALID_ARGUMENT;
+    if (cfg->tile != kTile) return GS_ERR_UNSUPPORTED;
+    if (!finite_f(cfg->dilation) || !finite_f(cfg->alpha_min) || !finite_f(cfg->alpha_max) ||
+        !finite_f(cfg->t_min) || !finite_f(cfg->extent) || !(cfg->extent > 0.0f))
+        return GS_ERR_INVALID_ARGUMENT;
+    return GS_OK;
+}
+inline int check_cams(int32_t C, const gs_camera* cams) {
+    if (!cams || C < 1 || C > GS_MAX_VIEWS) return GS_ERR_INVALID_ARGUMENT;
+    for (int c = 0; c < C; ++c) {
+        const gs_camera& k = cams[c];
+        if (k.width < 1 || k.height < 1 || k.width > 65536 || k.height > 65536) return GS_ERR_INVALID_ARGUMENT;
+        if (k.width != cams[0].width || k.height != cams[0].height) return GS_ERR_INVALID_ARGUMENT;
+        if (!finite_f(k.fx) || !finite_f(k.fy) || !finite_f(k.cx) || !finite_f(k.cy) || !(k.fx > 0.0f) || !(k.fy > 0.0f))
+            return GS_ERR_INVALID_ARGUMENT;
+        for (int j = 0; j < 12; ++j)
+            if (!finite_f(k.viewmat[j])) return GS_ERR_INVALID_ARGUMENT;
+        if (!(k.near_plane > 0.0f) || !(k.far_plane > k.near_plane)) return GS_ERR_INVALID_ARGUMENT;
+    }
+    return GS_OK;
+}
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
+
+inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? GS_OK : GS_ERR_CUDA; }
+inline int launch_status() { return cuda_status(cudaGetLastError()); }
+
+// Tile rectangle of O-P1 step 8, fp32 with one rounding per operation (no FMA contraction:
+// the same bits must come out of P1, the emit kernel and the host-side reference).
+__device__ __forceinline__ int clampi(int a, int lo, int hi) { return min(max(a, lo), hi); }
+__device__ __forceinline__ int floor_to_int_sat(float a) {
+    // __float2int_rd saturates and maps NaN to 0; clamp to +-2e9 like the definition
+    float f = floorf(a);
+    f = fminf(fmaxf(f, -2.0e9f), 2.0e9f);
+    return (int)f;
+}
+__device__ __forceinline__ void tile_rect(float u, float v, int radius, int gx, int gy, int& x0, int& x1, int& y0, int& y1) {
+    const float inv = 1.0f / (float)kTile;
+    const float r_lo = (float)radius;
+    const float r_hi = (float)(radius + kTile - 1);
+    x0 = clampi(floor_to_int_sat(__fmul_rn(__fsub_rn(u, r_lo), inv)), 0, gx);
+    x1 = clampi(floor_to_int_sat(__fmul_rn(__fadd_rn(u, r_hi), inv)), 0, gx);
+    y0 = clampi(floor_to_int_sat(__fmul_rn(__fsub_rn(v, r_lo), inv)), 0, gy);
+    y1 = clampi(floor_to_int_sat(__fmul_rn(__fadd_rn(v, r_hi), inv)), 0, gy);
+}
+
+// Real spherical-harmonic constants, degrees 0..3 (closed forms evaluated in double, rounded once).
+constexpr float kC0 = 0.28209479177387814f;   // 1/(2 sqrt(pi))
+constexpr float kC1 = 0.4886025119029199f;    // sqrt(3/(4 pi))
+constexpr float kC2a = 1.0925484305920792f;   // 1/2 sqrt(15/pi)
+constexpr float kC2b = 0.31539156525252005f;  // 1/4 sqrt(5/pi)
+constexpr float kC2c = 0.5462742152960396f;   // 1/4 sqrt(15/pi)
+constexpr float kC3a = 0.5900435899266435f;   // 1/4 sqrt(35/(2 pi))
+constexpr float kC3b = 2.890611442640554f;    // 1/2 sqrt(105/pi)
+constexpr float kC3c = 0.4570457994644658f;   // 1/4 sqrt(21/(2 pi))
+constexpr float kC3d = 0.3731763325901154f;   // 1/4 sqrt(7/pi)
+constexpr float kC3e = 1.445305721320277f;    // 1/4 sqrt(105/pi)
+
+}  // namespace gs

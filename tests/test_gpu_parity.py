@@ -1,0 +1,397 @@
+"""GPU parity tests (run with `-m gpu` on the B200 box): the CUDA path, called through the
+C ABI, against the CPU oracle on the same seeded inputs.
+
+Stage isolation (SURVEY.md §8(c) reading A17): each CUDA stage is fed the ORACLE's output of
+the previous stage, rounded to fp32 exactly as the ABI stores it, and the oracle evaluates
+the stage in double on those same fp32 inputs.  Bars (north_star): keys / ranges / values
+bit-exact; images max-abs <= 1e-4 per channel; gradients relative L2 <= 1e-3.  Pixels or
+entries whose decision (alpha >= 1/255, T' < 1e-4, ceil, floor) lies within 2e-5 (relative) of
+its threshold are "ambiguous": both outcomes are correct there, so they are compared with the
+looser bound stated in each test and counted.
+"""
+import numpy as np
+import pytest
+
+from paper_2606_11390_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+AMB_EPS = 2e-5
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_11390_b200 import binding
+    binding.lib()          # fails loudly if the extension is missing
+    return binding
+
+
+def dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda().contiguous()
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, np.float64).ravel(); b = np.asarray(b, np.float64).ravel()
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-30))
+
+
+def small_scenes():
+    """(name, scene): sizes the oracle finishes in seconds, spanning several tiles of every kernel
+    (emit tile 1024 entries, sort tile 4096 records, raster batch 256 records) with ragged tails."""
+    out = []
+    out.append(("tiny", scenes.make_scene("tiny")))
+    sc = scenes.make_scene("object", n=20_011)
+    sc["cameras"] = [scenes.make_camera(480, 270, 375.0, 375.0, np.asarray(c["viewmat"])[:, :3].T @ -np.asarray(c["viewmat"])[:, 3],
+                                        (0, 0, 0), (0, -1, 0)) for c in sc["cameras"][:3]]
+    sc["log_scales"] = sc["log_scales"] + 0.4
+    out.append(("object-small", sc))
+    sc = scenes.make_scene("room", n=30_001)
+    sc["cameras"] = [scenes.make_camera(333, 190, 260.0, 260.0, e, (5, 2, 5), (0, 1, 0))
+                     for e in [(2.5, 1.6, 2.5), (7.5, 1.6, 7.5)]]
+    sc["bg"] = np.array([0.1, 0.3, 0.2], np.float32)
+    out.append(("room-small", sc))
+    return out
+
+
+SCENES = small_scenes()
+
+
+def oracle_cfg(oracle, sc):
+    return oracle.make_cfg(sh_degree=sc["sh_degree"])
+
+
+def run_project_fwd(B, sc):
+    cams = B.make_cameras(sc["cameras"])
+    cfg = B.default_config(sh_degree=sc["sh_degree"])
+    N, C = sc["means"].shape[0], len(cams)
+    f32 = torch.float32
+    out = {"means2d": torch.zeros((C, N, 2), dtype=f32, device="cuda"), "depths": torch.zeros((C, N), dtype=f32, device="cuda"),
+           "conics": torch.zeros((C, N, 3), dtype=f32, device="cuda"), "opacities": torch.zeros((C, N), dtype=f32, device="cuda"),
+           "rgbs": torch.zeros((C, N, 3), dtype=f32, device="cuda"), "radii": torch.zeros((C, N), dtype=torch.int32, device="cuda"),
+           "tiles_touched": torch.zeros((C, N), dtype=torch.int32, device="cuda")}
+    B.gs_project_fwd(cfg, dev(sc["means"]), dev(sc["log_scales"]), dev(sc["quats"]), dev(sc["opacity_logits"]), dev(sc["sh"]),
+                     cams, out["means2d"], out["depths"], out["conics"], out["opacities"], out["rgbs"], out["radii"],
+                     out["tiles_touched"])
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+# ------------------------------------------------------------------------------------ P1
+@pytest.mark.parametrize("name,sc", SCENES, ids=[s[0] for s in SCENES])
+def test_project_fwd_parity(B, oracle, name, sc):
+    cfg = oracle_cfg(oracle, sc)
+    ref = oracle.project_fwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], sc["cameras"])
+    got = run_project_fwd(B, sc)
+    rr = ref["radius_real"]
+    # the integer radius is decided in fp32 on the GPU: entries whose 3*sqrt(lambda) lies within 1e-4
+    # (relative) of an integer may legitimately round the other way
+    amb_r = np.abs(rr - np.round(rr)) <= 1e-4 * np.maximum(rr, 1.0)
+    # the tile rectangle is decided from the fp32 mean: ambiguous when a bound is within 1e-3 px of a tile edge
+    u = ref["means2d"]
+    r = ref["radii"].astype(np.float64)[..., None]
+    lo, hi = (u - r) / 16.0, (u + r + 15.0) / 16.0
+    near_edge = (np.abs(lo - np.round(lo)) < 1e-4) | (np.abs(hi - np.round(hi)) < 1e-4)
+    amb_t = near_edge.any(axis=-1) | amb_r
+    vis_ref, vis_got = ref["radii"] > 0, got["radii"] > 0
+    bad_vis = (vis_ref != vis_got) & ~amb_t
+    assert not bad_vis.any(), f"{bad_vis.sum()} visibility mismatches"
+    both = vis_ref & vis_got
+    assert both.sum() > 0.2 * vis_ref.size or name != "tiny"
+    dr = (got["radii"] != ref["radii"]) & both
+    assert not (dr & ~amb_r).any(), "radius mismatch away from a rounding boundary"
+    assert np.all(np.abs(got["radii"][dr] - ref["radii"][dr]) <= 1)
+    dt = (got["tiles_touched"].astype(np.int64) != ref["tiles_touched"].astype(np.int64)) & both
+    assert not (dt & ~amb_t).any(), "tiles_touched mismatch away from a tile edge"
+    stats = {}
+    m = both
+    err_u = np.abs(got["means2d"][m] - ref["means2d"][m])
+    assert np.all(err_u <= 2e-6 * np.abs(ref["means2d"][m]) + 2e-4), err_u.max()
+    np.testing.assert_allclose(got["depths"][m], ref["depths"][m], rtol=3e-6)
+    # conic: error relative to the largest entry of that Gaussian's conic
+    cn = np.abs(ref["conics"][m]).max(axis=-1, keepdims=True)
+    err_c = np.abs(got["conics"][m] - ref["conics"][m]) / cn
+    assert err_c.max() <= 2e-4, err_c.max()
+    np.testing.assert_allclose(got["opacities"][m], ref["opacities"][m], rtol=2e-6)
+    assert np.abs(got["rgbs"][m] - ref["rgbs"][m]).max() <= 5e-6
+    print(f"[{name}] visible {both.sum()} radius-ambiguous {int((dr).sum())} tile-ambiguous {int(dt.sum())} "
+          f"max err mean2d {err_u.max():.2e} conic(rel) {err_c.max():.2e}")
+
+
+# ------------------------------------------------------------------------------------ B1..B4
+def oracle_stage1(oracle, sc):
+    cfg = oracle_cfg(oracle, sc)
+    pf = oracle.project_fwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], sc["cameras"])
+    rec = {k: pf[k].astype(np.float32) for k in ("means2d", "depths", "conics", "opacities", "rgbs")}
+    return cfg, pf, rec
+
+
+def run_bin(B, sc, rec, radii, capacity=None, sync=True):
+    cams = B.make_cameras(sc["cameras"])
+    cfg = B.default_config(sh_degree=sc["sh_degree"])
+    C, N = radii.shape
+    gx, gy = B.grid_of(cams)
+    cap = int(capacity if capacity is not None else 1 << 20)
+    keys = torch.zeros((cap,), dtype=torch.int64, device="cuda")
+    vals = torch.zeros((cap,), dtype=torch.int32, device="cuda")
+    ranges = torch.full((C * gx * gy, 2), -1, dtype=torch.int64, device="cuda")
+    ws = torch.empty((B.gs_bin_tiles_workspace_bytes(cfg, N, cams, cap),), dtype=torch.uint8, device="cuda")
+    M_dev = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+    M = B.gs_bin_tiles(cfg, N, cams, dev(rec["means2d"]), dev(rec["depths"]), dev(radii), ws, cap, keys, vals, ranges, M_dev, sync)
+    torch.cuda.synchronize()
+    return M, int(M_dev.item()), keys.cpu().numpy().view(np.uint64), vals.cpu().numpy(), ranges.cpu().numpy()
+
+
+@pytest.mark.parametrize("name,sc", SCENES, ids=[s[0] for s in SCENES])
+def test_bin_tiles_bit_exact(B, oracle, name, sc):
+    """north_star: "tile keys and per-tile ranges bit-exact when built from the oracle's projected
+    means and radii" -- and, because the emit is index-ordered, the values too."""
+    cfg, pf, rec = oracle_stage1(oracle, sc)
+    keys, vals, ranges = oracle.bin_tiles(cfg, sc["cameras"], rec["means2d"], rec["depths"], pf["radii"])
+    M, M_dev, gk, gv, gr = run_bin(B, sc, rec, pf["radii"], capacity=len(keys) + 1000)
+    assert M == len(keys) == M_dev
+    np.testing.assert_array_equal(gk[:M], keys)
+    np.testing.assert_array_equal(gv[:M], vals)
+    np.testing.assert_array_equal(gr, ranges)
+    # same call without the host synchronisation
+    M2, M_dev2, gk2, gv2, gr2 = run_bin(B, sc, rec, pf["radii"], capacity=len(keys), sync=False)
+    assert M2 is None and M_dev2 == len(keys)
+    np.testing.assert_array_equal(gk2[:M], keys)
+    np.testing.assert_array_equal(gv2[:M], vals)
+    np.testing.assert_array_equal(gr2, ranges)
+    print(f"[{name}] M = {M}")
+
+
+def test_bin_tiles_edge_cases(B, oracle):
+    name, sc = SCENES[1]
+    cfg, pf, rec = oracle_stage1(oracle, sc)
+    keys, vals, ranges = oracle.bin_tiles(cfg, sc["cameras"], rec["means2d"], rec["depths"], pf["radii"])
+    # capacity too small: error status carries the needed size, nothing is written out of bounds
+    with pytest.raises(B.GsError) as ei:
+        run_bin(B, sc, rec, pf["radii"], capacity=len(keys) // 3)
+    assert ei.value.status == B.GS_ERR_CAPACITY and ei.value.needed == len(keys)
+    # everything culled -> M = 0, all ranges [0, 0)
+    zero = np.zeros_like(pf["radii"])
+    M, M_dev, gk, gv, gr = run_bin(B, sc, rec, zero, capacity=128)
+    assert M == 0 and M_dev == 0 and np.all(gr == 0)
+    # a single visible entry, last index of the last view
+    one = zero.copy()
+    idx = np.argwhere(pf["radii"][-1] > 0)[-1][0]
+    one[-1, idx] = pf["radii"][-1, idx]
+    k1, v1, r1 = oracle.bin_tiles(cfg, sc["cameras"], rec["means2d"], rec["depths"], one)
+    M, M_dev, gk, gv, gr = run_bin(B, sc, rec, one, capacity=max(len(k1), 1))
+    assert M == len(k1)
+    np.testing.assert_array_equal(gk[:M], k1); np.testing.assert_array_equal(gv[:M], v1); np.testing.assert_array_equal(gr, r1)
+
+
+def test_bin_tiles_whole_screen_splat_and_depth_ties(B, oracle):
+    """A Gaussian covering every tile (largest per-entry record count) plus exact depth ties."""
+    cams = [scenes.make_camera(640, 360, 500.0, 500.0, (0, 0, -3), (0, 0, 0), (0, -1, 0))] * 2
+    sc = {"cameras": cams, "sh_degree": 0}
+    rng = np.random.default_rng(0)
+    N = 3000
+    m2d = np.stack([rng.uniform(-50, 690, (2, N)), rng.uniform(-50, 410, (2, N))], axis=-1).astype(np.float32)
+    dep = rng.choice(np.linspace(0.5, 9.0, 40).astype(np.float32), size=(2, N))        # many exact ties
+    rad = rng.integers(0, 40, (2, N)).astype(np.int32)
+    rad[0, 17] = 5000; rad[1, 2999] = 100000
+    cfg = oracle.make_cfg(sh_degree=0)
+    keys, vals, ranges = oracle.bin_tiles(cfg, cams, m2d, dep, rad)
+    M, M_dev, gk, gv, gr = run_bin(B, sc, {"means2d": m2d, "depths": dep}, rad, capacity=len(keys))
+    assert M == len(keys)
+    np.testing.assert_array_equal(gk[:M], keys)
+    np.testing.assert_array_equal(gv[:M], vals)
+    np.testing.assert_array_equal(gr, ranges)
+
+
+@pytest.mark.parametrize("n,end_bit,skip", [(1, 64, 0), (255, 40, 1), (4096, 64, 0), (4097, 47, 1), (100_003, 64, 0),
+                                            (1_000_000, 49, 1), (3_000_001, 33, 1)])
+def test_sort_pairs_matches_stable_library_sort(B, n, end_bit, skip):
+    """B3 alone against numpy's stable sort on the sorted bit range; sizes around the 4096-key tile."""
+    rng = np.random.default_rng(n)
+    keys = rng.integers(0, 2 ** 63, n, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, n, dtype=np.uint64)
+    mask = np.uint64((1 << end_bit) - 1 if end_bit < 64 else 0xFFFFFFFFFFFFFFFF)
+    if skip:
+        mask &= ~np.uint64(1 << 31)
+    keys &= mask
+    if n > 1000:
+        keys[rng.integers(0, n, n // 3)] = keys[rng.integers(0, n, n // 3)]      # duplicates: stability matters
+    vals = np.arange(n, dtype=np.int32)
+    order = np.argsort(keys, kind="stable")
+    ws = torch.empty((B.gs_sort_pairs_workspace_bytes(n),), dtype=torch.uint8, device="cuda")
+    dk, dv = dev(keys.view(np.int64)), dev(vals)
+    B.gs_sort_pairs(n, end_bit, skip, dk, dv, ws)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(dk.cpu().numpy().view(np.uint64), keys[order])
+    np.testing.assert_array_equal(dv.cpu().numpy(), vals[order])
+
+
+# ------------------------------------------------------------------------------------ R1
+def oracle_stage2(oracle, sc):
+    cfg, pf, rec = oracle_stage1(oracle, sc)
+    keys, vals, ranges = oracle.bin_tiles(cfg, sc["cameras"], rec["means2d"], rec["depths"], pf["radii"])
+    return cfg, pf, rec, vals, ranges
+
+
+def run_raster_fwd(B, sc, rec, vals, ranges):
+    cams = B.make_cameras(sc["cameras"])
+    cfg = B.default_config(sh_degree=sc["sh_degree"])
+    C = len(cams); H, W = cams[0].height, cams[0].width
+    img = torch.full((C, H, W, 3), -1.0, dtype=torch.float32, device="cuda")
+    T = torch.full((C, H, W), -1.0, dtype=torch.float32, device="cuda")
+    nc = torch.full((C, H, W), -1, dtype=torch.int32, device="cuda")
+    dv = dev(vals) if len(vals) else torch.zeros((1,), dtype=torch.int32, device="cuda")
+    B.gs_raster_fwd(cfg, cams, dv, dev(ranges), dev(rec["means2d"]), dev(rec["conics"]), dev(rec["opacities"]),
+                    dev(rec["rgbs"]), sc["bg"], img, T, nc)
+    torch.cuda.synchronize()
+    return img.cpu().numpy(), T.cpu().numpy(), nc.cpu().numpy()
+
+
+@pytest.mark.parametrize("name,sc", SCENES, ids=[s[0] for s in SCENES])
+def test_raster_fwd_parity(B, oracle, name, sc):
+    cfg, pf, rec, vals, ranges = oracle_stage2(oracle, sc)
+    img, T, nc, amb = oracle.raster_fwd(cfg, sc["cameras"], vals, ranges, rec["means2d"], rec["conics"], rec["opacities"],
+                                        rec["rgbs"], sc["bg"], ambiguity_eps=AMB_EPS)
+    gi, gT, gn = run_raster_fwd(B, sc, rec, vals, ranges)
+    clear = amb == 0
+    err = np.abs(gi - img).max(axis=-1)
+    assert err[clear].max() <= 1e-4, err[clear].max()             # north_star: max-abs 1e-4 per channel in fp32
+    assert np.abs(gT - T)[clear].max() <= 1e-4
+    assert np.array_equal(gn[clear], nc[clear])
+    # ambiguous pixels: one flipped decision is worth at most ~alpha_min * |rgb| (or the last composited term)
+    if (~clear).any():
+        assert err[~clear].max() <= 2e-2
+    assert clear.mean() > 0.995
+    print(f"[{name}] max err {err[clear].max():.2e}; ambiguous pixels {int((~clear).sum())} of {clear.size}, "
+          f"max err there {err[~clear].max() if (~clear).any() else 0:.2e}")
+
+
+def test_raster_fwd_empty_and_background(B, oracle):
+    name, sc = SCENES[0]
+    sc = dict(sc); sc["bg"] = np.array([0.25, 0.5, 0.75], np.float32)
+    cfg, pf, rec, vals, ranges = oracle_stage2(oracle, sc)
+    gi, gT, gn = run_raster_fwd(B, sc, rec, np.zeros((0,), np.int32), np.zeros_like(ranges))
+    assert np.all(gi == sc["bg"][None, None, None, :]) and np.all(gT == 1.0) and np.all(gn == 0)
+
+
+# ------------------------------------------------------------------------------------ R2
+def run_raster_bwd(B, sc, rec, vals, ranges, final_T, n_contrib, dL, radii=None):
+    cams = B.make_cameras(sc["cameras"])
+    cfg = B.default_config(sh_degree=sc["sh_degree"])
+    C, N = rec["opacities"].shape
+    g = {"means2d": torch.full((C, N, 2), 7.0, dtype=torch.float32, device="cuda"),
+         "conics": torch.full((C, N, 3), 7.0, dtype=torch.float32, device="cuda"),
+         "opacities": torch.full((C, N), 7.0, dtype=torch.float32, device="cuda"),
+         "rgbs": torch.full((C, N, 3), 7.0, dtype=torch.float32, device="cuda")}
+    B.gs_raster_bwd(cfg, cams, C * N, dev(vals), dev(ranges), dev(rec["means2d"]), dev(rec["conics"]), dev(rec["opacities"]),
+                    dev(rec["rgbs"]), sc["bg"], dev(final_T, torch.float32), dev(n_contrib), dev(dL, torch.float32),
+                    dev(radii) if radii is not None else None, g["means2d"], g["conics"], g["opacities"], g["rgbs"])
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in g.items()}
+
+
+@pytest.mark.parametrize("name,sc", SCENES, ids=[s[0] for s in SCENES])
+def test_raster_bwd_parity(B, oracle, name, sc):
+    cfg, pf, rec, vals, ranges = oracle_stage2(oracle, sc)
+    img, T, nc = oracle.raster_fwd(cfg, sc["cameras"], vals, ranges, rec["means2d"], rec["conics"], rec["opacities"],
+                                   rec["rgbs"], sc["bg"])
+    rng = np.random.default_rng(3)
+    dL = (rng.standard_normal(img.shape) / img[0].size).astype(np.float32)
+    T32 = T.astype(np.float32)
+    ref = oracle.raster_bwd(cfg, sc["cameras"], vals, ranges, rec["means2d"], rec["conics"], rec["opacities"], rec["rgbs"],
+                            sc["bg"], T32, nc, dL)
+    for radii in (None, pf["radii"]):
+        got = run_raster_bwd(B, sc, rec, vals, ranges, T32, nc, dL, radii)
+        vis = pf["radii"] > 0
+        for k in ref:
+            e = rel_l2(got[k][vis], ref[k][vis])
+            assert e <= 1e-3, (k, e)                                  # north_star: relative L2 1e-3
+            if radii is None:
+                assert np.all(got[k][~vis] == 0)                     # dense zero-fill
+            else:
+                assert np.all(got[k][~vis] == 7.0)                   # culled rows untouched
+        print(f"[{name}] rel L2: " + ", ".join(f"{k} {rel_l2(got[k][vis], ref[k][vis]):.1e}" for k in ref))
+
+
+# ------------------------------------------------------------------------------------ P5
+def run_project_bwd(B, sc, radii, g2, accumulate=False, init=None):
+    cams = B.make_cameras(sc["cameras"])
+    cfg = B.default_config(sh_degree=sc["sh_degree"])
+    N = sc["means"].shape[0]
+    K = (sc["sh_degree"] + 1) ** 2
+    shapes = {"means": (N, 3), "log_scales": (N, 3), "quats": (N, 4), "opacity_logits": (N,), "sh": (N, K, 3)}
+    out = {k: torch.full(s, 3.0 if init is None else init, dtype=torch.float32, device="cuda") for k, s in shapes.items()}
+    B.gs_project_bwd(cfg, dev(sc["means"]), dev(sc["log_scales"]), dev(sc["quats"]), dev(sc["opacity_logits"]), dev(sc["sh"]),
+                     cams, dev(radii), dev(g2["means2d"], torch.float32), dev(g2["conics"], torch.float32),
+                     dev(g2["opacities"], torch.float32), dev(g2["rgbs"], torch.float32), out["means"], out["log_scales"],
+                     out["quats"], out["opacity_logits"], out["sh"], accumulate)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+@pytest.mark.parametrize("name,sc", SCENES, ids=[s[0] for s in SCENES])
+def test_project_bwd_parity(B, oracle, name, sc):
+    cfg, pf, rec, vals, ranges = oracle_stage2(oracle, sc)
+    rng = np.random.default_rng(4)
+    vis = pf["radii"] > 0
+    g2 = {"means2d": rng.standard_normal(rec["means2d"].shape).astype(np.float32),
+          "conics": rng.standard_normal(rec["conics"].shape).astype(np.float32),
+          "opacities": rng.standard_normal(rec["opacities"].shape).astype(np.float32),
+          "rgbs": rng.standard_normal(rec["rgbs"].shape).astype(np.float32)}
+    for k in g2:      # rows of culled entries hold garbage on purpose: they must never be read
+        g2[k][~vis] = np.nan
+    g2z = {k: np.nan_to_num(v, nan=0.0) for k, v in g2.items()}
+    ref = oracle.project_bwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], sc["cameras"],
+                             pf["radii"], g2z["means2d"], g2z["conics"], g2z["opacities"], g2z["rgbs"])
+    got = run_project_bwd(B, sc, pf["radii"], g2)
+    anyvis = vis.any(axis=0)
+    for k in ref:
+        assert np.isfinite(got[k]).all(), k
+        e = rel_l2(got[k], ref[k])
+        assert e <= 1e-3, (k, e)
+        assert np.all(got[k][~anyvis] == 0)                          # accumulate = 0 overwrites every row
+    acc = run_project_bwd(B, sc, pf["radii"], g2, accumulate=True, init=3.0)
+    for k in ref:
+        assert rel_l2(acc[k][anyvis] - 3.0, ref[k][anyvis]) <= 2e-3
+        assert np.all(acc[k][~anyvis] == 3.0)                        # accumulate = 1 leaves invisible rows alone
+    print(f"[{name}] rel L2: " + ", ".join(f"{k} {rel_l2(got[k], ref[k]):.1e}" for k in ref))
+
+
+# ------------------------------------------------------------------------------------ whole pipeline
+@pytest.mark.parametrize("name,sc", SCENES, ids=[s[0] for s in SCENES])
+def test_end_to_end_step_against_oracle(B, oracle, name, sc):
+    """All CUDA stages chained (as bench.py runs them) against the oracle chained the same way."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    cfg = oracle_cfg(oracle, sc)
+    tgt = scenes.target_image(sc)
+    st = SplatStep(sc)
+    st.set_target(tgt)
+    st.step(sync=True)
+    torch.cuda.synchronize()
+    r = oracle.render(cfg, sc, ambiguity_eps=AMB_EPS)
+    assert st.M == len(r["keys"]) or abs(st.M - len(r["keys"])) <= 1e-3 * len(r["keys"])
+    gi = st.image.cpu().numpy()
+    clear = r["ambiguous"] == 0
+    err = np.abs(gi - r["image"]).max(axis=-1)
+    # chained stages differ from the oracle by fp32 rounding of the projected records (not only of the
+    # compositing), so a few pixels sit on flipped decisions; the bulk must be at the 1e-4 bar
+    frac_bad = (err[clear] > 1e-4).mean()
+    assert frac_bad <= 2e-3, frac_bad
+    assert np.median(err) <= 2e-6
+    # gradients of the L1 loss
+    diff = r["image"] - tgt.astype(np.float64)
+    dL = (np.sign(diff) / diff.size)
+    g2 = oracle.raster_bwd(cfg, sc["cameras"], r["vals"], r["ranges"], r["rec"]["means2d"], r["rec"]["conics"],
+                           r["rec"]["opacities"], r["rec"]["rgbs"], sc["bg"], r["final_T"].astype(np.float32), r["n_contrib"], dL)
+    gp = oracle.project_bwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], sc["cameras"],
+                            r["proj"]["radii"], g2["means2d"], g2["conics"], g2["opacities"], g2["rgbs"])
+    loss_ref = np.abs(diff).mean()
+    assert abs(float(st.loss.item()) - loss_ref) <= 1e-5 * max(loss_ref, 1e-3)
+    errs = {k: rel_l2(st.grads[k].cpu().numpy(), gp[k]) for k in gp}
+    print(f"[{name}] M {st.M} image err>1e-4 frac {frac_bad:.2e}; grad rel L2 {errs}")
+    for k, e in errs.items():
+        assert e <= 1e-3, (k, e)

@@ -1,17 +1,27 @@
 // raster.cu -- per-pixel stages R1 (gs_raster_fwd) and R2 (gs_raster_bwd) plus the harness L1 loss.
 //
-// One 16x16 thread block per (view, tile).  The tile's sorted records are staged through shared
-// memory in batches of 256 (one gathered record per thread), every thread then walks the batch for
-// its pixel.  Forward: a warp leaves the batch loop as soon as all of its 32 pixels are saturated and
-// the block stops fetching when every warp has.  Backward: back-to-front from
-// the tile's largest n_contrib, per-record partial sums are reduced inside the warp with a
-// value-splitting butterfly (14 shuffles for 9 values), combined across the block's warps in shared
-// memory and flushed with one device-scope atomic per value and record.
+// One 256-thread block per (view, tile); each of its 8 warps owns an 8x4 pixel block of the 16x16
+// tile (lane = pixel).  The tile's sorted records are staged through shared memory in batches of 256
+// (one gathered record per thread, conic pre-scaled to the log2 domain).  Only ~1/4 of the (pixel,
+// record) pairs of a tile list pass the alpha >= alpha_min rule, so before evaluating anything a
+// warp FILTERS the batch: lane l bounds record (chunk*32 + l) over the warp's 8x4 pixel rectangle
+// (exact maximum of the concave exponent over the rectangle, conservative margin) and a ballot
+// gives the records that can contribute; the warp then walks only those bits.  The filter never
+// changes a per-pixel decision, it only skips records for which every pixel would be skipped.
+// Forward: a warp stops when all its pixels are saturated, the block stops fetching when every warp
+// has.  Backward: back to front from the tile's largest n_contrib; the 9
+// partial sums of a record are reduced inside the warp with a value-splitting butterfly (14
+// shuffles), written to the warp's own shared-memory slot (shared-memory float atomics are CAS loops
+// on this hardware), summed across the 8 warps at the end of the batch and flushed with one
+// device-scope red.add per value and (tile, record).
 #include "common.cuh"
 
 namespace gs {
 
 constexpr int kBlock = kTile * kTile;  // 256
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+constexpr float kFilterMargin = 0.01f;  // log2 units: a record is dropped only if alpha < 0.993 alpha_min everywhere
 
 struct RasterArgs {
     int32_t width, height, gx, gy;
@@ -20,25 +30,98 @@ struct RasterArgs {
     const float* means2d; const float* conics; const float* opacities; const float* rgbs;
     float bg0, bg1, bg2;
     float alpha_min, alpha_max, t_min;
+    float filter_thr;      // log2(alpha_min) - margin (-inf when alpha_min <= 0)
 };
 
 struct RasterFwdOut {
     float* image; float* final_T; int32_t* n_contrib;
 };
 
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// scaled exponent e(dx,dy) = A' dx^2 + B' dx dy + C' dy^2  (= power * log2(e))
+__device__ __forceinline__ float quad_form(float A, float B, float C, float dx, float dy) {
+    const float t = fmaf(B, dy, A * dx);
+    return fmaf(C * dy, dy, t * dx);
+}
+
+// Can the record contribute to any pixel centre of the rectangle [X0, X0+7] x [Y0, Y0+3]?
+// g0 = (u, v, A', B'), g1.x = C', g1.y = log2(opacity).  Exact maximum of the concave exponent over
+// the rectangle (inside -> 0, otherwise on the edge(s) facing the mean), compared with a margin.
+__device__ __forceinline__ bool rect_may_contribute(const float4 g0, const float4 g1, float X0, float Y0, float thr) {
+    const float A = g0.z, B = g0.w, C = g1.x;
+    const float dx0 = g0.x - (X0 + 7.0f), dx1 = g0.x - X0;
+    const float dy0 = g0.y - (Y0 + 3.0f), dy1 = g0.y - Y0;
+    const bool inx = (dx0 <= 0.0f) && (dx1 >= 0.0f), iny = (dy0 <= 0.0f) && (dy1 >= 0.0f);
+    const bool concave = (A <= 0.0f) && (C <= 0.0f) && (4.0f * A * C - B * B >= 0.0f);
+    float emax = 0.0f;
+    if (!(inx && iny)) {
+        emax = -3.0e38f;
+        if (!inx) {
+            const float dxe = dx0 > 0.0f ? dx0 : dx1;
+            const float dys = fminf(fmaxf(-B * dxe / (2.0f * C), dy0), dy1);
+            emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxe, dys), fmaxf(quad_form(A, B, C, dxe, dy0), quad_form(A, B, C, dxe, dy1))));
+        }
+        if (!iny) {
+            const float dye = dy0 > 0.0f ? dy0 : dy1;
+            const float dxs = fminf(fmaxf(-B * dye / (2.0f * A), dx0), dx1);
+            emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxs, dye), fmaxf(quad_form(A, B, C, dx0, dye), quad_form(A, B, C, dx1, dye))));
+        }
+    }
+    return !concave || !(emax + g1.y < thr);
+}
+
+// One staged record: 48 bytes of shared memory, conic in the log2 domain.
+struct __align__(16) Rec {
+    float4 a;   // u, v, A', B'
+    float4 b;   // C', log2(opacity), r, g
+    float4 c;   // b, opacity, bit pattern of the entry id, unused
+};
+
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
+// gather one record and stage it in the log2 domain
+__device__ __forceinline__ void stage_record(const RasterArgs& a, int g, Rec& r) {
+    const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + g);
+    const float A = __ldg(a.conics + 3 * (int64_t)g), B = __ldg(a.conics + 3 * (int64_t)g + 1), Cc = __ldg(a.conics + 3 * (int64_t)g + 2);
+    const float op = __ldg(a.opacities + g);
+    r.a = make_float4(uv.x, uv.y, -0.5f * kLog2e * A, -kLog2e * B);
+    r.b = make_float4(-0.5f * kLog2e * Cc, __log2f(op), __ldg(a.rgbs + 3 * (int64_t)g), __ldg(a.rgbs + 3 * (int64_t)g + 1));
+    r.c = make_float4(__ldg(a.rgbs + 3 * (int64_t)g + 2), op, __int_as_float(g), 0.0f);
+}
+
 __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, const RasterFwdOut o) {
-    __shared__ float4 s_geo[kBlock];   // u, v, A, B
-    __shared__ float4 s_col[kBlock];   // C, opacity, r, g
-    __shared__ float s_b[kBlock];      // b
-    const int tid = threadIdx.x;
+    __shared__ Rec s_rec[kBlock];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t bt = blockIdx.x;                  // view * tiles + tile
     const int64_t view = bt / a.tiles;
     const int t = (int)(bt - view * a.tiles);
     const int ty = t / a.gx, tx = t - ty * a.gx;
-    const int j = tx * kTile + (tid & (kTile - 1));
-    const int i = ty * kTile + (tid >> 4);
+    const int bx0 = tx * kTile + (warp & 1) * 8, by0 = ty * kTile + (warp >> 1) * 4;   // the warp's 8x4 pixel block
+    const int j = bx0 + (lane & 7), i = by0 + (lane >> 3);
     const bool inside = (i < a.height) && (j < a.width);
     const float px = (float)j + 0.5f, py = (float)i + 0.5f;
+    const float X0 = (float)bx0 + 0.5f, Y0 = (float)by0 + 0.5f;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_rec);
+    const float alpha_min = a.alpha_min, alpha_max = a.alpha_max, t_min = a.t_min;
 
     const int64_t start = __ldg(a.ranges + 2 * bt), end = __ldg(a.ranges + 2 * bt + 1);
     float T = 1.0f, c0 = 0.f, c1 = 0.f, c2 = 0.f;
@@ -47,33 +130,37 @@ __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, 
     for (int64_t base = start; base < end; base += kBlock) {
         if (__syncthreads_and(done)) break;
         const int64_t k = base + tid;
-        if (k < end) {
-            const int g = __ldg(a.vals + k);
-            const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + g);
-            const float A = __ldg(a.conics + 3 * (int64_t)g), B = __ldg(a.conics + 3 * (int64_t)g + 1), Cc = __ldg(a.conics + 3 * (int64_t)g + 2);
-            s_geo[tid] = make_float4(uv.x, uv.y, A, B);
-            s_col[tid] = make_float4(Cc, __ldg(a.opacities + g), __ldg(a.rgbs + 3 * (int64_t)g), __ldg(a.rgbs + 3 * (int64_t)g + 1));
-            s_b[tid] = __ldg(a.rgbs + 3 * (int64_t)g + 2);
-        }
+        if (k < end) stage_record(a, __ldg(a.vals + k), s_rec[tid]);
         __syncthreads();
         const int cnt = (int)((end - base) < kBlock ? (end - base) : kBlock);
-        const int nbase = (int)(base - start);
-        for (int q = 0; q < cnt && !done; ++q) {
-            const float4 ge = s_geo[q];
-            const float4 co = s_col[q];
-            const float dx = ge.x - px, dy = ge.y - py;
-            const float power = -0.5f * (ge.z * dx * dx + co.x * dy * dy) - ge.w * dx * dy;
-            if (power > 0.0f) continue;
-            const float alpha = fminf(a.alpha_max, co.y * __expf(power));
-            if (alpha < a.alpha_min) continue;
-            const float Tn = T * (1.0f - alpha);
-            if (Tn < a.t_min) { done = true; break; }
-            const float wgt = alpha * T;
-            c0 = fmaf(co.z, wgt, c0);
-            c1 = fmaf(co.w, wgt, c1);
-            c2 = fmaf(s_b[q], wgt, c2);
-            T = Tn;
-            last = nbase + q + 1;
+        const int nbase = (int)(base - start) + 1;
+        bool warp_done = __all_sync(0xffffffffu, done);
+        for (int ch = 0; ch * 32 < cnt && !warp_done; ++ch) {
+            const int r = ch * 32 + lane;
+            unsigned int mask = __ballot_sync(0xffffffffu, r < cnt && rect_may_contribute(s_rec[r].a, s_rec[r].b, X0, Y0, a.filter_thr));
+            while (mask) {
+                const int q = ch * 32 + __ffs(mask) - 1;
+                mask &= mask - 1;
+                const uint32_t addr = sbase + (uint32_t)q * (uint32_t)sizeof(Rec);
+                const float4 ga = lds128(addr);
+                const float4 gb = lds128(addr + 16);
+                const float bl = lds32(addr + 32);
+                const float dx = ga.x - px, dy = ga.y - py;
+                const float e = quad_form(ga.z, ga.w, gb.x, dx, dy);
+                const float alpha = fminf(alpha_max, ex2_approx(e + gb.y));
+                const float Tn = T * (1.0f - alpha);
+                const bool ok = !done && !(e > 0.0f) && !(alpha < alpha_min);
+                const bool term = ok && (Tn < t_min);
+                const bool upd = ok && !term;
+                const float wgt = upd ? alpha * T : 0.0f;
+                c0 = fmaf(gb.z, wgt, c0);
+                c1 = fmaf(gb.w, wgt, c1);
+                c2 = fmaf(bl, wgt, c2);
+                T = upd ? Tn : T;
+                last = upd ? nbase + q : last;
+                done = done || term;
+                if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
+            }
         }
     }
     if (inside) {
@@ -129,23 +216,33 @@ __device__ __forceinline__ void warp_reduce9(const float v[9], int lane, float& 
     out9 = w;
 }
 
+constexpr int kBwdBatch = 128;              // records staged per batch in the backward kernel
+constexpr int kBwdChunks = kBwdBatch / 32;
+constexpr int kWarps = kBlock / 32;
+
+struct BwdSmem {
+    Rec rec[kBwdBatch];
+    float slot[kWarps][kBwdBatch][9];       // per-warp partial sums of a record: du, dv, dA, dB, dC, o*do, dr, dg, db
+    unsigned int vis[kWarps][kBwdChunks];   // which records of the batch a warp wrote
+    int max_contrib;
+};
+
 __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, const RasterBwdIO io) {
-    __shared__ float4 s_geo[kBlock];   // u, v, A, B
-    __shared__ float4 s_col[kBlock];   // C, opacity, r, g
-    __shared__ float s_b[kBlock];
-    __shared__ int s_id[kBlock];
-    __shared__ float s_acc[kBlock][9]; // per record: du, dv, dA, dB, dC, do, dr, dg | db
-    __shared__ int s_max;
-    const int tid = threadIdx.x, lane = tid & 31;
+    extern __shared__ __align__(16) unsigned char bwd_smem_raw[];
+    BwdSmem& sm = *reinterpret_cast<BwdSmem*>(bwd_smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t bt = blockIdx.x;
     const int64_t view = bt / a.tiles;
     const int t = (int)(bt - view * a.tiles);
     const int ty = t / a.gx, tx = t - ty * a.gx;
-    const int j = tx * kTile + (tid & (kTile - 1));
-    const int i = ty * kTile + (tid >> 4);
+    const int bx0 = tx * kTile + (warp & 1) * 8, by0 = ty * kTile + (warp >> 1) * 4;
+    const int j = bx0 + (lane & 7), i = by0 + (lane >> 3);
     const bool inside = (i < a.height) && (j < a.width);
     const float px = (float)j + 0.5f, py = (float)i + 0.5f;
+    const float X0 = (float)bx0 + 0.5f, Y0 = (float)by0 + 0.5f;
     const int64_t start = __ldg(a.ranges + 2 * bt);
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.rec);
+    const float alpha_min = a.alpha_min, alpha_max = a.alpha_max;
 
     float T = 0.f, g0 = 0.f, g1 = 0.f, g2 = 0.f;
     int ncon = 0;
@@ -155,90 +252,99 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
         ncon = __ldg(io.n_contrib + pix);
         g0 = __ldg(io.dL_dimage + 3 * pix); g1 = __ldg(io.dL_dimage + 3 * pix + 1); g2 = __ldg(io.dL_dimage + 3 * pix + 2);
     }
-    if (tid == 0) s_max = 0;
+    if (tid == 0) sm.max_contrib = 0;
     __syncthreads();
-    {
-        int m = ncon;
+    int wmax = ncon;
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, d));
-        if (lane == 0 && m > 0) atomicMax(&s_max, m);
-    }
+    for (int d = 16; d > 0; d >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, d));
+    if (lane == 0 && wmax > 0) atomicMax(&sm.max_contrib, wmax);
     __syncthreads();
-    const int maxn = s_max;
+    const int maxn = sm.max_contrib;
     if (maxn == 0) return;
     // colour accumulated behind the current record
     float S0 = a.bg0, S1 = a.bg1, S2 = a.bg2;
-    const int nb = (maxn + kBlock - 1) / kBlock;
+    const int nb = (maxn + kBwdBatch - 1) / kBwdBatch;
     for (int b = nb - 1; b >= 0; --b) {
-        const int cnt = min(kBlock, maxn - b * kBlock);
+        const int cnt = min(kBwdBatch, maxn - b * kBwdBatch);
         __syncthreads();   // previous batch fully flushed
-        if (tid < cnt) {
-            const int g = __ldg(a.vals + start + (int64_t)b * kBlock + tid);
-            const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + g);
-            const float A = __ldg(a.conics + 3 * (int64_t)g), B = __ldg(a.conics + 3 * (int64_t)g + 1), Cc = __ldg(a.conics + 3 * (int64_t)g + 2);
-            s_geo[tid] = make_float4(uv.x, uv.y, A, B);
-            s_col[tid] = make_float4(Cc, __ldg(a.opacities + g), __ldg(a.rgbs + 3 * (int64_t)g), __ldg(a.rgbs + 3 * (int64_t)g + 1));
-            s_b[tid] = __ldg(a.rgbs + 3 * (int64_t)g + 2);
-            s_id[tid] = g;
-        }
-#pragma unroll
-        for (int k = 0; k < 9; ++k) s_acc[tid][k] = 0.f;
+        if (tid < cnt) stage_record(a, __ldg(a.vals + start + (int64_t)b * kBwdBatch + tid), sm.rec[tid]);
         __syncthreads();
-        for (int q = cnt - 1; q >= 0; --q) {
-            const int idx = b * kBlock + q;           // position of the record in the tile's list
-            bool valid = idx < ncon;
-            float v[9];
-#pragma unroll
-            for (int k = 0; k < 9; ++k) v[k] = 0.f;
-            if (valid) {
-                const float4 ge = s_geo[q];
-                const float4 co = s_col[q];
-                const float dx = ge.x - px, dy = ge.y - py;
-                const float power = -0.5f * (ge.z * dx * dx + co.x * dy * dy) - ge.w * dx * dy;
-                const float G = __expf(power);
-                const float raw = co.y * G;
-                const float alpha = fminf(a.alpha_max, raw);
-                valid = (power <= 0.0f) && (alpha >= a.alpha_min);
-                if (valid) {
-                    const float cb = s_b[q];
-                    T = T / (1.0f - alpha);          // transmittance in front of this record
-                    const float wgt = alpha * T;
-                    v[6] = wgt * g0; v[7] = wgt * g1; v[8] = wgt * g2;
-                    const float dL_dalpha = T * ((co.z - S0) * g0 + (co.w - S1) * g1 + (cb - S2) * g2);
-                    S0 = alpha * co.z + (1.0f - alpha) * S0;
-                    S1 = alpha * co.w + (1.0f - alpha) * S1;
-                    S2 = alpha * cb + (1.0f - alpha) * S2;
-                    if (!(raw > a.alpha_max)) {       // no gradient through the alpha_max clamp
-                        v[5] = G * dL_dalpha;
-                        const float gp = alpha * dL_dalpha;
-                        v[2] = -0.5f * dx * dx * gp;
-                        v[3] = -dx * dy * gp;
-                        v[4] = -0.5f * dy * dy * gp;
-                        v[0] = -(ge.z * dx + ge.w * dy) * gp;
-                        v[1] = -(ge.w * dx + co.x * dy) * gp;
-                    }
-                }
-            }
-            if (__any_sync(0xffffffffu, valid)) {
+        for (int ch = kBwdChunks - 1; ch >= 0; --ch) {
+            const int r = ch * 32 + lane;
+            unsigned int mask = __ballot_sync(0xffffffffu, r < cnt && (b * kBwdBatch + r) < wmax &&
+                                                               rect_may_contribute(sm.rec[r].a, sm.rec[r].b, X0, Y0, a.filter_thr));
+            unsigned int written = 0;
+            while (mask) {
+                const int bit = 31 - __clz(mask);
+                mask ^= 1u << bit;
+                const int q = ch * 32 + bit;
+                const int idx = b * kBwdBatch + q;           // position of the record in the tile's list
+                const uint32_t addr = sbase + (uint32_t)q * (uint32_t)sizeof(Rec);
+                const float4 ga = lds128(addr);
+                const float4 gb = lds128(addr + 16);
+                const float dx = ga.x - px, dy = ga.y - py;
+                const float e = quad_form(ga.z, ga.w, gb.x, dx, dy);
+                const float raw = ex2_approx(e + gb.y);
+                const float alpha = fminf(alpha_max, raw);
+                const bool valid = (idx < ncon) && !(e > 0.0f) && !(alpha < alpha_min);
+                if (!__any_sync(0xffffffffu, valid)) continue;
+                const float cb = lds32(addr + 32);
+                float v[9];
+                // quantities of an invalid lane are computed but selected away
+                const float Tf = T * rcp_approx(1.0f - alpha);   // transmittance in front of this record
+                const float wgt = valid ? alpha * Tf : 0.0f;
+                v[6] = wgt * g0; v[7] = wgt * g1; v[8] = wgt * g2;
+                const float d0 = gb.z - S0, d1 = gb.w - S1, d2 = cb - S2;
+                const float dL_dalpha = Tf * (d0 * g0 + d1 * g1 + d2 * g2);
+                const float am = valid ? alpha : 0.0f;
+                S0 = fmaf(am, d0, S0);
+                S1 = fmaf(am, d1, S1);
+                S2 = fmaf(am, d2, S2);
+                T = valid ? Tf : T;
+                // no gradient through the alpha_max clamp
+                const float gp = (valid && !(raw > alpha_max)) ? alpha * dL_dalpha : 0.0f;   // dL/dpower
+                v[5] = gp;                                       // = o * dL/do  (divided by o at the flush)
+                const float hx = dx * gp, hy = dy * gp;
+                v[2] = -0.5f * dx * hx;
+                v[3] = -dx * hy;
+                v[4] = -0.5f * dy * hy;
+                const float gs = gp * kLn2;                      // A dx + B dy = -(2A' dx + B' dy) ln 2
+                v[0] = fmaf(2.0f * ga.z, dx, ga.w * dy) * gs;
+                v[1] = fmaf(2.0f * gb.x, dy, ga.w * dx) * gs;
                 float r8, r9;
                 warp_reduce9(v, lane, r8, r9);
-                if ((lane & 3) == 0) atomicAdd(&s_acc[q][lane >> 2], r8);
-                if (lane == 1) atomicAdd(&s_acc[q][8], r9);
+                float* slot = &sm.slot[warp][q][0];
+                if ((lane & 3) == 0) slot[lane >> 2] = r8;
+                if (lane == 1) slot[8] = r9;
+                written |= 1u << bit;
             }
+            if (lane == 0) sm.vis[warp][ch] = written;
         }
         __syncthreads();
         if (tid < cnt) {
-            const int64_t g = s_id[tid];
-            const float* acc = s_acc[tid];
-            if (acc[0] != 0.f) atomicAdd(io.g_means2d + 2 * g, acc[0]);
-            if (acc[1] != 0.f) atomicAdd(io.g_means2d + 2 * g + 1, acc[1]);
-            if (acc[2] != 0.f) atomicAdd(io.g_conics + 3 * g, acc[2]);
-            if (acc[3] != 0.f) atomicAdd(io.g_conics + 3 * g + 1, acc[3]);
-            if (acc[4] != 0.f) atomicAdd(io.g_conics + 3 * g + 2, acc[4]);
-            if (acc[5] != 0.f) atomicAdd(io.g_opacities + g, acc[5]);
-            if (acc[6] != 0.f) atomicAdd(io.g_rgbs + 3 * g, acc[6]);
-            if (acc[7] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 1, acc[7]);
-            if (acc[8] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 2, acc[8]);
+            float acc[9];
+#pragma unroll
+            for (int k = 0; k < 9; ++k) acc[k] = 0.f;
+            bool any = false;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w)
+                if ((sm.vis[w][tid >> 5] >> (tid & 31)) & 1u) {
+                    any = true;
+#pragma unroll
+                    for (int k = 0; k < 9; ++k) acc[k] += sm.slot[w][tid][k];
+                }
+            if (any) {
+                const int64_t g = __float_as_int(sm.rec[tid].c.z);
+                if (acc[0] != 0.f) atomicAdd(io.g_means2d + 2 * g, acc[0]);
+                if (acc[1] != 0.f) atomicAdd(io.g_means2d + 2 * g + 1, acc[1]);
+                if (acc[2] != 0.f) atomicAdd(io.g_conics + 3 * g, acc[2]);
+                if (acc[3] != 0.f) atomicAdd(io.g_conics + 3 * g + 1, acc[3]);
+                if (acc[4] != 0.f) atomicAdd(io.g_conics + 3 * g + 2, acc[4]);
+                if (acc[5] != 0.f) atomicAdd(io.g_opacities + g, acc[5] / sm.rec[tid].c.y);
+                if (acc[6] != 0.f) atomicAdd(io.g_rgbs + 3 * g, acc[6]);
+                if (acc[7] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 1, acc[7]);
+                if (acc[8] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 2, acc[8]);
+            }
         }
     }
 }
@@ -290,6 +396,7 @@ static int fill_args(const gs_config* cfg, int32_t C, const gs_camera* cams, con
     a.vals = vals; a.ranges = ranges; a.means2d = means2d; a.conics = conics; a.opacities = opacities; a.rgbs = rgbs;
     a.bg0 = bg[0]; a.bg1 = bg[1]; a.bg2 = bg[2];
     a.alpha_min = cfg->alpha_min; a.alpha_max = cfg->alpha_max; a.t_min = cfg->t_min;
+    a.filter_thr = cfg->alpha_min > 0.0f ? log2f(cfg->alpha_min) - kFilterMargin : -3.0e38f;
     return GS_OK;
 }
 
@@ -336,7 +443,13 @@ extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* c
         }
     }
     RasterBwdIO io{final_T, n_contrib, dL_dimage, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs};
-    raster_bwd_kernel<<<(unsigned)(C * a.tiles), kBlock, 0, st>>>(a, io);
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(raster_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BwdSmem)) != cudaSuccess)
+            return GS_ERR_CUDA;
+        attr_set = true;
+    }
+    raster_bwd_kernel<<<(unsigned)(C * a.tiles), kBlock, sizeof(BwdSmem), st>>>(a, io);
     return launch_status();
 }
 

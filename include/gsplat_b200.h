@@ -81,8 +81,10 @@ int gs_project_fwd(const gs_config* cfg /*host*/, int64_t N, const float* means,
  * For every entry e = c*N + i with radii[e] > 0, in ascending e, one record per overlapped 16x16
  * tile (tile rectangle recomputed in fp32 from means2d and radii exactly as in P1 step 8):
  *   key = (uint64)(c*tiles + ty*Gx + tx) << 32 | bit pattern of depths[e],  value = e.
- * Records are stably radix-sorted by key (equal keys keep ascending e), and tile_ranges[t] =
+ * Records are put in stable key order (equal keys keep ascending e), and tile_ranges[t] =
  * [first, last+1) of the records whose key >> 32 == t ([0,0) when none), t in [0, C*tiles).
+ * The order is produced by two stable radix sorts (depth bits on the visible entries, then the
+ * tile id on the records), which is the same order as one stable sort on the 64-bit key.
  * workspace == NULL: only *workspace_bytes (host) is written (size query for N, C, capacity_M).
  * capacity_M: number of records isect_keys / isect_vals can hold.
  * M_dev (device, optional): receives the total record count M.
@@ -90,7 +92,9 @@ int gs_project_fwd(const gs_config* cfg /*host*/, int64_t N, const float* means,
  *   GS_ERR_CAPACITY when M > capacity_M (outputs are then incomplete but nothing is written
  *   out of bounds).  With M_out == NULL the call never synchronises; overflow is reported only
  *   through M_dev.
- * isect_keys[capacity_M] (uint64), isect_vals[capacity_M] (int32), tile_ranges[C*tiles,2] (int64). */
+ * isect_keys[capacity_M] (uint64, optional: NULL = the sorted keys are not materialised; the
+ * rasteriser reads only values and ranges), isect_vals[capacity_M] (int32),
+ * tile_ranges[C*tiles,2] (int64).  depths must be positive (they are: depth > near > 0). */
 int gs_bin_tiles(const gs_config* cfg /*host*/, int64_t N, int32_t C, const gs_camera* cams /*host*/,
                  const float* means2d, const float* depths, const int32_t* radii, void* workspace,
                  size_t* workspace_bytes /*host*/, int64_t capacity_M, uint64_t* isect_keys,

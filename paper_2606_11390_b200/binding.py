@@ -135,14 +135,16 @@ def gs_bin_tiles_workspace_bytes(cfg, N, cams, capacity_M):
 
 def gs_bin_tiles(cfg, N, cams, means2d, depths, radii, workspace, capacity_M, isect_keys, isect_vals, tile_ranges,
                  M_dev=None, sync=True, stream=None):
-    """Returns M (host int) when ``sync`` is true, else None (M is then only in ``M_dev``).
+    """``isect_keys`` may be None (the 64-bit keys are then not materialised).
+    Returns M (host int) when ``sync`` is true, else None (M is then only in ``M_dev``).
     Raises GsError(GS_ERR_CAPACITY) with ``.needed`` set when capacity_M is too small."""
     import torch
     wb = C.c_size_t(workspace.numel() * workspace.element_size())
     m = C.c_int64(0)
     rc = lib().gs_bin_tiles(C.byref(cfg), C.c_int64(N), C.c_int32(len(cams)), cams, _ptr(means2d, torch.float32),
                             _ptr(depths, torch.float32), _ptr(radii, torch.int32), _ptr(workspace), C.byref(wb),
-                            C.c_int64(capacity_M), _ptr(isect_keys), _ptr(isect_vals, torch.int32),
+                            C.c_int64(capacity_M), _ptr(isect_keys) if isect_keys is not None else None,
+                            _ptr(isect_vals, torch.int32),
                             _ptr(tile_ranges, torch.int64), _ptr(M_dev, torch.int64) if M_dev is not None else None,
                             C.byref(m) if sync else None, _stream(stream))
     if rc == GS_ERR_CAPACITY:

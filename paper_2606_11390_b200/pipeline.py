@@ -17,7 +17,9 @@ from . import binding as B
 class SplatStep:
     """Device-resident state for a batch of C views of one scene."""
 
-    def __init__(self, scene, device="cuda:0", capacity_M=None, upload=True):
+    def __init__(self, scene, device="cuda:0", capacity_M=None, upload=True, want_keys=False):
+        # want_keys: also materialise the sorted 64-bit (tile | depth) keys; no later stage reads them
+        self.want_keys = bool(want_keys)
         self.device = torch.device(device)
         self.scene_name = scene.get("name", "")
         self.cams_host = scene["cameras"]
@@ -70,7 +72,8 @@ class SplatStep:
     def _alloc_isect(self, capacity_M):
         self.capacity_M = int(capacity_M)
         d = self.device
-        self.isect_keys = torch.empty((self.capacity_M,), dtype=torch.int64, device=d)   # uint64 bit patterns
+        self.isect_keys = (torch.empty((self.capacity_M,), dtype=torch.int64, device=d)   # uint64 bit patterns
+                           if self.want_keys else None)
         self.isect_vals = torch.empty((self.capacity_M,), dtype=torch.int32, device=d)
         nbytes = B.gs_bin_tiles_workspace_bytes(self.cfg, self.N, self.cams, self.capacity_M)
         self.workspace = torch.empty((nbytes,), dtype=torch.uint8, device=d)
@@ -135,9 +138,11 @@ class SplatStep:
         self.l1_loss()
         self.backward()
 
-    # launches of this library's kernels in one step (memsets excluded): P1, emit, hist, P sort passes,
-    # ranges, R1, L1, zero rows, R2, P5
+    # launches of this library's kernels in one step (memsets excluded): P1, compact, depth-sort
+    # histogram + passes, emit, histogram scan, tile-sort passes, ranges (+ keys), R1, L1, zero rows, R2, P5
     def launches_per_step(self):
         tile_bits = max(1, int(np.ceil(np.log2(self.C * self.gx * self.gy))))
-        passes = 4 + (tile_bits + 7) // 8
-        return 1 + 1 + 1 + passes + 1 + 1 + 1 + 1 + 1 + 1
+        view_bits = int(np.ceil(np.log2(self.C))) if self.C > 1 else 0
+        depth_passes = 4 + (view_bits + 7) // 8
+        tile_passes = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
+        return 1 + 1 + 1 + depth_passes + 1 + 1 + tile_passes + 1 + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

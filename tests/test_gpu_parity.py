@@ -43,7 +43,7 @@ def rel_l2(a, b):
 
 def small_scenes():
     """(name, scene): sizes the oracle finishes in seconds, spanning several tiles of every kernel
-    (emit tile 1024 entries, sort tile 4096 records, raster batch 256 records) with ragged tails."""
+    (compact/emit tile 1024 entries, sort tiles 4096 records, raster batch 256 records) with ragged tails."""
     out = []
     out.append(("tiny", scenes.make_scene("tiny")))
     sc = scenes.make_scene("object", n=20_011)
@@ -131,7 +131,7 @@ def oracle_stage1(oracle, sc):
     return cfg, pf, rec
 
 
-def run_bin(B, sc, rec, radii, capacity=None, sync=True):
+def run_bin(B, sc, rec, radii, capacity=None, sync=True, want_keys=True):
     cams = B.make_cameras(sc["cameras"])
     cfg = B.default_config(sh_degree=sc["sh_degree"])
     C, N = radii.shape
@@ -142,7 +142,8 @@ def run_bin(B, sc, rec, radii, capacity=None, sync=True):
     ranges = torch.full((C * gx * gy, 2), -1, dtype=torch.int64, device="cuda")
     ws = torch.empty((B.gs_bin_tiles_workspace_bytes(cfg, N, cams, cap),), dtype=torch.uint8, device="cuda")
     M_dev = torch.full((1,), -1, dtype=torch.int64, device="cuda")
-    M = B.gs_bin_tiles(cfg, N, cams, dev(rec["means2d"]), dev(rec["depths"]), dev(radii), ws, cap, keys, vals, ranges, M_dev, sync)
+    M = B.gs_bin_tiles(cfg, N, cams, dev(rec["means2d"]), dev(rec["depths"]), dev(radii), ws, cap, keys if want_keys else None,
+                       vals, ranges, M_dev, sync)
     torch.cuda.synchronize()
     return M, int(M_dev.item()), keys.cpu().numpy().view(np.uint64), vals.cpu().numpy(), ranges.cpu().numpy()
 
@@ -164,6 +165,11 @@ def test_bin_tiles_bit_exact(B, oracle, name, sc):
     np.testing.assert_array_equal(gk2[:M], keys)
     np.testing.assert_array_equal(gv2[:M], vals)
     np.testing.assert_array_equal(gr2, ranges)
+    # keys not requested (as the pipeline calls it): values and ranges unchanged, key buffer untouched
+    M3, M_dev3, gk3, gv3, gr3 = run_bin(B, sc, rec, pf["radii"], capacity=len(keys) + 7, want_keys=False)
+    assert M3 == len(keys) and not gk3.any()
+    np.testing.assert_array_equal(gv3[:M], vals)
+    np.testing.assert_array_equal(gr3, ranges)
     print(f"[{name}] M = {M}")
 
 
@@ -203,6 +209,26 @@ def test_bin_tiles_whole_screen_splat_and_depth_ties(B, oracle):
     keys, vals, ranges = oracle.bin_tiles(cfg, cams, m2d, dep, rad)
     M, M_dev, gk, gv, gr = run_bin(B, sc, {"means2d": m2d, "depths": dep}, rad, capacity=len(keys))
     assert M == len(keys)
+    np.testing.assert_array_equal(gk[:M], keys)
+    np.testing.assert_array_equal(gv[:M], vals)
+    np.testing.assert_array_equal(gr, ranges)
+
+
+@pytest.mark.parametrize("W,H,C", [(3840, 2160, 4), (8192, 8192, 2), (4000, 33, 3)])
+def test_bin_tiles_tile_sort_pass_plans(B, oracle, W, H, C):
+    """Tile-id widths of 17 bits (2 passes of 9 bits), 19 bits (3 passes) and 10 bits (2 narrow passes)."""
+    cams = [scenes.make_camera(W, H, 1000.0, 1000.0, (0, 0, -3), (0, 0, 0), (0, -1, 0))] * C
+    sc = {"cameras": cams, "sh_degree": 0}
+    rng = np.random.default_rng(W + C)
+    N = 5000
+    m2d = np.stack([rng.uniform(-100, W + 100, (C, N)), rng.uniform(-100, H + 100, (C, N))], axis=-1).astype(np.float32)
+    dep = rng.uniform(0.3, 50.0, (C, N)).astype(np.float32)
+    dep[:, ::7] = dep[:, 1::7][:, : dep[:, ::7].shape[1]]                    # some exact ties
+    rad = rng.integers(0, 120, (C, N)).astype(np.int32)
+    cfg = oracle.make_cfg(sh_degree=0)
+    keys, vals, ranges = oracle.bin_tiles(cfg, cams, m2d, dep, rad)
+    M, M_dev, gk, gv, gr = run_bin(B, sc, {"means2d": m2d, "depths": dep}, rad, capacity=len(keys) + 3)
+    assert M == len(keys) == M_dev
     np.testing.assert_array_equal(gk[:M], keys)
     np.testing.assert_array_equal(gv[:M], vals)
     np.testing.assert_array_equal(gr, ranges)

@@ -1,27 +1,33 @@
 // binning.cu -- tile binning B1..B4 (gs_bin_tiles) and the stand-alone radix sort (gs_sort_pairs).
 //
 // The result defined by SURVEY.md 8(c) O-B is the list of (tile | depth, entry) records in stable
-// key order.  A stable sort by the 64-bit key (tile << 32 | depth) equals a stable sort by depth
-// followed by a stable sort by tile, and only the second one has to touch the M records (M is 19..80
-// times the number V of visible entries).  So the work is split in two levels:
+// key order plus the per-tile ranges.  A stable sort by the 64-bit key (tile << 32 | depth) equals a
+// stable sort by depth followed by a stable sort by tile, and only the second one has to touch the M
+// records (M is 19..80 times the number V of visible entries).  The per-tile record counts (hence the
+// ranges and every digit histogram of the tile sort) do not depend on the order at all: they follow
+// from the tile rectangles alone.  So the work is organised as
 //
-//   compact_kernel     B1a: visible entries (radius > 0, >= 1 tile) in ascending entry order ->
-//                      (view << 32 | depth bits, entry); ordered chained scan (decoupled look-back).
-//   hist_kernel +      depth sort of the V compacted entries: stable LSD radix sort on the depth bits
-//   onesweep_kernel    and the view bits (64-bit keys, 8-bit digits; also serves gs_sort_pairs).
-//   emit_kernel        B1b+B2: per-entry tile counts scanned in DEPTH order (ordered chained scan), one
-//                      (32-bit tile id, entry) record per overlapped tile, written warp-cooperatively;
-//                      the digit histograms of the tile sort are accumulated on the fly.
-//   scan_hist_kernel   exclusive scan of those histograms -> global digit bases.
-//   tile_sweep_kernel  B3: stable LSD radix sort of the M records on the tile id only: 2 passes of 8 or
-//                      9 bits for every BASELINE configuration (one read + one write of 8 bytes per
-//                      record and pass), persistent blocks, per-digit decoupled look-back.
-//   ranges_kernel      B4: per-tile [start, end) from the sorted tile ids.
-//   keys_kernel        optional: the 64-bit keys (tile << 32 | depth bits) of the sorted records.
+//   compact_kernel      B1a: visible entries (radius > 0, >= 1 tile) in ascending entry order ->
+//                       (view << 32 | depth bits, entry), ordered chained scan (decoupled look-back);
+//                       each rectangle also adds +1/-1 at its four corners of a per-view difference grid.
+//   tile_yscan_kernel,  B4: 2-D prefix sum of the difference grid = records per tile; exclusive scan
+//   tile_xscan_kernel,  over the tiles = tile_ranges; the same pass accumulates the digit histograms of
+//   tile_ranges_kernel  the tile sort and the total record count M.
+//   hist_kernel +       depth sort of the V compacted entries: stable LSD radix sort on the depth bits
+//   onesweep_kernel     and the view bits (64-bit keys, 8-bit digits; also serves gs_sort_pairs).
+//   offsets_kernel      B1b: per-entry tile counts scanned in DEPTH order -> record offset, first tile
+//                       id, rectangle width and entry id (16 bytes per visible entry), plus the first
+//                       entry of every chunk (one sort tile, 8192 records) of the record list.
+//   tile_sweep_kernel   B2+B3: stable LSD radix sort of the M records on the 32-bit tile id, 2 passes
+//                       of 8 or 9 bits for every BASELINE configuration.  The first pass GENERATES its
+//                       chunk of records from the entry table (the unsorted record list is never
+//                       written to memory), the last pass writes only the values.  Persistent blocks,
+//                       per-digit decoupled look-back, ballot-based stable ranking.
+//   keys_kernel         optional: the 64-bit keys (tile << 32 | depth bits) of the sorted records.
 //
 // Equal (tile, depth) records keep ascending entry order (reading A10) because every step is
-// order-preserving: index-ordered compaction, stable depth sort, depth-ordered emit, stable tile sort.
-// The counts V and M live in device memory; no stage needs the host.
+// order-preserving: index-ordered compaction, stable depth sort, depth-ordered generation, stable
+// tile sort.  The counts V and M live in device memory; no stage needs the host.
 #include "common.cuh"
 
 namespace gs {
@@ -30,21 +36,18 @@ namespace gs {
 struct BinHeader {
     unsigned long long M;          // records the batch needs (sum of tile counts of all visible entries)
     unsigned long long V;          // visible entries (clamped to the compact capacity)
-    unsigned long long n_rec;      // records actually emitted = min(M, capacity_M)
-    unsigned long long M_acc;      // accumulator behind M
-    unsigned int compact_done;
-    unsigned int emit_ticket;
+    unsigned long long n_rec;      // records to sort = M, or 0 when M > capacity_M
+    unsigned int compact_ticket, xscan_ticket, rscan_ticket, offs_ticket;
     unsigned int sort_ticket[8];   // depth-sort passes
     unsigned int tsort_ticket[4];  // tile-sort passes
-    unsigned int compact_ticket;
-    unsigned int pad;
+    unsigned int pad[2];
 };
 static_assert(sizeof(BinHeader) == 96, "header size");
 
 constexpr int kRadix = 256;            // depth sort: 8-bit digits
 constexpr int kMaxPasses = 8;
 
-constexpr int kScanThreads = 256;      // compact / emit: 4 entries per thread
+constexpr int kScanThreads = 256;      // chained scans: 4 items per thread
 constexpr int kScanItems = 4;
 constexpr int kScanTile = kScanThreads * kScanItems;
 
@@ -55,11 +58,18 @@ constexpr int kSortTile = kSortThreads * kSortItems;
 
 constexpr int kTsThreads = 512;        // tile sort
 constexpr int kTsWarps = kTsThreads / 32;
-constexpr int kTsItems = 8;
+#ifndef GS_TS_ITEMS
+#define GS_TS_ITEMS 16
+#endif
+constexpr int kTsItems = GS_TS_ITEMS;
 constexpr int kTsTile = kTsThreads * kTsItems;
 constexpr int kTsMaxBits = 9;
 constexpr int kTsMaxBins = 1 << kTsMaxBits;
 constexpr int kTsMaxPasses = 4;
+#ifndef GS_LOOK_WIDE
+#define GS_LOOK_WIDE 1
+#endif
+constexpr int kLookWide = GS_LOOK_WIDE;   // predecessors inspected per look-back round trip
 
 struct SortPlan {
     int P;
@@ -75,37 +85,56 @@ struct TilePlan {
     unsigned int mask[kTsMaxPasses];
 };
 
+// one visible entry in depth order: where its records start, which tiles they are, whose they are
+struct __align__(16) EntryRec {
+    unsigned int off;      // offset of the entry's first record in the (virtual) unsorted record list
+    unsigned int t0;       // tile id of the rectangle's first tile (view * tiles + y0 * gx + x0)
+    unsigned int w;        // rectangle width in tiles
+    int id;                // entry e = c * N + i
+};
+
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Workspace {
-    size_t off_header, off_hist, off_thist, off_compact_status, off_emit_status, off_sort_status, off_tsort_status, zero_bytes;
-    size_t off_ckeys0, off_ckeys1, off_cvals0, off_cvals1, off_tkeys0, off_tkeys1, off_vals, total;
-    int64_t vcap;
+    size_t off_header, off_hist, off_thist, off_tdiff, off_compact_status, off_xscan_status, off_rscan_status, off_offs_status,
+        off_sort_status, off_tsort_status, zero_bytes;
+    size_t off_ckeys0, off_ckeys1, off_cvals0, off_cvals1, off_entries, off_chunk_first, off_tkeys0, off_tkeys1, off_vals, total;
+    int64_t vcap, cells, n_chunks;
 };
-static Workspace layout(int64_t n_entries, int64_t capacity) {
+static Workspace layout(int64_t n_entries, int64_t capacity, int64_t cells) {
     Workspace w;
     // every visible entry emits >= 1 record, so V <= M; a call that fits capacity has V <= capacity
     w.vcap = n_entries < capacity ? n_entries : capacity;
     if (w.vcap < 1) w.vcap = 1;
+    w.cells = cells;
+    w.n_chunks = (capacity + kTsTile - 1) / kTsTile;
     size_t o = 0;
     w.off_header = o; o += sizeof(BinHeader);
     o = align_up(o, 256);
     w.off_hist = o; o += (size_t)kMaxPasses * kRadix * sizeof(unsigned int);
     w.off_thist = o; o += (size_t)kTsMaxPasses * kTsMaxBins * sizeof(unsigned int);
     o = align_up(o, 256);
+    w.off_tdiff = o; o += (size_t)(cells + kScanTile) * sizeof(int);
+    o = align_up(o, 256);
     w.off_compact_status = o; o += (size_t)((n_entries + kScanTile - 1) / kScanTile + 1) * sizeof(unsigned long long);
     o = align_up(o, 256);
-    w.off_emit_status = o; o += (size_t)((w.vcap + kScanTile - 1) / kScanTile + 1) * sizeof(unsigned long long);
+    w.off_xscan_status = o; o += (size_t)((cells + kScanTile - 1) / kScanTile + 1) * sizeof(unsigned long long);
+    o = align_up(o, 256);
+    w.off_rscan_status = o; o += (size_t)((cells + kScanTile - 1) / kScanTile + 1) * sizeof(unsigned long long);
+    o = align_up(o, 256);
+    w.off_offs_status = o; o += (size_t)((w.vcap + kScanTile - 1) / kScanTile + 1) * sizeof(unsigned long long);
     o = align_up(o, 256);
     w.off_sort_status = o; o += (size_t)((w.vcap + kSortTile - 1) / kSortTile + 1) * kRadix * sizeof(unsigned long long);
     o = align_up(o, 256);
-    w.off_tsort_status = o; o += (size_t)((capacity + kTsTile - 1) / kTsTile + 1) * kTsMaxBins * sizeof(unsigned long long);
+    w.off_tsort_status = o; o += (size_t)(w.n_chunks + 1) * kTsMaxBins * sizeof(unsigned long long);
     o = align_up(o, 256);
     w.zero_bytes = o;  // everything up to here is cleared at the start of a call
     w.off_ckeys0 = o; o += (size_t)w.vcap * sizeof(uint64_t); o = align_up(o, 256);
     w.off_ckeys1 = o; o += (size_t)w.vcap * sizeof(uint64_t); o = align_up(o, 256);
     w.off_cvals0 = o; o += (size_t)w.vcap * sizeof(int32_t); o = align_up(o, 256);
     w.off_cvals1 = o; o += (size_t)w.vcap * sizeof(int32_t); o = align_up(o, 256);
+    w.off_entries = o; o += (size_t)w.vcap * sizeof(EntryRec); o = align_up(o, 256);
+    w.off_chunk_first = o; o += (size_t)(w.n_chunks + 2) * sizeof(unsigned int); o = align_up(o, 256);
     w.off_tkeys0 = o; o += (size_t)capacity * sizeof(uint32_t); o = align_up(o, 256);
     w.off_tkeys1 = o; o += (size_t)capacity * sizeof(uint32_t); o = align_up(o, 256);
     w.off_vals = o; o += (size_t)capacity * sizeof(int32_t); o = align_up(o, 256);
@@ -176,15 +205,16 @@ constexpr unsigned long long kValMask = (1ull << 62) - 1ull;
 
 // Ordered chained scan step (warp 0 of a block): publish this block's total, look back over the
 // preceding blocks (32 at a time) until an inclusive prefix is found, publish the own inclusive
-// prefix, return the exclusive one.  `tile` is the block's position in ticket order.
+// prefix, return the exclusive one.  `tile` is the block's position in ticket order.  Sums are taken
+// modulo 2^62 (callers that scan signed values truncate the result to 32 bits).
 __device__ __forceinline__ unsigned long long chained_scan_lookback(unsigned long long* status, int64_t tile,
                                                                      unsigned long long block_total, int lane) {
     unsigned long long excl = 0;
     if (tile == 0) {
-        if (lane == 0) st_volatile_u64(status, kFlagIncl | block_total);
+        if (lane == 0) st_volatile_u64(status, kFlagIncl | (block_total & kValMask));
         return 0;
     }
-    if (lane == 0) st_volatile_u64(status + tile, kFlagAgg | block_total);
+    if (lane == 0) st_volatile_u64(status + tile, kFlagAgg | (block_total & kValMask));
     int64_t look = tile - 1;
     while (true) {
         const int64_t idx = look - lane;
@@ -204,8 +234,42 @@ __device__ __forceinline__ unsigned long long chained_scan_lookback(unsigned lon
         if (incl) break;
         look -= 32;
     }
-    if (lane == 0) st_volatile_u64(status + tile, kFlagIncl | (excl + block_total));
+    if (lane == 0) st_volatile_u64(status + tile, kFlagIncl | ((excl + block_total) & kValMask));
     return excl;
+}
+
+// Block-wide part of an ordered chained scan: every thread passes the sum of its items, gets the
+// global exclusive prefix of that sum; `block_total` and `block_excl` are returned to all threads.
+struct ChainScanSmem {
+    unsigned long long warp_sum[kScanThreads / 32];
+    unsigned long long base;
+};
+__device__ __forceinline__ unsigned long long block_chained_scan(unsigned long long thread_sum, unsigned long long* status, int64_t tile,
+                                                                   ChainScanSmem& sm, unsigned long long& block_excl,
+                                                                   unsigned long long& block_total) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    unsigned long long inc = thread_sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned long long o = shfl_up_u64(inc, d);
+        if (lane >= d) inc += o;
+    }
+    if (lane == 31) sm.warp_sum[warp] = inc;
+    __syncthreads();
+    unsigned long long wbase = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) {
+        if (w < warp) wbase += sm.warp_sum[w];
+        total += sm.warp_sum[w];
+    }
+    if (warp == 0) {
+        const unsigned long long excl = chained_scan_lookback(status, tile, total, lane);
+        if (lane == 0) sm.base = excl;
+    }
+    __syncthreads();
+    block_excl = sm.base;
+    block_total = total;
+    return sm.base + wbase + inc - thread_sum;
 }
 
 // ------------------------------------------------------------------------------ B1a: compaction
@@ -216,19 +280,16 @@ struct CompactArgs {
     const float* means2d; const float* depths; const int32_t* radii;
     int64_t vcap;
     unsigned long long* ckeys; int32_t* cvals;
+    int* tdiff;             // [C][gy+1][gx+1] corner differences of the tile rectangles
     BinHeader* hdr;
     unsigned long long* status;
     unsigned int n_blocks;
-    unsigned long long* M_dev;
 };
 
 __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs a) {
     __shared__ unsigned int s_ticket;
-    __shared__ unsigned long long s_base;
-    __shared__ unsigned long long s_warp_tiles[kScanThreads / 32];
-    __shared__ unsigned int s_warp_vis[kScanThreads / 32];
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    __shared__ ChainScanSmem s_scan;
+    const int tid = threadIdx.x;
     if (tid == 0) s_ticket = atomicAdd(&a.hdr->compact_ticket, 1u);
     __syncthreads();
     const int64_t tile = s_ticket;
@@ -243,71 +304,38 @@ __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs
         for (int k = 0; k < kScanItems; ++k) rad[k] = (e0 + k < a.n_entries) ? __ldg(a.radii + e0 + k) : 0;
     }
     unsigned long long key[kScanItems];
-    bool vis[kScanItems];
-    unsigned long long t_tiles = 0;
-    unsigned int t_vis = 0;
+    unsigned int vis_mask = 0, t_vis = 0;
+    const int sx = a.gx + 1, sy = a.gy + 1;
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k) {
-        vis[k] = false; key[k] = 0;
+        key[k] = 0;
         if (rad[k] > 0) {
             const int64_t e = e0 + k;
             const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + e);
             int x0, x1, y0, y1;
             tile_rect(uv.x, uv.y, rad[k], a.gx, a.gy, x0, x1, y0, y1);
-            const unsigned int cnt = (unsigned int)(x1 - x0) * (unsigned int)(y1 - y0);
-            if (cnt) {
-                const unsigned long long view = (unsigned long long)(e / a.N);
-                key[k] = (view << 32) | (unsigned long long)__float_as_uint(__ldg(a.depths + e));
-                vis[k] = true;
-                t_tiles += cnt;
+            if (x1 > x0 && y1 > y0) {
+                const int64_t view = e / a.N;
+                key[k] = ((unsigned long long)view << 32) | (unsigned long long)__float_as_uint(__ldg(a.depths + e));
+                vis_mask |= 1u << k;
                 ++t_vis;
+                int* g = a.tdiff + view * (int64_t)sx * sy;
+                atomicAdd(g + y0 * sx + x0, 1);
+                atomicAdd(g + y0 * sx + x1, -1);
+                atomicAdd(g + y1 * sx + x0, -1);
+                atomicAdd(g + y1 * sx + x1, 1);
             }
         }
     }
-    // block totals; exclusive scan of the visible count
-    unsigned int inc_v = t_vis;
-    unsigned long long sum_t = t_tiles;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const unsigned int ov = __shfl_up_sync(0xffffffffu, inc_v, d);
-        if (lane >= d) inc_v += ov;
-        sum_t += shfl_u64(sum_t, lane ^ d);
+    unsigned long long block_excl, block_total;
+    unsigned long long pos = block_chained_scan(t_vis, a.status, tile, s_scan, block_excl, block_total);
+    if (tid == 0 && tile == (int64_t)a.n_blocks - 1) {
+        const unsigned long long V = block_excl + block_total;
+        a.hdr->V = V < (unsigned long long)a.vcap ? V : (unsigned long long)a.vcap;
     }
-    if (lane == 31) { s_warp_vis[warp] = inc_v; s_warp_tiles[warp] = sum_t; }
-    __syncthreads();
-    unsigned int wbase_v = 0, block_vis = 0;
-    unsigned long long block_tiles = 0;
-#pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) {
-        if (w < warp) wbase_v += s_warp_vis[w];
-        block_vis += s_warp_vis[w];
-        block_tiles += s_warp_tiles[w];
-    }
-    if (warp == 0) {
-        const unsigned long long excl = chained_scan_lookback(a.status, tile, block_vis, lane);
-        if (lane == 0) {
-            s_base = excl;
-            // total record count: unordered sum, published by whichever block finishes last
-            atomicAdd(&a.hdr->M_acc, block_tiles);
-            __threadfence();
-            const unsigned int done = atomicAdd(&a.hdr->compact_done, 1u);
-            if (done == a.n_blocks - 1) {
-                __threadfence();
-                const unsigned long long M = ld_volatile_u64(&a.hdr->M_acc);
-                a.hdr->M = M;
-                if (a.M_dev) *a.M_dev = M;
-            }
-            if (tile == (int64_t)a.n_blocks - 1) {
-                const unsigned long long V = excl + block_vis;
-                a.hdr->V = V < (unsigned long long)a.vcap ? V : (unsigned long long)a.vcap;
-            }
-        }
-    }
-    __syncthreads();
-    unsigned long long pos = s_base + wbase_v + inc_v - t_vis;
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k)
-        if (vis[k]) {
+        if ((vis_mask >> k) & 1u) {
             if (pos < (unsigned long long)a.vcap) {
                 a.ckeys[pos] = key[k];
                 a.cvals[pos] = (int)(e0 + k);
@@ -316,156 +344,124 @@ __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs
         }
 }
 
-// ------------------------------------------------------------------------------ B1b + B2: emit
-struct EmitArgs {
-    int64_t N;
-    int32_t gx, gy;
-    unsigned int tiles;            // gx * gy
-    const float* means2d; const int32_t* radii;
-    const int32_t* cvals;          // visible entries in (view, depth, entry) order
-    int64_t capacity;
-    unsigned int* tkeys; int32_t* vals;
-    BinHeader* hdr;
-    unsigned long long* status;
-    unsigned int* thist;           // [P][kTsMaxBins]
-    TilePlan plan;
-};
-
-constexpr unsigned int kEmitBig = 2048;   // entries with more records than this are written by the whole block
-
-__device__ __forceinline__ void emit_record(const EmitArgs& a, unsigned int* s_hist, unsigned long long pos, unsigned int k,
-                                            unsigned int w, float inv_w, unsigned int t0, int id) {
-    // k -> (row, column) of the tile rectangle: reciprocal estimate, then an exact fix-up
-    unsigned int ry = (unsigned int)(((float)k + 0.5f) * inv_w);
-    int rx = (int)(k - ry * w);
-    if (rx < 0) { --ry; rx += (int)w; }
-    else if (rx >= (int)w) { ++ry; rx -= (int)w; }
-    const unsigned int t = t0 + ry * (unsigned int)a.gx + (unsigned int)rx;
-    if (pos < (unsigned long long)a.capacity) {   // records beyond the capacity are dropped (and not counted)
+// ------------------------------------------------------------------------------ B4: counts, ranges, histograms
+// column prefix sums of the difference grid (one thread per (view, column))
+__global__ void __launch_bounds__(128) tile_yscan_kernel(int* __restrict__ tdiff, int C, int gx, int gy) {
+    const int sx = gx + 1, sy = gy + 1;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= C * sx) return;
+    const int view = col / sx, x = col - view * sx;
+    int* p = tdiff + (int64_t)view * sx * sy + x;
+    int acc = 0;
+    int y = 0;
+    for (; y + 8 <= sy; y += 8) {
+        int v[8];
 #pragma unroll
-        for (int p = 0; p < kTsMaxPasses; ++p)
-            if (p < a.plan.P) atomicAdd(&s_hist[p * kTsMaxBins + ((t >> a.plan.shift[p]) & a.plan.mask[p])], 1u);
-        a.tkeys[pos] = t;
-        a.vals[pos] = id;
+        for (int k = 0; k < 8; ++k) v[k] = p[(int64_t)(y + k) * sx];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { acc += v[k]; p[(int64_t)(y + k) * sx] = acc; }
     }
+    for (; y < sy; ++y) { acc += p[(int64_t)y * sx]; p[(int64_t)y * sx] = acc; }
 }
 
-__global__ void __launch_bounds__(kScanThreads) emit_kernel(const EmitArgs a) {
+// inclusive prefix sum of the flattened grid (every padded row sums to zero, so the running sum at a
+// cell is the number of rectangles covering that tile); in place
+__global__ void __launch_bounds__(kScanThreads) tile_xscan_kernel(int* __restrict__ tdiff, int64_t cells, BinHeader* hdr,
+                                                                  unsigned long long* status) {
     __shared__ unsigned int s_ticket;
-    __shared__ unsigned long long s_base;
-    __shared__ unsigned long long s_warp_tiles[kScanThreads / 32];
-    __shared__ unsigned long long s_off[kScanTile];   // record offset of the entry within the block
-    __shared__ unsigned int s_cnt[kScanTile];
-    __shared__ unsigned int s_t0[kScanTile];          // tile id of the rectangle's first tile
-    __shared__ unsigned int s_w[kScanTile];
-    __shared__ int s_id[kScanTile];
-    __shared__ unsigned int s_big[kScanTile];
-    __shared__ unsigned int s_nbig;
-    __shared__ unsigned int s_hist[kTsMaxPasses * kTsMaxBins];
+    __shared__ ChainScanSmem s_scan;
+    const int tid = threadIdx.x;
+    if (tid == 0) s_ticket = atomicAdd(&hdr->xscan_ticket, 1u);
+    __syncthreads();
+    const int64_t tile = s_ticket;
+    const int64_t i0 = tile * kScanTile + (int64_t)tid * kScanItems;
+    // the array is padded to a multiple of the scan tile (zeros), so vector access is always in bounds
+    int4 v = *reinterpret_cast<const int4*>(tdiff + i0);
+    const int s = v.x + v.y + v.z + v.w;
+    unsigned long long be, bt;
+    const unsigned int excl = (unsigned int)block_chained_scan((unsigned long long)(long long)s, status, tile, s_scan, be, bt);
+    v.x += (int)excl; v.y += v.x; v.z += v.y; v.w += v.z;
+    if (i0 < cells) *reinterpret_cast<int4*>(tdiff + i0) = v;
+}
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// exclusive scan of the per-tile counts -> tile_ranges; digit histograms of the tile sort; M
+struct RangesArgs {
+    const int* tcount;          // flattened padded grid after both scans
+    int64_t cells;
+    int32_t C, gx, gy;
+    int64_t capacity;
+    int64_t* ranges;            // [C * gx * gy][2]
+    unsigned int* thist;        // [P][kTsMaxBins]
+    TilePlan plan;
+    BinHeader* hdr;
+    unsigned long long* status;
+    unsigned int n_blocks;
+    unsigned long long* M_dev;
+};
+
+__global__ void __launch_bounds__(kScanThreads) tile_ranges_kernel(const RangesArgs a) {
+    __shared__ unsigned int s_ticket;
+    __shared__ ChainScanSmem s_scan;
+    __shared__ unsigned int s_hist[kTsMaxPasses * kTsMaxBins];
+    const int tid = threadIdx.x;
+    if (tid == 0) s_ticket = atomicAdd(&a.hdr->rscan_ticket, 1u);
     for (int k = tid; k < a.plan.P * kTsMaxBins; k += kScanThreads) s_hist[k] = 0;
-    const unsigned long long V = a.hdr->V;
-    const int64_t n_blocks = (int64_t)((V + kScanTile - 1) / kScanTile);
-    while (true) {
-        __syncthreads();   // shared arrays of the previous tile are no longer read
-        if (tid == 0) { s_ticket = atomicAdd(&a.hdr->emit_ticket, 1u); s_nbig = 0; }
-        __syncthreads();
-        const int64_t tile = s_ticket;
-        if (tile >= n_blocks) break;
-        const int64_t j0 = tile * kScanTile + (int64_t)tid * kScanItems;
-        int id[kScanItems];
-        if (j0 + kScanItems <= (int64_t)V) {
-            const int4 v4 = __ldg(reinterpret_cast<const int4*>(a.cvals + j0));
-            id[0] = v4.x; id[1] = v4.y; id[2] = v4.z; id[3] = v4.w;
-        } else {
+    __syncthreads();
+    const int64_t tile = s_ticket;
+    const int64_t i0 = tile * kScanTile + (int64_t)tid * kScanItems;
+    const int sx = a.gx + 1, sy = a.gy + 1;
+    const int4 v4 = *reinterpret_cast<const int4*>(a.tcount + i0);
+    int cnt[kScanItems] = {v4.x, v4.y, v4.z, v4.w};
+    long long tid_of[kScanItems];
+    unsigned long long sum = 0;
 #pragma unroll
-            for (int k = 0; k < kScanItems; ++k) id[k] = (j0 + k < (int64_t)V) ? __ldg(a.cvals + j0 + k) : -1;
+    for (int k = 0; k < kScanItems; ++k) {
+        const int64_t i = i0 + k;
+        tid_of[k] = -1;
+        if (i < a.cells) {
+            const int64_t row = i / sx;
+            const int x = (int)(i - row * sx);
+            const int64_t view = row / sy;
+            const int y = (int)(row - view * sy);
+            if (x < a.gx && y < a.gy) tid_of[k] = (view * a.gy + y) * a.gx + x;
         }
-        unsigned int cnt[kScanItems], t0[kScanItems], ww[kScanItems];
-        unsigned long long t_tiles = 0;
+        if (tid_of[k] < 0) cnt[k] = 0;
+        sum += (unsigned long long)cnt[k];
+    }
+    unsigned long long be, bt;
+    unsigned long long start = block_chained_scan(sum, a.status, tile, s_scan, be, bt);
 #pragma unroll
-        for (int k = 0; k < kScanItems; ++k) {
-            cnt[k] = 0; t0[k] = 0; ww[k] = 1;
-            if (id[k] >= 0) {
-                const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + id[k]);
-                const int rad = __ldg(a.radii + id[k]);
-                int x0, x1, y0, y1;
-                tile_rect(uv.x, uv.y, rad, a.gx, a.gy, x0, x1, y0, y1);
-                ww[k] = (unsigned int)(x1 - x0);
-                cnt[k] = ww[k] * (unsigned int)(y1 - y0);
-                const unsigned int view = (unsigned int)((int64_t)id[k] / a.N);
-                t0[k] = view * a.tiles + (unsigned int)y0 * (unsigned int)a.gx + (unsigned int)x0;
-                t_tiles += cnt[k];
+    for (int k = 0; k < kScanItems; ++k) {
+        if (tid_of[k] >= 0) {
+            const bool some = cnt[k] > 0;
+            a.ranges[2 * tid_of[k]] = some ? (int64_t)start : 0;
+            a.ranges[2 * tid_of[k] + 1] = some ? (int64_t)(start + cnt[k]) : 0;
+            if (some) {
+                const unsigned int t = (unsigned int)tid_of[k];
+#pragma unroll
+                for (int p = 0; p < kTsMaxPasses; ++p)
+                    if (p < a.plan.P) atomicAdd(&s_hist[p * kTsMaxBins + ((t >> a.plan.shift[p]) & a.plan.mask[p])], (unsigned int)cnt[k]);
             }
+            start += cnt[k];
         }
-        unsigned long long inc_t = t_tiles;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned long long ot = shfl_up_u64(inc_t, d);
-            if (lane >= d) inc_t += ot;
-        }
-        if (lane == 31) s_warp_tiles[warp] = inc_t;
-        __syncthreads();
-        unsigned long long wbase_t = 0, block_tiles = 0;
-#pragma unroll
-        for (int w = 0; w < kScanThreads / 32; ++w) {
-            if (w < warp) wbase_t += s_warp_tiles[w];
-            block_tiles += s_warp_tiles[w];
-        }
-        unsigned long long off = wbase_t + inc_t - t_tiles;   // exclusive
-#pragma unroll
-        for (int k = 0; k < kScanItems; ++k) {
-            const int ci = tid * kScanItems + k;
-            s_off[ci] = off; s_cnt[ci] = cnt[k]; s_t0[ci] = t0[k]; s_w[ci] = ww[k]; s_id[ci] = id[k];
-            if (cnt[k] > kEmitBig) s_big[atomicAdd(&s_nbig, 1u)] = (unsigned int)ci;
-            off += cnt[k];
-        }
-        if (warp == 0) {
-            const unsigned long long excl = chained_scan_lookback(a.status, tile, block_tiles, lane);
-            if (lane == 0) {
-                s_base = excl;
-                if (tile == n_blocks - 1) {
-                    const unsigned long long tot = excl + block_tiles;
-                    a.hdr->n_rec = tot < (unsigned long long)a.capacity ? tot : (unsigned long long)a.capacity;
-                }
-            }
-        }
-        __syncthreads();
-        const unsigned long long base = s_base;
-        const int64_t rem = (int64_t)V - tile * kScanTile;
-        const int nvalid = (int)(rem < kScanTile ? rem : kScanTile);
-        // warp-cooperative emit: each warp takes entries round-robin, its 32 lanes write the entry's
-        // records to consecutive addresses
-        for (int j = warp; j < nvalid; j += kScanThreads / 32) {
-            const unsigned int c = s_cnt[j];
-            if (c > kEmitBig) continue;
-            const unsigned int w = s_w[j], tt0 = s_t0[j];
-            const unsigned long long o = base + s_off[j];
-            const int e = s_id[j];
-            const float inv_w = 1.0f / (float)w;
-            for (unsigned int k = lane; k < c; k += 32) emit_record(a, s_hist, o + k, k, w, inv_w, tt0, e);
-        }
-        // very large entries (whole-screen splats): the whole block writes them
-        const unsigned int nbig = s_nbig;
-        for (unsigned int b = 0; b < nbig; ++b) {
-            const int j = (int)s_big[b];
-            const unsigned int c = s_cnt[j], w = s_w[j], tt0 = s_t0[j];
-            const unsigned long long o = base + s_off[j];
-            const int e = s_id[j];
-            const float inv_w = 1.0f / (float)w;
-            for (unsigned int k = tid; k < c; k += kScanThreads) emit_record(a, s_hist, o + k, k, w, inv_w, tt0, e);
-        }
+    }
+    if (tid == 0 && tile == (int64_t)a.n_blocks - 1) {
+        const unsigned long long M = be + bt;
+        a.hdr->M = M;
+        a.hdr->n_rec = M <= (unsigned long long)a.capacity ? M : 0ull;
+        if (a.M_dev) *a.M_dev = M;
     }
     __syncthreads();
     for (int k = tid; k < a.plan.P * kTsMaxBins; k += kScanThreads) {
         const unsigned int v = s_hist[k];
-        if (v) atomicAdd(a.thist + k, v);
+        if (v) atomicAdd(a.thist + k, v);   // wraps only when M >= 2^32, i.e. far beyond the capacity limit
     }
 }
 
-// exclusive scan of the tile-sort digit histograms (one block; P * kTsMaxBins values)
-__global__ void __launch_bounds__(kTsMaxBins) scan_hist_kernel(unsigned int* thist, int P) {
+// exclusive scan of the tile-sort digit histograms (one block); when the records do not fit the
+// capacity nothing is sorted, so every range is cleared ("outputs incomplete, nothing out of bounds")
+__global__ void __launch_bounds__(kTsMaxBins) scan_hist_kernel(unsigned int* thist, int P, const BinHeader* hdr, int64_t capacity,
+                                                               int64_t* ranges, int64_t n_ranges) {
     __shared__ unsigned int s[kTsMaxBins];
     const int tid = threadIdx.x;
     for (int p = 0; p < P; ++p) {
@@ -481,6 +477,73 @@ __global__ void __launch_bounds__(kTsMaxBins) scan_hist_kernel(unsigned int* thi
         thist[p * kTsMaxBins + tid] = s[tid] - v;
         __syncthreads();
     }
+    if (hdr->M > (unsigned long long)capacity)
+        for (int64_t k = tid; k < 2 * n_ranges; k += kTsMaxBins) ranges[k] = 0;
+}
+
+// ------------------------------------------------------------------------------ B1b: entry table in depth order
+struct OffsetsArgs {
+    int64_t N;
+    int32_t gx, gy;
+    unsigned int tiles;            // gx * gy
+    const float* means2d; const int32_t* radii;
+    const int32_t* cvals;          // visible entries in (view, depth, entry) order
+    EntryRec* entries;
+    unsigned int* chunk_first;     // [n_chunks]: entry holding record c * kTsTile
+    int64_t n_chunks;
+    BinHeader* hdr;
+    unsigned long long* status;
+};
+
+__global__ void __launch_bounds__(kScanThreads) offsets_kernel(const OffsetsArgs a) {
+    __shared__ unsigned int s_ticket;
+    __shared__ ChainScanSmem s_scan;
+    const int tid = threadIdx.x;
+    const unsigned long long V = a.hdr->V;
+    const int64_t n_blocks = (int64_t)((V + kScanTile - 1) / kScanTile);
+    if (tid == 0) s_ticket = atomicAdd(&a.hdr->offs_ticket, 1u);
+    __syncthreads();
+    const int64_t tile = s_ticket;
+    if (tile >= n_blocks) return;
+    const int64_t j0 = tile * kScanTile + (int64_t)tid * kScanItems;
+    int id[kScanItems];
+    if (j0 + kScanItems <= (int64_t)V) {
+        const int4 v4 = __ldg(reinterpret_cast<const int4*>(a.cvals + j0));
+        id[0] = v4.x; id[1] = v4.y; id[2] = v4.z; id[3] = v4.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) id[k] = (j0 + k < (int64_t)V) ? __ldg(a.cvals + j0 + k) : -1;
+    }
+    unsigned int cnt[kScanItems], t0[kScanItems], ww[kScanItems];
+    unsigned long long t_tiles = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        cnt[k] = 0; t0[k] = 0; ww[k] = 1;
+        if (id[k] >= 0) {
+            const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + id[k]);
+            const int rad = __ldg(a.radii + id[k]);
+            int x0, x1, y0, y1;
+            tile_rect(uv.x, uv.y, rad, a.gx, a.gy, x0, x1, y0, y1);
+            ww[k] = (unsigned int)(x1 - x0);
+            cnt[k] = ww[k] * (unsigned int)(y1 - y0);
+            const unsigned int view = (unsigned int)((int64_t)id[k] / a.N);
+            t0[k] = view * a.tiles + (unsigned int)y0 * (unsigned int)a.gx + (unsigned int)x0;
+            t_tiles += cnt[k];
+        }
+    }
+    unsigned long long be, bt;
+    unsigned long long off = block_chained_scan(t_tiles, a.status, tile, s_scan, be, bt);
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k)
+        if (id[k] >= 0) {
+            EntryRec r;
+            r.off = (unsigned int)off; r.t0 = t0[k]; r.w = ww[k]; r.id = id[k];
+            a.entries[j0 + k] = r;
+            // chunks whose first record lies inside this entry
+            const unsigned long long c_lo = (off + kTsTile - 1) / kTsTile, c_hi = (off + cnt[k] - 1) / kTsTile;
+            for (unsigned long long c = c_lo; c <= c_hi && c < (unsigned long long)a.n_chunks; ++c) a.chunk_first[c] = (unsigned int)(j0 + k);
+            off += cnt[k];
+        }
 }
 
 // ------------------------------------------------------------------------------ histograms
@@ -651,33 +714,37 @@ __global__ void __launch_bounds__(kSortThreads) onesweep_kernel(const SweepArgs 
     }
 }
 
-// ------------------------------------------------------------------------------ B3: tile sort
+// ------------------------------------------------------------------------------ B2 + B3: tile sort
 struct TileSweepArgs {
-    const unsigned int* keys_in; const int32_t* vals_in;
-    unsigned int* keys_out; int32_t* vals_out;
+    const unsigned int* keys_in; const int32_t* vals_in;   // unused by the generating pass
+    unsigned int* keys_out; int32_t* vals_out;               // keys_out may be NULL in the last pass
     const unsigned long long* count;   // device: number of records (BinHeader::n_rec)
     int shift; unsigned int mask; int pass;
     const unsigned int* digit_base;    // [BINS] exclusive digit bases of this pass
     unsigned long long* status;        // [tiles][BINS], tag in the high word
     unsigned int* ticket;
+    // generating pass
+    const EntryRec* entries; const unsigned int* chunk_first; const unsigned long long* n_entries; int32_t gx;
 };
 
 template <int BITS>
 struct TileSweepSmem {
     static constexpr int BINS = 1 << BITS;
-    unsigned short warp_hist[kTsWarps][BINS];   // <= 256 items per warp
+    unsigned short warp_hist[kTsWarps][BINS];   // <= 32 * kTsItems items per warp
     unsigned int keys[kTsTile];
     int vals[kTsTile];
     int goff[BINS];                  // global base of the digit minus its start inside the tile
     unsigned int bin_start[BINS];
+    unsigned short head[kTsTile];    // generating pass: 1 + (entry - first entry) at the entry's first record
     unsigned int scan_tmp[kTsWarps];
-    unsigned int tile;
+    unsigned int tile, next_tile;
 };
 
-template <int BITS>
+template <int BITS, bool GEN>
 __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSweepArgs a) {
     using Smem = TileSweepSmem<BITS>;
     constexpr int BINS = Smem::BINS;
+    static_assert(kTsItems % 8 == 0, "blocked generation reads 8 heads per vector");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -688,36 +755,115 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
     const unsigned long long tag_incl = ((unsigned long long)(a.pass * 4 + 6)) << 32;
     unsigned int dbase = 0;
     if (tid < BINS) dbase = __ldg(a.digit_base + tid);
+    if (tid == 0) sm.next_tile = atomicAdd(a.ticket, 1u);
 
     while (true) {
-        __syncthreads();   // shared memory of the previous tile is no longer read
-        if (tid == 0) sm.tile = atomicAdd(a.ticket, 1u);
-        for (int k = tid; k < kTsWarps * BINS / 2; k += kTsThreads) reinterpret_cast<unsigned int*>(&sm.warp_hist[0][0])[k] = 0;
-        __syncthreads();
-        const int64_t tile = sm.tile;
+        __syncthreads();   // shared memory of the previous tile is no longer read; next_tile is visible
+        const int64_t tile = sm.next_tile;
         if (tile >= n_tiles) break;
+        for (int k = tid; k < kTsWarps * BINS / 2; k += kTsThreads) reinterpret_cast<unsigned int*>(&sm.warp_hist[0][0])[k] = 0;
+        if (GEN)
+            for (int k = tid; k < kTsTile / 2; k += kTsThreads) reinterpret_cast<unsigned int*>(sm.head)[k] = 0;
         const int64_t base = tile * kTsTile;
         const int valid = (int)((n - base) < kTsTile ? (n - base) : kTsTile);
+        __syncthreads();
+        if (tid == 0) sm.next_tile = atomicAdd(a.ticket, 1u);   // the next ticket travels while this tile is processed
 
-        // load, warp-striped: item j of lane l sits at warp*(32*items) + j*32 + l (order = (j, lane))
         unsigned int key[kTsItems];
         int val[kTsItems];
+        if (GEN) {
+            // ---- generate the chunk's records from the entry table (depth order)
+            const unsigned int j0 = __ldg(a.chunk_first + tile);
+            const unsigned int j1 = (tile + 1 < n_tiles) ? __ldg(a.chunk_first + tile + 1) : (unsigned int)(*a.n_entries - 1);
+            for (unsigned int j = j0 + tid; j <= j1; j += kTsThreads) {
+                const unsigned int off = __ldg(&a.entries[j].off);
+                const long long slot = (long long)off - (long long)base;
+                if (slot < valid) sm.head[slot > 0 ? slot : 0] = (unsigned short)(j - j0 + 1);
+            }
+            __syncthreads();
+            // blocked arrangement: thread owns kTsItems consecutive records; running maximum of the heads
+            unsigned int e_rel[kTsItems];
+            unsigned int run = 0;
 #pragma unroll
-        for (int j = 0; j < kTsItems; ++j) {
-            const int idx = warp * (32 * kTsItems) + j * 32 + lane;
-            key[j] = idx < valid ? __ldg(a.keys_in + base + idx) : 0xffffffffu;
-        }
+            for (int v8 = 0; v8 < kTsItems / 8; ++v8) {
+                const uint4 h = *reinterpret_cast<const uint4*>(&sm.head[tid * kTsItems + v8 * 8]);
+                const unsigned int hw[4] = {h.x, h.y, h.z, h.w};
 #pragma unroll
-        for (int j = 0; j < kTsItems; ++j) {
-            const int idx = warp * (32 * kTsItems) + j * 32 + lane;
-            val[j] = idx < valid ? __ldg(a.vals_in + base + idx) : 0;
+                for (int q = 0; q < 4; ++q) {
+                    run = max(run, hw[q] & 0xffffu); e_rel[v8 * 8 + 2 * q] = run;
+                    run = max(run, hw[q] >> 16); e_rel[v8 * 8 + 2 * q + 1] = run;
+                }
+            }
+            unsigned int inc = run;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) inc = max(inc, __shfl_up_sync(0xffffffffu, inc, d));
+            if (lane == 31) sm.scan_tmp[warp] = inc;
+            unsigned int carry = __shfl_up_sync(0xffffffffu, inc, 1);
+            if (lane == 0) carry = 0;
+            __syncthreads();
+#pragma unroll
+            for (int w = 0; w < kTsWarps; ++w)
+                if (w < warp) carry = max(carry, sm.scan_tmp[w]);
+            unsigned int cur = 0xffffffffu;
+            EntryRec en;
+            en.off = 0; en.t0 = 0; en.w = 1; en.id = 0;
+            float inv_w = 1.0f;
+#pragma unroll
+            for (int k = 0; k < kTsItems; ++k) {
+                const int p = tid * kTsItems + k;
+                if (p < valid) {
+                    const unsigned int er = max(carry, e_rel[k]);   // >= 1: record 0 of the chunk always has a head
+                    if (er != cur) {
+                        cur = er;
+                        const uint4 raw = __ldg(reinterpret_cast<const uint4*>(a.entries + (j0 + er - 1)));
+                        en.off = raw.x; en.t0 = raw.y; en.w = raw.z; en.id = (int)raw.w;
+                        inv_w = __frcp_rn((float)en.w);
+                    }
+                    // record index inside the entry -> (row, column) of its tile rectangle: reciprocal
+                    // estimate, then an exact fix-up
+                    const unsigned int kk = (unsigned int)(base + p) - en.off;
+                    unsigned int ry = (unsigned int)(((float)kk + 0.5f) * inv_w);
+                    int rx = (int)(kk - ry * en.w);
+                    if (rx < 0) { --ry; rx += (int)en.w; }
+                    else if (rx >= (int)en.w) { ++ry; rx -= (int)en.w; }
+                    sm.keys[p] = en.t0 + ry * (unsigned int)a.gx + (unsigned int)rx;
+                    sm.vals[p] = en.id;
+                }
+            }
+            __syncthreads();
+            // warp-striped arrangement for the ranking: item j of lane l is record warp*32*items + j*32 + l
+#pragma unroll
+            for (int j = 0; j < kTsItems; ++j) {
+                const int idx = warp * (32 * kTsItems) + j * 32 + lane;
+                key[j] = idx < valid ? sm.keys[idx] : 0xffffffffu;
+                val[j] = idx < valid ? sm.vals[idx] : 0;
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < kTsItems; ++j) {
+                const int idx = warp * (32 * kTsItems) + j * 32 + lane;
+                key[j] = idx < valid ? __ldg(a.keys_in + base + idx) : 0xffffffffu;
+            }
+#pragma unroll
+            for (int j = 0; j < kTsItems; ++j) {
+                const int idx = warp * (32 * kTsItems) + j * 32 + lane;
+                val[j] = idx < valid ? __ldg(a.vals_in + base + idx) : 0;
+            }
         }
-        // rank inside the warp, digit by digit, keeping (j, lane) order
+        // ---- rank inside the warp, digit by digit, keeping (j, lane) order
         unsigned short rank[kTsItems];
 #pragma unroll
         for (int j = 0; j < kTsItems; ++j) {
             const unsigned int d = (key[j] >> a.shift) & a.mask;
-            const unsigned int peers = __match_any_sync(0xffffffffu, d);
+            // lanes with the same digit, from one ballot per digit bit (MATCH.ANY occupies the ADU pipe
+            // for ~64 cycles per warp instruction on sm_100a; ballots go through the ALU path)
+            unsigned int peers = 0xffffffffu;
+#pragma unroll
+            for (int b = 0; b < BITS; ++b) {
+                const bool bit = (d >> b) & 1u;
+                const unsigned int m = __ballot_sync(0xffffffffu, bit);
+                peers &= bit ? m : ~m;
+            }
             const int leader = __ffs(peers) - 1;
             unsigned int old = 0;
             if (lane == leader) old = sm.warp_hist[warp][d];
@@ -726,8 +872,8 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
             if (lane == leader) sm.warp_hist[warp][d] = (unsigned short)(old + __popc(peers));
             __syncwarp();
         }
-        __syncthreads();
-        // thread d owns digit d: per-warp exclusive offsets and the tile's count of this digit
+        __syncthreads();   // (also: every thread has read its generated records out of sm.keys / sm.vals)
+        // ---- thread d owns digit d: per-warp exclusive offsets and the tile's count of this digit
         unsigned int count = 0;
         if (tid < BINS) {
 #pragma unroll
@@ -754,15 +900,25 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
                 if (w < warp) bc += sm.scan_tmp[w];
             const unsigned int bin_start = bc + inc_c - count;
             // look back over the earlier tiles for the exclusive prefix of this digit
+            // (kLookWide predecessors are read per round trip: the walk is latency bound)
             unsigned int excl = 0;
             if (tile > 0) {
                 int64_t look = tile - 1;
-                while (true) {
-                    unsigned long long st;
-                    do { st = ld_volatile_u64(a.status + look * BINS + tid); } while ((st >> 34) != (unsigned long long)(a.pass + 1));
-                    excl += (unsigned int)st;
-                    if (((st >> 32) & 3ull) == 2ull) break;
-                    --look;
+                bool done = false;
+                while (!done) {
+                    unsigned long long st[kLookWide];
+#pragma unroll
+                    for (int q = 0; q < kLookWide; ++q)
+                        st[q] = (look - q >= 0) ? ld_volatile_u64(a.status + (look - q) * BINS + tid) : 0ull;
+#pragma unroll
+                    for (int q = 0; q < kLookWide; ++q) {
+                        if (!done) {
+                            while ((st[q] >> 34) != (unsigned long long)(a.pass + 1)) st[q] = ld_volatile_u64(a.status + (look - q) * BINS + tid);
+                            excl += (unsigned int)st[q];
+                            done = ((st[q] >> 32) & 3ull) == 2ull;   // tile 0 always publishes an inclusive prefix
+                        }
+                    }
+                    look -= kLookWide;
                 }
                 st_volatile_u64(a.status + tile * BINS + tid, tag_incl | (unsigned long long)(excl + count));
             }
@@ -770,7 +926,7 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
             sm.goff[tid] = (int)(dbase + excl) - (int)bin_start;
         }
         __syncthreads();
-        // records -> shared memory in sorted order
+        // ---- records -> shared memory in sorted order
 #pragma unroll
         for (int j = 0; j < kTsItems; ++j) {
             const unsigned int d = (key[j] >> a.shift) & a.mask;
@@ -779,36 +935,17 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
             sm.vals[pos] = val[j];
         }
         __syncthreads();
-        // every digit run goes to consecutive global addresses
+        // ---- every digit run goes to consecutive global addresses
 #pragma unroll
         for (int k = 0; k < kTsItems; ++k) {
             const int p = tid + k * kTsThreads;
             if (p < valid) {
                 const unsigned int kk = sm.keys[p];
                 const int dst = sm.goff[(kk >> a.shift) & a.mask] + p;
-                a.keys_out[dst] = kk;
+                if (a.keys_out) a.keys_out[dst] = kk;
                 a.vals_out[dst] = sm.vals[p];
             }
         }
-    }
-}
-
-// ------------------------------------------------------------------------------ B4
-__global__ void __launch_bounds__(256) ranges_kernel(const unsigned int* __restrict__ tkeys, const unsigned long long* count,
-                                                     int64_t* __restrict__ ranges) {
-    const int64_t n = (int64_t)(*count);
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t t = (int64_t)__ldg(tkeys + i);
-        if (i == 0) {
-            ranges[2 * t] = 0;
-        } else {
-            const int64_t tp = (int64_t)__ldg(tkeys + i - 1);
-            if (tp != t) {
-                ranges[2 * t] = i;
-                ranges[2 * tp + 1] = i;
-            }
-        }
-        if (i == n - 1) ranges[2 * t + 1] = n;
     }
 }
 
@@ -862,19 +999,19 @@ static int run_sort(const SortPlan& plan, uint64_t* k0, int32_t* v0, uint64_t* k
     return GS_OK;
 }
 
-template <int BITS>
+template <int BITS, bool GEN>
 static int launch_tile_sweep(const TileSweepArgs& a, int64_t capacity, cudaStream_t st) {
     static int blocks_per_sm = 0;
     const int smem = (int)sizeof(TileSweepSmem<BITS>);
     if (!blocks_per_sm) {
-        if (cudaFuncSetAttribute(tile_sweep_kernel<BITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GS_ERR_CUDA;
+        if (cudaFuncSetAttribute(tile_sweep_kernel<BITS, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GS_ERR_CUDA;
         int b = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, tile_sweep_kernel<BITS>, kTsThreads, smem) != cudaSuccess || b < 1) return GS_ERR_CUDA;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, tile_sweep_kernel<BITS, GEN>, kTsThreads, smem) != cudaSuccess || b < 1) return GS_ERR_CUDA;
         blocks_per_sm = b;
     }
     const int64_t tiles = (capacity + kTsTile - 1) / kTsTile;
     const int64_t resident = (int64_t)sm_count() * blocks_per_sm;
-    tile_sweep_kernel<BITS><<<(unsigned)(tiles < resident ? tiles : resident), kTsThreads, smem, st>>>(a);
+    tile_sweep_kernel<BITS, GEN><<<(unsigned)(tiles < resident ? tiles : resident), kTsThreads, smem, st>>>(a);
     return launch_status();
 }
 
@@ -894,10 +1031,11 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
     if ((int64_t)C * N >= (1LL << 31) || capacity_M >= (1LL << 30)) return GS_ERR_UNSUPPORTED;
     const int gx = (cams[0].width + kTile - 1) / kTile, gy = (cams[0].height + kTile - 1) / kTile;
     const int64_t tiles = (int64_t)gx * gy;
-    if ((int64_t)C * tiles >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
+    const int64_t cells = (int64_t)C * (gx + 1) * (gy + 1);
+    if ((int64_t)C * tiles >= (1LL << 31) || cells >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
     const int64_t n_entries = (int64_t)C * N;
     const int64_t cap = capacity_M > 0 ? capacity_M : 1;
-    const Workspace w = layout(n_entries, cap);
+    const Workspace w = layout(n_entries, cap, cells);
     if (!workspace) {
         if (!workspace_bytes) return GS_ERR_INVALID_ARGUMENT;
         *workspace_bytes = w.total;
@@ -912,79 +1050,96 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
     while ((1 << view_bits) < C) ++view_bits;
     const SortPlan dplan = make_plan(32 + view_bits, true);
     const TilePlan tplan = make_tile_plan(tile_bits);
+    const int sms = sm_count();
 
     unsigned char* ws = reinterpret_cast<unsigned char*>(workspace);
     BinHeader* hdr = reinterpret_cast<BinHeader*>(ws + w.off_header);
     unsigned int* hist = reinterpret_cast<unsigned int*>(ws + w.off_hist);
     unsigned int* thist = reinterpret_cast<unsigned int*>(ws + w.off_thist);
+    int* tdiff = reinterpret_cast<int*>(ws + w.off_tdiff);
+    auto status_at = [&](size_t off) { return reinterpret_cast<unsigned long long*>(ws + off); };
     uint64_t* ck[2] = {reinterpret_cast<uint64_t*>(ws + w.off_ckeys0), reinterpret_cast<uint64_t*>(ws + w.off_ckeys1)};
     int32_t* cv[2] = {reinterpret_cast<int32_t*>(ws + w.off_cvals0), reinterpret_cast<int32_t*>(ws + w.off_cvals1)};
     unsigned int* tk[2] = {reinterpret_cast<unsigned int*>(ws + w.off_tkeys0), reinterpret_cast<unsigned int*>(ws + w.off_tkeys1)};
-    // the tile sort ping-pongs between buffer 0 and 1; the caller's array is the one the last pass writes
+    // pass p writes buffer (p + 1) & 1; the caller's array is the one the last pass writes
     int32_t* tv[2];
     tv[tplan.P & 1] = isect_vals;
     tv[(tplan.P & 1) ^ 1] = reinterpret_cast<int32_t*>(ws + w.off_vals);
 
     if (cudaMemsetAsync(ws, 0, w.zero_bytes, st) != cudaSuccess) return GS_ERR_CUDA;
-    if (cudaMemsetAsync(tile_ranges, 0, (size_t)C * tiles * 2 * sizeof(int64_t), st) != cudaSuccess) return GS_ERR_CUDA;
     const int64_t n_blocks = (n_entries + kScanTile - 1) / kScanTile;
     if (n_blocks > 0) {
         CompactArgs a;
         a.n_entries = n_entries; a.N = N; a.gx = gx; a.gy = gy;
         a.means2d = means2d; a.depths = depths; a.radii = radii;
         a.vcap = w.vcap; a.ckeys = reinterpret_cast<unsigned long long*>(ck[0]); a.cvals = cv[0];
-        a.hdr = hdr; a.status = reinterpret_cast<unsigned long long*>(ws + w.off_compact_status);
+        a.tdiff = tdiff;
+        a.hdr = hdr; a.status = status_at(w.off_compact_status);
         a.n_blocks = (unsigned int)n_blocks;
-        a.M_dev = reinterpret_cast<unsigned long long*>(M_dev);
         compact_kernel<<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a);
         rc = launch_status();
         if (rc) return rc;
-    } else if (M_dev) {
-        if (cudaMemsetAsync(M_dev, 0, sizeof(int64_t), st) != cudaSuccess) return GS_ERR_CUDA;
+    }
+    // records per tile -> ranges, digit histograms, M
+    {
+        const int cols = C * (gx + 1);
+        tile_yscan_kernel<<<(cols + 127) / 128, 128, 0, st>>>(tdiff, C, gx, gy);
+        rc = launch_status();
+        if (rc) return rc;
+        const unsigned int cb = (unsigned int)((cells + kScanTile - 1) / kScanTile);
+        tile_xscan_kernel<<<cb, kScanThreads, 0, st>>>(tdiff, cells, hdr, status_at(w.off_xscan_status));
+        rc = launch_status();
+        if (rc) return rc;
+        RangesArgs a;
+        a.tcount = tdiff; a.cells = cells; a.C = C; a.gx = gx; a.gy = gy; a.capacity = capacity_M;
+        a.ranges = tile_ranges; a.thist = thist; a.plan = tplan; a.hdr = hdr; a.status = status_at(w.off_rscan_status);
+        a.n_blocks = cb; a.M_dev = reinterpret_cast<unsigned long long*>(M_dev);
+        tile_ranges_kernel<<<cb, kScanThreads, 0, st>>>(a);
+        rc = launch_status();
+        if (rc) return rc;
+        scan_hist_kernel<<<1, kTsMaxBins, 0, st>>>(thist, tplan.P, hdr, capacity_M, tile_ranges, (int64_t)C * tiles);
+        rc = launch_status();
+        if (rc) return rc;
     }
     if (capacity_M > 0 && n_blocks > 0) {
         // depth sort of the visible entries (bits of the fp32 depth, then the view index)
-        rc = run_sort(dplan, ck[0], cv[0], ck[1], cv[1], &hdr->V, hdr->sort_ticket, hist,
-                      reinterpret_cast<unsigned long long*>(ws + w.off_sort_status), w.vcap, st);
+        rc = run_sort(dplan, ck[0], cv[0], ck[1], cv[1], &hdr->V, hdr->sort_ticket, hist, status_at(w.off_sort_status), w.vcap, st);
         if (rc) return rc;
         const int32_t* sorted_entries = cv[dplan.P & 1];
-        const int sms = sm_count();
+        EntryRec* entries = reinterpret_cast<EntryRec*>(ws + w.off_entries);
+        unsigned int* chunk_first = reinterpret_cast<unsigned int*>(ws + w.off_chunk_first);
         {
-            EmitArgs a;
+            OffsetsArgs a;
             a.N = N; a.gx = gx; a.gy = gy; a.tiles = (unsigned int)tiles;
             a.means2d = means2d; a.radii = radii; a.cvals = sorted_entries;
-            a.capacity = capacity_M; a.tkeys = tk[0]; a.vals = tv[0];
-            a.hdr = hdr; a.status = reinterpret_cast<unsigned long long*>(ws + w.off_emit_status);
-            a.thist = thist; a.plan = tplan;
-            const int64_t eb = (w.vcap + kScanTile - 1) / kScanTile;
-            const int64_t resident = (int64_t)sms * 6;
-            emit_kernel<<<(unsigned)(eb < resident ? eb : resident), kScanThreads, 0, st>>>(a);
+            a.entries = entries; a.chunk_first = chunk_first; a.n_chunks = w.n_chunks;
+            a.hdr = hdr; a.status = status_at(w.off_offs_status);
+            offsets_kernel<<<(unsigned)((w.vcap + kScanTile - 1) / kScanTile), kScanThreads, 0, st>>>(a);
             rc = launch_status();
             if (rc) return rc;
         }
-        scan_hist_kernel<<<1, kTsMaxBins, 0, st>>>(thist, tplan.P);
-        rc = launch_status();
-        if (rc) return rc;
         for (int p = 0; p < tplan.P; ++p) {
+            const bool last = p == tplan.P - 1;
             TileSweepArgs a;
             a.keys_in = tk[p & 1]; a.vals_in = tv[p & 1];
-            a.keys_out = tk[(p & 1) ^ 1]; a.vals_out = tv[(p & 1) ^ 1];
+            a.keys_out = (last && !isect_keys) ? nullptr : tk[(p & 1) ^ 1];
+            a.vals_out = tv[(p & 1) ^ 1];
             a.count = &hdr->n_rec;
             a.shift = tplan.shift[p]; a.mask = tplan.mask[p]; a.pass = p;
             a.digit_base = thist + p * kTsMaxBins;
-            a.status = reinterpret_cast<unsigned long long*>(ws + w.off_tsort_status);
+            a.status = status_at(w.off_tsort_status);
             a.ticket = &hdr->tsort_ticket[p];
-            rc = tplan.bits == 9 ? launch_tile_sweep<9>(a, capacity_M, st) : launch_tile_sweep<8>(a, capacity_M, st);
+            a.entries = entries; a.chunk_first = chunk_first; a.n_entries = &hdr->V; a.gx = gx;
+            if (p == 0)
+                rc = tplan.bits == 9 ? launch_tile_sweep<9, true>(a, capacity_M, st) : launch_tile_sweep<8, true>(a, capacity_M, st);
+            else
+                rc = tplan.bits == 9 ? launch_tile_sweep<9, false>(a, capacity_M, st) : launch_tile_sweep<8, false>(a, capacity_M, st);
             if (rc) return rc;
         }
-        const unsigned int* sorted_tiles = tk[tplan.P & 1];
-        const int64_t rb = (capacity_M + 255) / 256;
-        const unsigned grid = (unsigned)(rb < (int64_t)sms * 8 ? rb : (int64_t)sms * 8);
-        ranges_kernel<<<grid, 256, 0, st>>>(sorted_tiles, &hdr->n_rec, tile_ranges);
-        rc = launch_status();
-        if (rc) return rc;
         if (isect_keys) {
-            keys_kernel<<<grid, 256, 0, st>>>(sorted_tiles, isect_vals, depths, &hdr->n_rec, isect_keys);
+            const int64_t rb = (capacity_M + 255) / 256;
+            const unsigned grid = (unsigned)(rb < (int64_t)sms * 8 ? rb : (int64_t)sms * 8);
+            keys_kernel<<<grid, 256, 0, st>>>(tk[tplan.P & 1], isect_vals, depths, &hdr->n_rec, isect_keys);
             rc = launch_status();
             if (rc) return rc;
         }

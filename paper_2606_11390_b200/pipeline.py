@@ -138,11 +138,12 @@ class SplatStep:
         self.l1_loss()
         self.backward()
 
-    # launches of this library's kernels in one step (memsets excluded): P1, compact, depth-sort
-    # histogram + passes, emit, histogram scan, tile-sort passes, ranges (+ keys), R1, L1, zero rows, R2, P5
+    # launches of this library's kernels in one step (memsets excluded): P1; compact, tile y-scan, x-scan,
+    # ranges, histogram scan, depth-sort histogram + passes, entry offsets, tile-sort passes (+ keys); R1, L1,
+    # zero rows, R2, P5
     def launches_per_step(self):
         tile_bits = max(1, int(np.ceil(np.log2(self.C * self.gx * self.gy))))
         view_bits = int(np.ceil(np.log2(self.C))) if self.C > 1 else 0
         depth_passes = 4 + (view_bits + 7) // 8
         tile_passes = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
-        return 1 + 1 + 1 + depth_passes + 1 + 1 + tile_passes + 1 + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1
+        return 1 + 5 + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

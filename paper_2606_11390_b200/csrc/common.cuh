@@ -22,6 +22,7 @@ struct DevCam {
     float near_plane, far_plane;
     float lim_x, lim_y;
     float ox, oy, oz;
+    float wnorm2;              // upper bound of |W|_2^2 (1 for a rigid transform): max absolute row sum of W W^T
     int32_t width, height, gx, gy;
 };
 
@@ -42,6 +43,15 @@ inline DevCam make_devcam(const gs_camera& c) {
     d.ox = -(d.W[0] * d.tau[0] + d.W[3] * d.tau[1] + d.W[6] * d.tau[2]);
     d.oy = -(d.W[1] * d.tau[0] + d.W[4] * d.tau[1] + d.W[7] * d.tau[2]);
     d.oz = -(d.W[2] * d.tau[0] + d.W[5] * d.tau[1] + d.W[8] * d.tau[2]);
+    d.wnorm2 = 1.0f;
+    for (int r = 0; r < 3; ++r) {
+        float row = 0.0f;
+        for (int j = 0; j < 3; ++j) {
+            const float g = d.W[3 * r] * d.W[3 * j] + d.W[3 * r + 1] * d.W[3 * j + 1] + d.W[3 * r + 2] * d.W[3 * j + 2];
+            row += g < 0.0f ? -g : g;
+        }
+        if (row > d.wnorm2) d.wnorm2 = row;
+    }
     d.width = c.width; d.height = c.height;
     d.gx = (c.width + kTile - 1) / kTile;
     d.gy = (c.height + kTile - 1) / kTile;

@@ -1,11 +1,22 @@
 // project.cu -- per-Gaussian stages P1 (gs_project_fwd) and P5 (gs_project_bwd) for sm_100a.
 //
-// One thread per Gaussian; the C views of the batch are looped inside the thread so that the
-// parameters (236 B at SH degree 3) are read once for all cameras ("outputs colors
-// and projected geometric quantities for all cameras in the batch").  Culling happens on the
-// 12-byte mean first; scale/rotation are read only for Gaussians inside some view's depth range
-// and the SH coefficients only for Gaussians visible in at least one view, so the HBM traffic is
-// 12 N + 224 V_any + 48 sum_c V_c + 8 N C ("algorithmic bytes").
+// The C views of the batch are looped inside one thread per Gaussian so that the parameters (236 B
+// at SH degree 3) are read once for all cameras ("outputs colors and projected
+// geometric quantities for all cameras in the batch").  Both kernels are persistent; every WARP works
+// on its own chunks of consecutive Gaussians, independently of the other warps (no block barrier), in two phases:
+//   phase A (streaming, every thread, vector loads/stores): P1 reads the 12-byte means (4 Gaussians =
+//     3 x 16 B per thread), applies the near/far test of every view and zero-fills the chunk's radii /
+//     tiles_touched; P5 reads the saved radii and zero-fills the chunk's rows of the five dense
+//     gradient arrays with fully coalesced 16-byte stores.  The surviving Gaussians are pushed
+//     onto a shared-memory stack that is carried across chunks;
+//   phase B (runs whenever a full block of survivors is waiting, one thread each, so its warps are
+//     fully populated even when a few per cent of the Gaussians survive): P1 first drops the views
+//     whose tile rectangle must be empty from the mean and the largest scale alone (B0), then reads
+//     rotation and the SH coefficients only for Gaussians that can be visible (B1); P5 evaluates the
+//     chain rule for the visible Gaussians.
+// So the HBM traffic is 12 N + 224 V_any + 48 sum_c V_c + 8 N C for P1 and 4 N C + 36 sum_c V_c +
+// 236 V_any + 236 N for P5 ("algorithmic bytes"), and in the city/block regime (a few
+// per cent visible) nearly all of it moves in phase A at full memory-level parallelism.
 #include "project_math.cuh"
 
 namespace gs {
@@ -17,9 +28,15 @@ struct ProjFwdArgs {
     float* means2d; float* depths; float* conics; float* opacities; float* rgbs;
     int32_t* radii; uint32_t* tiles;
     float dilation, extent;
+    int32_t vec_in, vec_out;   // 16-byte vector access allowed on means / on radii+tiles rows
 };
 
-constexpr int kProjThreads = 128;
+constexpr int kProjThreads = 128;   // P1 block
+constexpr int kBwdThreads = 128;    // P5 block (168 registers per thread)
+#ifndef GS_PROJ_ITEMS
+#define GS_PROJ_ITEMS 8
+#endif
+constexpr int kProjItems = GS_PROJ_ITEMS;   // Gaussians per thread in P1's streaming phase
 
 template <int DEG>
 __device__ __forceinline__ void load_sh(const float* __restrict__ sh, int64_t i, float* f) {
@@ -38,21 +55,40 @@ __device__ __forceinline__ void load_sh(const float* __restrict__ sh, int64_t i,
     }
 }
 
-template <int DEG>
-__global__ void __launch_bounds__(kProjThreads) project_fwd_kernel(const ProjFwdArgs a, const __grid_constant__ CamBatch cams) {
-    const int64_t i = (int64_t)blockIdx.x * kProjThreads + threadIdx.x;
-    if (i >= a.N) return;
-    const float px = __ldg(a.means + 3 * i), py = __ldg(a.means + 3 * i + 1), pz = __ldg(a.means + 3 * i + 2);
+// A warp's shared-memory stack of pending Gaussians: index, view mask and (P1 only) the mean, so that
+// the later phases do not read it from memory again.  CAP entries per warp.
+template <int CAP, bool WITH_MEAN>
+struct WarpStack {
+    uint32_t idx[CAP];
+    uint32_t msk[CAP];
+    float xyz[WITH_MEAN ? 3 : 1][WITH_MEAN ? CAP : 1];
+};
 
-    // depth-range test on the mean alone (step 1)
-    uint32_t zmask = 0;
-    for (int c = 0; c < a.C; ++c) {
-        const DevCam& cam = cams.cam[c];
-        const float tz = cam.W[6] * px + cam.W[7] * py + cam.W[8] * pz + cam.tau[2];
-        if (tz > cam.near_plane && tz < cam.far_plane) zmask |= 1u << c;
+// Warp-wide push of the items with a non-zero mask; `cnt` (the stack height) is warp-uniform.  The
+// order is irrelevant: every output is addressed by the index.
+template <int ITEMS, int CAP, bool WITH_MEAN>
+__device__ __forceinline__ void warp_push(const uint32_t (&idx)[ITEMS], const uint32_t (&msk)[ITEMS], const float* m /*[3*ITEMS] or null*/,
+                                          WarpStack<CAP, WITH_MEAN>& st, int& cnt, int lane) {
+    const unsigned int lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        const unsigned int b = __ballot_sync(0xffffffffu, msk[k] != 0u);
+        if (msk[k]) {
+            const int p = cnt + __popc(b & lt);
+            st.idx[p] = idx[k];
+            st.msk[p] = msk[k];
+            if (WITH_MEAN) { st.xyz[0][p] = m[3 * k]; st.xyz[WITH_MEAN ? 1 : 0][p] = m[3 * k + 1]; st.xyz[WITH_MEAN ? 2 : 0][p] = m[3 * k + 2]; }
+        }
+        cnt += __popc(b);
     }
+}
+
+// phase B of P1 for one Gaussian inside the depth range of the views in zmask
+template <int DEG>
+__device__ __forceinline__ void project_fwd_one(const ProjFwdArgs& a, const CamBatch& cams, int64_t i, uint32_t zmask, float px, float py,
+                                                float pz) {
     uint32_t vis = 0;
-    if (zmask) {
+    {
         float ls[3], q[4], s[3], qh[4], qn, R[9];
         Sym3 S;
         ls[0] = __ldg(a.log_scales + 3 * i); ls[1] = __ldg(a.log_scales + 3 * i + 1); ls[2] = __ldg(a.log_scales + 3 * i + 2);
@@ -89,12 +125,6 @@ __global__ void __launch_bounds__(kProjThreads) project_fwd_kernel(const ProjFwd
             a.tiles[e] = nt;
         }
     }
-    for (int c = 0; c < a.C; ++c)
-        if (!((vis >> c) & 1u)) {
-            const int64_t e = (int64_t)c * a.N + i;
-            a.radii[e] = 0;
-            a.tiles[e] = 0;
-        }
     if (!vis) return;
 
     // steps 9, 10: colour and opacity, only for Gaussians visible somewhere
@@ -122,6 +152,131 @@ __global__ void __launch_bounds__(kProjThreads) project_fwd_kernel(const ProjFwd
     }
 }
 
+// Conservative screen-space pre-cull from the mean and the largest scale alone (no rotation needed):
+// |Sigma'| <= (s_max |J|_F |W|_2)^2 =: L, so lambda_max <= 2 (L + dilation) + sqrt(0.1) and the integer radius
+// is at most rb = extent sqrt(that) + 1.  A view whose tile rectangle must then be empty (mean more
+// than rb outside the 16-pixel-padded image) is dropped from the mask; phase B would cull it at step 8
+// anyway, so no result changes.  Non-finite intermediates fail every comparison and keep the view.
+__device__ __forceinline__ uint32_t lateral_precull(const ProjFwdArgs& a, const CamBatch& cams, float lmax, float px, float py, float pz,
+                                                    uint32_t zmask) {
+    const float smax = expf(lmax);
+    uint32_t keep = 0;
+    for (int c = 0; c < a.C; ++c) {
+        if (!((zmask >> c) & 1u)) continue;
+        const DevCam& cam = cams.cam[c];
+        const float tx = cam.W[0] * px + cam.W[1] * py + cam.W[2] * pz + cam.tau[0];
+        const float ty = cam.W[3] * px + cam.W[4] * py + cam.W[5] * pz + cam.tau[1];
+        const float tz = cam.W[6] * px + cam.W[7] * py + cam.W[8] * pz + cam.tau[2];
+        const float rz = 1.0f / tz;
+        const float u = cam.fx * tx * rz + cam.cx, v = cam.fy * ty * rz + cam.cy;
+        const float jf = (cam.fx * cam.fx * (1.0f + cam.lim_x * cam.lim_x) + cam.fy * cam.fy * (1.0f + cam.lim_y * cam.lim_y)) * cam.wnorm2 * rz * rz;
+        const float L = smax * smax * jf;
+        const float rb = a.extent * sqrtf(2.0f * (L + fmaxf(a.dilation, 0.0f)) + 0.32f) * 1.001f + 3.0f;
+        const float w16 = (float)(cam.gx * kTile), h16 = (float)(cam.gy * kTile);
+        const bool out = (u + rb + 16.0f < 0.0f) || (u - rb > w16) || (v + rb + 16.0f < 0.0f) || (v - rb > h16);
+        if (!out) keep |= 1u << c;
+    }
+    return keep;
+}
+
+template <int DEG, int ITEMS>
+__global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const ProjFwdArgs a, const __grid_constant__ CamBatch cams) {
+    constexpr int CHUNK = 32 * ITEMS;                   // Gaussians per warp and phase-A step
+    constexpr int WARPS = kProjThreads / 32;
+    __shared__ WarpStack<32 + CHUNK, true> s1_all[WARPS];   // Gaussians inside some view's depth range
+    __shared__ WarpStack<64, true> s2_all[WARPS];           // survivors of the screen-space pre-cull
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpStack<32 + CHUNK, true>& s1 = s1_all[warp];
+    WarpStack<64, true>& s2 = s2_all[warp];
+    const int64_t n_chunks = (a.N + CHUNK - 1) / CHUNK;
+    const int64_t stride = (int64_t)gridDim.x * WARPS;
+    int64_t chunk = (int64_t)blockIdx.x * WARPS + warp;
+    int cnt1 = 0, cnt2 = 0;    // warp-uniform stack heights
+    while (true) {
+        // ---- phase A (streaming) until a full warp of depth candidates is waiting: means -> near/far
+        //      test of every view; zero radii / tiles_touched of the chunk
+        while (cnt1 < 32 && chunk < n_chunks) {
+            const int64_t i0 = chunk * CHUNK + (int64_t)lane * ITEMS;
+            float m[3 * ITEMS];
+            const bool full = i0 + ITEMS <= a.N;
+            if (ITEMS % 4 == 0 && a.vec_in && full) {
+                const float4* p4 = reinterpret_cast<const float4*>(a.means + 3 * i0);
+#pragma unroll
+                for (int k = 0; k < 3 * ITEMS / 4; ++k) {
+                    const float4 v = __ldg(p4 + k);
+                    m[4 * k] = v.x; m[4 * k + 1] = v.y; m[4 * k + 2] = v.z; m[4 * k + 3] = v.w;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < 3 * ITEMS; ++k) m[k] = (i0 + k / 3 < a.N) ? __ldg(a.means + 3 * i0 + k) : 0.0f;
+            }
+            uint32_t idx[ITEMS], msk[ITEMS];
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) msk[k] = 0;
+            for (int c = 0; c < a.C; ++c) {
+                const DevCam& cam = cams.cam[c];
+                const float w0 = cam.W[6], w1 = cam.W[7], w2 = cam.W[8], t2 = cam.tau[2], zn = cam.near_plane, zf = cam.far_plane;
+#pragma unroll
+                for (int k = 0; k < ITEMS; ++k) {
+                    const float tz = w0 * m[3 * k] + w1 * m[3 * k + 1] + w2 * m[3 * k + 2] + t2;
+                    if (tz > zn && tz < zf) msk[k] |= 1u << c;
+                }
+                const int64_t e0 = (int64_t)c * a.N + i0;
+                if (ITEMS % 4 == 0 && a.vec_out && full) {
+#pragma unroll
+                    for (int k = 0; k < ITEMS / 4; ++k) {
+                        reinterpret_cast<int4*>(a.radii + e0)[k] = make_int4(0, 0, 0, 0);
+                        reinterpret_cast<uint4*>(a.tiles + e0)[k] = make_uint4(0u, 0u, 0u, 0u);
+                    }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < ITEMS; ++k)
+                        if (i0 + k < a.N) { a.radii[e0 + k] = 0; a.tiles[e0 + k] = 0u; }
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) {
+                if (i0 + k >= a.N) msk[k] = 0;
+                idx[k] = (uint32_t)(i0 + k);
+            }
+            warp_push<ITEMS>(idx, msk, m, s1, cnt1, lane);
+            chunk += stride;
+            __syncwarp();      // pushes visible to the warp; its zero-fill is ordered before phase B's stores
+        }
+        // ---- phase B0: screen-space pre-cull of up to one depth candidate per lane -> stack 2
+        if (cnt1 > 0 && cnt2 <= 32) {
+            const int n = cnt1 < 32 ? cnt1 : 32;
+            uint32_t idx[1] = {0u}, msk[1] = {0u};
+            float m[3] = {0.f, 0.f, 0.f};
+            if (lane < n) {
+                const int p = cnt1 - n + lane;
+                idx[0] = s1.idx[p];
+                m[0] = s1.xyz[0][p]; m[1] = s1.xyz[1][p]; m[2] = s1.xyz[2][p];
+                const float* ls = a.log_scales + 3 * (int64_t)idx[0];
+                const float lmax = fmaxf(__ldg(ls), fmaxf(__ldg(ls + 1), __ldg(ls + 2)));
+                msk[0] = lateral_precull(a, cams, lmax, m[0], m[1], m[2], s1.msk[p]);
+            }
+            cnt1 -= n;
+            __syncwarp();      // the popped entries have been read
+            warp_push<1>(idx, msk, m, s2, cnt2, lane);
+            __syncwarp();
+            if (cnt2 < 32 && (cnt1 > 0 || chunk < n_chunks)) continue;
+        }
+        if (cnt2 == 0) {
+            if (cnt1 == 0 && chunk >= n_chunks) break;
+            continue;
+        }
+        // ---- phase B1: full projection of up to one survivor per lane
+        const int n = cnt2 < 32 ? cnt2 : 32;
+        if (lane < n) {
+            const int p = cnt2 - n + lane;
+            project_fwd_one<DEG>(a, cams, (int64_t)s2.idx[p], s2.msk[p], s2.xyz[0][p], s2.xyz[1][p], s2.xyz[2][p]);
+        }
+        cnt2 -= n;
+        __syncwarp();          // the popped entries have been read
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 struct ProjBwdArgs {
     int64_t N;
@@ -132,6 +287,7 @@ struct ProjBwdArgs {
     float* d_means; float* d_log_scales; float* d_quats; float* d_logits; float* d_sh;
     float dilation;
     int32_t accumulate;
+    int32_t vec_in, vec_out;   // 16-byte vector access allowed on the radii rows / on the five gradient arrays
 };
 
 template <int DEG>
@@ -155,22 +311,17 @@ __device__ __forceinline__ void store_sh(float* __restrict__ out, int64_t i, con
     }
 }
 
+// phase B of P5 for one Gaussian visible in the views of `vis` (the rows were zero-filled in phase A
+// unless the caller accumulates)
 template <int DEG>
-__global__ void __launch_bounds__(kProjThreads) project_bwd_kernel(const ProjBwdArgs a, const __grid_constant__ CamBatch cams) {
-    const int64_t i = (int64_t)blockIdx.x * kProjThreads + threadIdx.x;
-    if (i >= a.N) return;
+__device__ __forceinline__ void project_bwd_one(const ProjBwdArgs& a, const CamBatch& cams, int64_t i, uint32_t vis) {
     constexpr int K = (DEG + 1) * (DEG + 1);
-
-    uint32_t vis = 0;
-    for (int c = 0; c < a.C; ++c)
-        if (__ldg(a.radii + (int64_t)c * a.N + i) > 0) vis |= 1u << c;
-
     float gp[3] = {0.f, 0.f, 0.f}, gl[3] = {0.f, 0.f, 0.f}, gq[4] = {0.f, 0.f, 0.f, 0.f}, glogit = 0.f;
     float gsh[3 * K];
 #pragma unroll
     for (int k = 0; k < 3 * K; ++k) gsh[k] = 0.f;
 
-    if (vis) {
+    {
         const float px = __ldg(a.means + 3 * i), py = __ldg(a.means + 3 * i + 1), pz = __ldg(a.means + 3 * i + 2);
         float ls[3], q[4], s[3], qh[4], qn, R[9];
         Sym3 S;
@@ -313,7 +464,6 @@ __global__ void __launch_bounds__(kProjThreads) project_bwd_kernel(const ProjBwd
     }
 
     if (a.accumulate) {
-        if (!vis) return;
 #pragma unroll
         for (int k = 0; k < 3; ++k) { a.d_means[3 * i + k] += gp[k]; a.d_log_scales[3 * i + k] += gl[k]; }
         float4* dq = reinterpret_cast<float4*>(a.d_quats) + i;
@@ -331,16 +481,119 @@ __global__ void __launch_bounds__(kProjThreads) project_bwd_kernel(const ProjBwd
     }
 }
 
+// warp-cooperative zero-fill of `count` floats at p (16-byte stores when `vec`: p is then 16-byte aligned)
+__device__ __forceinline__ void zero_span(float* __restrict__ p, int64_t count, bool vec, int lane) {
+    if (vec) {
+        const int64_t n4 = count >> 2;
+        float4* p4 = reinterpret_cast<float4*>(p);
+        for (int64_t k = lane; k < n4; k += 32) p4[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int64_t k = (n4 << 2) + lane; k < count; k += 32) p[k] = 0.f;
+    } else {
+        for (int64_t k = lane; k < count; k += 32) p[k] = 0.f;
+    }
+}
+
+template <int DEG, int ITEMS>
+__global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjBwdArgs a, const __grid_constant__ CamBatch cams) {
+    constexpr int CHUNK = 32 * ITEMS;                   // Gaussians per warp and phase-A step
+    constexpr int WARPS = kBwdThreads / 32;
+    constexpr int K3 = 3 * (DEG + 1) * (DEG + 1);
+    __shared__ WarpStack<32 + CHUNK, false> st_all[WARPS];   // visible Gaussians and the views they are visible in
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpStack<32 + CHUNK, false>& stk = st_all[warp];
+    const int64_t n_chunks = (a.N + CHUNK - 1) / CHUNK;
+    const int64_t stride = (int64_t)gridDim.x * WARPS;
+    int64_t chunk = (int64_t)blockIdx.x * WARPS + warp;
+    int cnt = 0;               // warp-uniform stack height
+    while (true) {
+        // ---- phase A until a full warp of visible Gaussians is waiting: visibility from the saved
+        //      radii; dense zero-fill of the chunk's gradient rows
+        while (cnt < 32 && chunk < n_chunks) {
+            const int64_t base = chunk * CHUNK;
+            const int64_t i0 = base + (int64_t)lane * ITEMS;
+            const bool full = i0 + ITEMS <= a.N;
+            uint32_t idx[ITEMS], vis[ITEMS];
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) vis[k] = 0;
+            for (int c = 0; c < a.C; ++c) {
+                const int64_t e0 = (int64_t)c * a.N + i0;
+                if (ITEMS == 4 && a.vec_in && full) {
+                    const int4 r = __ldg(reinterpret_cast<const int4*>(a.radii + e0));
+                    vis[0] |= (r.x > 0 ? 1u : 0u) << c; vis[1 % ITEMS] |= (r.y > 0 ? 1u : 0u) << c;
+                    vis[2 % ITEMS] |= (r.z > 0 ? 1u : 0u) << c; vis[3 % ITEMS] |= (r.w > 0 ? 1u : 0u) << c;
+                } else {
+#pragma unroll
+                    for (int k = 0; k < ITEMS; ++k)
+                        if (i0 + k < a.N && __ldg(a.radii + e0 + k) > 0) vis[k] |= 1u << c;
+                }
+            }
+            if (!a.accumulate) {
+                const int64_t n = (a.N - base) < CHUNK ? (a.N - base) : CHUNK;
+                const bool vec = a.vec_out != 0;
+                zero_span(a.d_sh + base * K3, n * K3, vec, lane);
+                zero_span(a.d_means + base * 3, n * 3, vec, lane);
+                zero_span(a.d_log_scales + base * 3, n * 3, vec, lane);
+                zero_span(a.d_quats + base * 4, n * 4, vec, lane);
+                zero_span(a.d_logits + base, n, vec, lane);
+            }
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) idx[k] = (uint32_t)(i0 + k);
+            warp_push<ITEMS>(idx, vis, nullptr, stk, cnt, lane);
+            chunk += stride;
+            __syncwarp();      // pushes visible to the warp; its zero-fill is ordered before phase B's stores
+        }
+        // ---- phase B: gradients of up to one visible Gaussian per lane (top of the stack)
+        if (cnt == 0) break;
+        const int n = cnt < 32 ? cnt : 32;
+        if (lane < n) project_bwd_one<DEG>(a, cams, (int64_t)stk.idx[cnt - n + lane], stk.msk[cnt - n + lane]);
+        cnt -= n;
+        __syncwarp();          // the popped entries have been read
+    }
+}
+
+static int sm_count() {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    return sms;
+}
+
+// persistent grid: resident blocks of the kernel, or fewer when there are fewer chunks
+template <typename Kernel>
+static unsigned persistent_grid(Kernel kernel, int threads, int64_t n_chunks, int sms) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+    const int64_t resident = (int64_t)per_sm * sms;
+    return (unsigned)(n_chunks < resident ? n_chunks : resident);
+}
+
+// several Gaussians per lane (16-byte accesses) when every resident warp still gets >= 8 chunks, else 1
 template <int DEG>
 int launch_fwd(const ProjFwdArgs& a, const CamBatch& cb, cudaStream_t st) {
-    const int64_t blocks = (a.N + kProjThreads - 1) / kProjThreads;
-    project_fwd_kernel<DEG><<<(unsigned)blocks, kProjThreads, 0, st>>>(a, cb);
+    const int sms = sm_count();
+    constexpr int warps = kProjThreads / 32;
+    const int64_t wide = (a.N + 32 * kProjItems - 1) / (32 * kProjItems);
+    const unsigned wide_grid = persistent_grid(project_fwd_kernel<DEG, kProjItems>, kProjThreads, (wide + warps - 1) / warps, sms);
+    if (wide >= 8 * (int64_t)wide_grid * warps) {
+        project_fwd_kernel<DEG, kProjItems><<<wide_grid, kProjThreads, 0, st>>>(a, cb);
+    } else {
+        const int64_t chunks = (a.N + 31) / 32;
+        project_fwd_kernel<DEG, 1><<<persistent_grid(project_fwd_kernel<DEG, 1>, kProjThreads, (chunks + warps - 1) / warps, sms), kProjThreads, 0, st>>>(a, cb);
+    }
     return launch_status();
 }
 template <int DEG>
 int launch_bwd(const ProjBwdArgs& a, const CamBatch& cb, cudaStream_t st) {
-    const int64_t blocks = (a.N + kProjThreads - 1) / kProjThreads;
-    project_bwd_kernel<DEG><<<(unsigned)blocks, kProjThreads, 0, st>>>(a, cb);
+    const int sms = sm_count();
+    constexpr int warps = kBwdThreads / 32;
+    const int64_t wide = (a.N + 32 * 4 - 1) / (32 * 4);
+    const unsigned wide_grid = persistent_grid(project_bwd_kernel<DEG, 4>, kBwdThreads, (wide + warps - 1) / warps, sms);
+    if (wide >= 8 * (int64_t)wide_grid * warps) {
+        project_bwd_kernel<DEG, 4><<<wide_grid, kBwdThreads, 0, st>>>(a, cb);
+    } else {
+        const int64_t chunks = (a.N + 31) / 32;
+        project_bwd_kernel<DEG, 1><<<persistent_grid(project_bwd_kernel<DEG, 1>, kBwdThreads, (chunks + warps - 1) / warps, sms), kBwdThreads, 0, st>>>(a, cb);
+    }
     return launch_status();
 }
 
@@ -362,7 +615,7 @@ extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* mean
         !rgbs || !radii || !tiles_touched)
         return GS_ERR_INVALID_ARGUMENT;
     if (!aligned(quats, 16) || !aligned(sh, 16) || !aligned(means2d, 8) || !aligned(means, 4)) return GS_ERR_INVALID_ARGUMENT;
-    if ((N + kProjThreads - 1) / kProjThreads > 0x7fffffffLL || (int64_t)C * N >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
+    if ((int64_t)C * N >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     for (int c0 = 0; c0 < C; c0 += kMaxCamsPerLaunch) {
         const int nc = C - c0 < kMaxCamsPerLaunch ? C - c0 : kMaxCamsPerLaunch;
@@ -375,6 +628,8 @@ extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* mean
         a.means2d = means2d + 2 * off; a.depths = depths + off; a.conics = conics + 3 * off;
         a.opacities = opacities + off; a.rgbs = rgbs + 3 * off; a.radii = radii + off; a.tiles = tiles_touched + off;
         a.dilation = cfg->dilation; a.extent = cfg->extent;
+        a.vec_in = aligned(means, 16) ? 1 : 0;
+        a.vec_out = (aligned(a.radii, 16) && aligned(a.tiles, 16) && (N % 4 == 0 || nc == 1)) ? 1 : 0;
         switch (cfg->sh_degree) {
             case 0: rc = launch_fwd<0>(a, cb, st); break;
             case 1: rc = launch_fwd<1>(a, cb, st); break;
@@ -403,7 +658,7 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
         return GS_ERR_INVALID_ARGUMENT;
     if (!aligned(quats, 16) || !aligned(sh, 16) || !aligned(dL_dquats, 16) || !aligned(dL_dsh, 16) || !aligned(dL_dmeans2d, 8))
         return GS_ERR_INVALID_ARGUMENT;
-    if ((N + kProjThreads - 1) / kProjThreads > 0x7fffffffLL || (int64_t)C * N >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
+    if ((int64_t)C * N >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     for (int c0 = 0; c0 < C; c0 += kMaxCamsPerLaunch) {
         const int nc = C - c0 < kMaxCamsPerLaunch ? C - c0 : kMaxCamsPerLaunch;
@@ -421,6 +676,9 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
         a.dilation = cfg->dilation;
         // the first chunk of cameras overwrites (unless the caller accumulates), later chunks add
         a.accumulate = (accumulate != 0 || c0 > 0) ? 1 : 0;
+        a.vec_in = (aligned(a.radii, 16) && (N % 4 == 0 || nc == 1)) ? 1 : 0;
+        a.vec_out = (aligned(dL_dmeans, 16) && aligned(dL_dlog_scales, 16) && aligned(dL_dquats, 16) &&
+                     aligned(dL_dopacity_logits, 16) && aligned(dL_dsh, 16)) ? 1 : 0;
         switch (cfg->sh_degree) {
             case 0: rc = launch_bwd<0>(a, cb, st); break;
             case 1: rc = launch_bwd<1>(a, cb, st); break;

@@ -1,0 +1,258 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(`SplatStep`, asynchronous binning with device-resident record count, dense gradient overwrite).
+
+* object (configs[1]: 100 k Gaussians, 8 x 1080p, SH degree 3): the whole chained step against the
+  oracle chained the same way -- every pixel and every gradient row (the oracle needs ~1 min).
+* room / block (1 M Gaussians x 4 x 4K; 10 M Gaussians x 4K): sampled outputs.  P1 on every entry;
+  binning by properties that hold at any size (ranges partition [0, M), every list sorted by depth) plus
+  the exact list of sampled tiles rebuilt one by one from the definition (rectangle overlap, stable order
+  by (depth bits, entry)); R1 / R2 on sampled tiles with the oracle's tile mask (stage isolation: the oracle
+  is fed the records and lists the CUDA path produced, and dL/dimage is zero outside the sampled tiles so
+  that the gradient sums of both sides cover the same pixels); P5 on every Gaussian.
+Bars as in test_gpu_parity.py (north_star): integer work bit-exact, image 1e-4, gradients rel. L2 1e-3.
+"""
+import numpy as np
+import pytest
+
+from paper_2606_11390_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+AMB_EPS = 2e-5
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, np.float64).ravel(); b = np.asarray(b, np.float64).ravel()
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-30))
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_11390_b200 import binding
+    binding.lib()
+    return binding
+
+
+def bench_like_step(sc):
+    """The launch sequence of bench.py: one synchronising forward to size the record buffers, then the
+    fully asynchronous step."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    st = SplatStep(sc)
+    st.set_target(scenes.target_image(sc))
+    st.forward(sync=True)
+    M = int(st.M)
+    st._alloc_isect(int(M * 1.05) + 4096)
+    st.step(sync=False)
+    torch.cuda.synchronize()
+    assert int(st.M_dev.item()) == M
+    return st, M
+
+
+def mean2d_tolerance(sc, ref):
+    """First-order fp32 forward error bound of u = fx t_x / t_z + cx (and v), eps = 2^-24:
+    |dt_k| <= 4 eps S_k with S_k = sum_j |W_kj p_j| + |tau_k| (three products, three sums), hence
+    |du| <= fx/t_z 4 eps S_x + |u - cx| (4 eps S_z / t_z + 3 eps) + eps |u|, plus 1e-5 px absolute.
+    (The 2e-6 |u| + 2e-4 px bar of the small scenes is this bound at their scale; at 4K with Gaussians
+    0.2 m in front of a camera in a 10 m room the magnification fx / t_z reaches 1.5e4 px per metre.)"""
+    eps = 2.0 ** -24
+    p = sc["means"].astype(np.float64)
+    tol = np.zeros(ref["means2d"].shape)
+    for c, cam in enumerate(sc["cameras"]):
+        vm = np.asarray(cam["viewmat"], np.float64)
+        S = np.abs(p) @ np.abs(vm[:, :3]).T + np.abs(vm[:, 3])[None, :]
+        tz = np.maximum(ref["depths"][c], 1e-6)
+        for k, (f, c0) in enumerate(((cam["fx"], cam["cx"]), (cam["fy"], cam["cy"]))):
+            u = ref["means2d"][c, :, k]
+            tol[c, :, k] = f / tz * 4 * eps * S[:, k] + np.abs(u - c0) * (4 * eps * S[:, 2] / tz + 3 * eps) + eps * np.abs(u) + 1e-5
+    return tol
+
+
+def depth_tolerance(sc, ref):
+    """|dt_z| <= 4 eps S_z + eps t_z (same bound as in mean2d_tolerance)."""
+    eps = 2.0 ** -24
+    p = np.abs(sc["means"].astype(np.float64))
+    tol = np.zeros(ref["depths"].shape)
+    for c, cam in enumerate(sc["cameras"]):
+        vm = np.abs(np.asarray(cam["viewmat"], np.float64))
+        tol[c] = 4 * eps * (p @ vm[2, :3] + vm[2, 3]) + eps * np.abs(ref["depths"][c])
+    return tol
+
+
+def check_project_fwd(st, ref, name, sc):
+    got = {k: getattr(st, k).cpu().numpy() for k in ("means2d", "depths", "conics", "opacities", "rgbs", "radii")}
+    got["tiles_touched"] = st.tiles_touched.cpu().numpy().view(np.uint32)
+    rr = ref["radius_real"]
+    amb_r = np.abs(rr - np.round(rr)) <= 1e-4 * np.maximum(rr, 1.0)
+    u = ref["means2d"]
+    r = ref["radii"].astype(np.float64)[..., None]
+    lo, hi = (u - r) / 16.0, (u + r + 15.0) / 16.0
+    near_edge = (np.abs(lo - np.round(lo)) < 1e-4) | (np.abs(hi - np.round(hi)) < 1e-4)
+    amb_t = near_edge.any(axis=-1) | amb_r
+    vis_ref, vis_got = ref["radii"] > 0, got["radii"] > 0
+    assert not ((vis_ref != vis_got) & ~amb_t).any()
+    both = vis_ref & vis_got
+    dr = (got["radii"] != ref["radii"]) & both
+    assert not (dr & ~amb_r).any()
+    assert np.all(np.abs(got["radii"][dr] - ref["radii"][dr]) <= 1)
+    dt = (got["tiles_touched"].astype(np.int64) != ref["tiles_touched"].astype(np.int64)) & both
+    assert not (dt & ~amb_t).any()
+    assert np.all(got["tiles_touched"][~vis_got] == 0)
+    m = both
+    err_u = np.abs(got["means2d"][m] - ref["means2d"][m])
+    tol_u = mean2d_tolerance(sc, ref)[m]
+    assert np.all(err_u <= tol_u), (err_u.max(), (err_u / tol_u).max())
+    err_d = np.abs(got["depths"][m] - ref["depths"][m])
+    assert np.all(err_d <= depth_tolerance(sc, ref)[m]), err_d.max()
+    cn = np.abs(ref["conics"][m]).max(axis=-1, keepdims=True)
+    err_c = (np.abs(got["conics"][m] - ref["conics"][m]) / cn).max(axis=-1)
+    assert err_c.max() <= 2e-4, (err_c.max(), ref["depths"][m][err_c.argmax()])
+    np.testing.assert_allclose(got["opacities"][m], ref["opacities"][m], rtol=2e-6)
+    assert np.abs(got["rgbs"][m] - ref["rgbs"][m]).max() <= 5e-6
+    print(f"[{name}] P1: visible {int(both.sum())} of {both.size}; ambiguous radius {int(dr.sum())}, tiles {int(dt.sum())}; "
+          f"mean2d max err {err_u.max():.2e} px, max err/bound {(err_u / tol_u).max():.2f}")
+    return got
+
+
+# ------------------------------------------------------------------------------------ object: everything
+def test_object_full_config_chained_step(B, oracle):
+    sc = scenes.make_scene("object")
+    cfg = oracle.make_cfg(sh_degree=sc["sh_degree"])
+    st, M = bench_like_step(sc)
+    r = oracle.render(cfg, sc, ambiguity_eps=AMB_EPS)
+    check_project_fwd(st, r["proj"], "object", sc)
+    # binning: the CUDA path fed the ORACLE's projected records must give the oracle's lists bit for bit
+    from test_gpu_parity import run_bin
+    Mo, M_dev, gk, gv, gr = run_bin(B, sc, r["rec"], r["proj"]["radii"], capacity=len(r["keys"]) + 4096, sync=False)
+    assert M_dev == len(r["keys"])
+    np.testing.assert_array_equal(gk[:M_dev], r["keys"])
+    np.testing.assert_array_equal(gv[:M_dev], r["vals"])
+    np.testing.assert_array_equal(gr, r["ranges"])
+    assert abs(M - len(r["keys"])) <= 1e-3 * len(r["keys"])
+    # image of the chained step
+    gi = st.image.cpu().numpy()
+    clear = r["ambiguous"] == 0
+    err = np.abs(gi - r["image"]).max(axis=-1)
+    frac_bad = (err[clear] > 1e-4).mean()
+    assert frac_bad <= 2e-3, frac_bad
+    assert np.median(err) <= 2e-6
+    # gradients of the L1 loss
+    tgt = scenes.target_image(sc)
+    diff = r["image"] - tgt.astype(np.float64)
+    dL = np.sign(diff) / diff.size
+    g2 = oracle.raster_bwd(cfg, sc["cameras"], r["vals"], r["ranges"], r["rec"]["means2d"], r["rec"]["conics"],
+                           r["rec"]["opacities"], r["rec"]["rgbs"], sc["bg"], r["final_T"].astype(np.float32), r["n_contrib"], dL)
+    gp = oracle.project_bwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], sc["cameras"],
+                            r["proj"]["radii"], g2["means2d"], g2["conics"], g2["opacities"], g2["rgbs"])
+    loss_ref = np.abs(diff).mean()
+    assert abs(float(st.loss.item()) - loss_ref) <= 1e-5 * max(loss_ref, 1e-3)
+    errs = {k: rel_l2(st.grads[k].cpu().numpy(), gp[k]) for k in gp}
+    print(f"[object] M {M}; image err>1e-4 frac {frac_bad:.2e}; grad rel L2 {errs}")
+    for k, e in errs.items():
+        assert e <= 1e-3, (k, e)
+
+
+# ------------------------------------------------------------------------------------ room / block: sampled
+def tile_list_from_definition(t, view, N, gx, gy, means2d, depths, radii):
+    """Entries (e = view*N + i) of tile t of one view in the order O-B defines, rebuilt from the stored
+    fp32 means and integer radii: rectangle overlap test, then stable order by (depth bits, entry)."""
+    ty, tx = divmod(t, gx)
+    u = means2d[view, :, 0].astype(np.float32); v = means2d[view, :, 1].astype(np.float32)
+    r = radii[view]
+    vis = r > 0
+    inv = np.float32(1.0 / 16.0)
+    rl = r.astype(np.float32); rh = (r + 15).astype(np.float32)
+    with np.errstate(invalid="ignore", over="ignore"):
+        x0 = np.clip(np.floor((u - rl) * inv), 0, gx); x1 = np.clip(np.floor((u + rh) * inv), 0, gx)
+        y0 = np.clip(np.floor((v - rl) * inv), 0, gy); y1 = np.clip(np.floor((v + rh) * inv), 0, gy)
+    hit = vis & (x0 <= tx) & (tx < x1) & (y0 <= ty) & (ty < y1)
+    idx = np.nonzero(hit)[0]
+    bits = depths[view, idx].astype(np.float32).view(np.uint32)
+    order = np.lexsort((idx, bits))
+    return (view * N + idx[order]).astype(np.int32)
+
+
+@pytest.mark.parametrize("workload,stride", [("room", 211), ("block", 97)])
+def test_full_size_sampled(B, oracle, workload, stride):
+    sc = scenes.make_scene(workload)
+    cfg = oracle.make_cfg(sh_degree=sc["sh_degree"])
+    cams = sc["cameras"]
+    C, N = len(cams), sc["means"].shape[0]
+    st, M = bench_like_step(sc)
+    # ---- P1 on every entry
+    ref = oracle.project_fwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], cams)
+    got = check_project_fwd(st, ref, workload, sc)
+    del ref
+    # ---- binning: properties at full size
+    gx, gy = st.gx, st.gy
+    tiles = gx * gy
+    ranges = st.tile_ranges.cpu().numpy()
+    vals = st.isect_vals.cpu().numpy()[:M]
+    lens = ranges[:, 1] - ranges[:, 0]
+    nz = lens > 0
+    assert lens.min() >= 0 and int(lens.sum()) == M
+    assert np.all(ranges[~nz] == 0)
+    starts = ranges[nz, 0]
+    assert starts[0] == 0 and np.array_equal(starts[1:], ranges[nz, 1][:-1]) and ranges[nz, 1][-1] == M   # partition in tile order
+    assert int(got["tiles_touched"].astype(np.int64).sum()) == M
+    d_sorted = got["depths"].reshape(-1)[vals]
+    inside = np.ones(M, bool)
+    inside[starts] = False                                     # first record of every list
+    assert np.all((np.diff(d_sorted) >= 0) | ~inside[1:])      # depth never decreases inside a list
+    # ---- binning: sampled tiles rebuilt one by one from the definition (bit-exact)
+    sample = np.arange(0, C * tiles, stride)
+    n_checked = 0
+    for bt in sample[:: max(1, len(sample) // 48)]:
+        view, t = divmod(int(bt), tiles)
+        want = tile_list_from_definition(t, view, N, gx, gy, got["means2d"], got["depths"], got["radii"])
+        np.testing.assert_array_equal(vals[ranges[bt, 0]:ranges[bt, 1]], want)
+        n_checked += 1
+    # ---- R1 / R2 on sampled tiles: oracle fed the CUDA path's records and lists
+    mask = np.zeros(C * tiles, np.uint8)
+    mask[sample] = 1
+    rec = {k: got[k] for k in ("means2d", "conics", "opacities", "rgbs")}
+    img, T, nc, amb = oracle.raster_fwd(cfg, cams, vals, ranges, rec["means2d"], rec["conics"], rec["opacities"], rec["rgbs"],
+                                        sc["bg"], ambiguity_eps=AMB_EPS, tile_mask=mask)
+    H, W = st.H, st.W
+    tm = mask.reshape(C, gy, gx).astype(bool)
+    pm = np.repeat(np.repeat(tm, 16, axis=1), 16, axis=2)[:, :H, :W]   # pixel mask of the sampled tiles
+    gi, gT, gn = st.image.cpu().numpy(), st.final_T.cpu().numpy(), st.n_contrib.cpu().numpy()
+    clear = pm & (amb == 0)
+    err = np.abs(gi - img).max(axis=-1)
+    assert err[clear].max() <= 1e-4, err[clear].max()
+    assert np.abs(gT - T)[clear].max() <= 1e-4
+    assert np.array_equal(gn[clear], nc[clear])
+    if (pm & ~clear).any():
+        assert err[pm & (amb != 0)].max() <= 2e-2
+    assert clear.sum() > 0.99 * pm.sum()
+    # backward: dL/dimage is zero outside the sampled tiles, so both sides sum the same pixels
+    rng = np.random.default_rng(5)
+    dL = np.zeros((C, H, W, 3), np.float32)
+    dL[pm] = (rng.standard_normal((int(pm.sum()), 3)) / (H * W)).astype(np.float32)
+    st.dL_dimage.copy_(torch.from_numpy(dL))
+    st.raster_bwd()
+    st.project_bwd()
+    torch.cuda.synchronize()
+    ref2 = oracle.raster_bwd(cfg, cams, vals, ranges, rec["means2d"], rec["conics"], rec["opacities"], rec["rgbs"], sc["bg"],
+                             gT, gn, dL, tile_mask=mask)
+    vis = got["radii"] > 0
+    g2 = {"means2d": st.g_means2d, "conics": st.g_conics, "opacities": st.g_opacities, "rgbs": st.g_rgbs}
+    g2 = {k: v.cpu().numpy() for k, v in g2.items()}
+    e2 = {k: rel_l2(g2[k][vis], ref2[k][vis]) for k in ref2}
+    for k, e in e2.items():
+        assert e <= 1e-3, (k, e)
+    # ---- P5 on every Gaussian, fed the CUDA path's 2-D gradients (rows of culled entries are never read)
+    g2z = {k: np.where(vis[..., None] if v.ndim == 3 else vis, v, 0.0) for k, v in g2.items()}
+    gp = oracle.project_bwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], cams,
+                            got["radii"], g2z["means2d"], g2z["conics"], g2z["opacities"], g2z["rgbs"])
+    anyvis = vis.any(axis=0)
+    e5 = {}
+    for k in gp:
+        g = st.grads[k].cpu().numpy()
+        assert np.all(g[~anyvis] == 0)                        # dense overwrite
+        e5[k] = rel_l2(g, gp[k])
+        assert e5[k] <= 1e-3, (k, e5[k])
+    print(f"[{workload}] M {M}; {n_checked} tile lists exact; {int(pm.sum())} pixels on {len(sample)} tiles, max err "
+          f"{err[clear].max():.2e}, ambiguous {int((pm & ~clear).sum())}; R2 rel L2 {e2}; P5 rel L2 {e5}")

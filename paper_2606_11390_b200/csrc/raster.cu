@@ -179,53 +179,99 @@ struct RasterBwdIO {
     float* g_means2d; float* g_conics; float* g_opacities; float* g_rgbs;
 };
 
-// Reduce 9 per-lane values over the warp.  Values 0..7 use a splitting butterfly (each exchange
-// halves the number of values a lane carries): 4 + 2 + 1 + 1 + 1 shuffles; value 8 takes the plain
-// 5-step butterfly.  On return lane (4*k) holds the warp total of value k (k = 0..7, bit pattern
-// k = lane bits 4..2) in `out8`, and every lane holds the total of value 8 in `out9`.
-__device__ __forceinline__ void warp_reduce9(const float v[9], int lane, float& out8, float& out9) {
-    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
-    float a0, a1, a2, a3;
-    {
-        const float s0 = b4 ? v[0] : v[4], s1 = b4 ? v[1] : v[5], s2 = b4 ? v[2] : v[6], s3 = b4 ? v[3] : v[7];
-        const float k0 = b4 ? v[4] : v[0], k1 = b4 ? v[5] : v[1], k2 = b4 ? v[6] : v[2], k3 = b4 ? v[7] : v[3];
-        a0 = k0 + __shfl_xor_sync(0xffffffffu, s0, 16);
-        a1 = k1 + __shfl_xor_sync(0xffffffffu, s1, 16);
-        a2 = k2 + __shfl_xor_sync(0xffffffffu, s2, 16);
-        a3 = k3 + __shfl_xor_sync(0xffffffffu, s3, 16);
-    }
-    float c0, c1;
-    {
-        const float s0 = b3 ? a0 : a2, s1 = b3 ? a1 : a3;
-        const float k0 = b3 ? a2 : a0, k1 = b3 ? a3 : a1;
-        c0 = k0 + __shfl_xor_sync(0xffffffffu, s0, 8);
-        c1 = k1 + __shfl_xor_sync(0xffffffffu, s1, 8);
-    }
-    float e;
-    {
-        const float s = b2 ? c0 : c1;
-        const float k = b2 ? c1 : c0;
-        e = k + __shfl_xor_sync(0xffffffffu, s, 4);
-    }
-    e += __shfl_xor_sync(0xffffffffu, e, 2);
-    e += __shfl_xor_sync(0xffffffffu, e, 1);
-    out8 = e;
-    float w = v[8];
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) w += __shfl_xor_sync(0xffffffffu, w, d);
-    out9 = w;
-}
-
-constexpr int kBwdBatch = 128;              // records staged per batch in the backward kernel
+// ---- backward reduction ----------------------------------------------------------------------
+// Per (pixel, record) pair the backward pass produces two scalars: gp = dL/dpower and wgt = alpha*T
+// (the weight of dL/dimage in dL/drgb).  Every per-record sum is a contraction of those over the
+// pixels: with pixel offsets (x, y) from the tile centre, the geometric gradients need the moments
+// sum gp*{1, x, y, x^2, xy, y^2} and dL/drgb needs sum wgt*g_c -- 9 values.  Instead of a 32-lane
+// butterfly per record (14 shuffles), a warp TRANSPOSES: lane = pixel writes (gp, wgt) of up to 8
+// records into a shared-memory tile, then lane (record g, pixel row t) reads its row of 8 pixels
+// (2+2 LDS.128), accumulates the moments with immediate x offsets (FFMA), and only the 4 lanes of a
+// record are combined by shuffles (value-splitting, 8 shuffles per 8 records).
+constexpr int kBwdBatch = 64;               // records staged per batch in the backward kernel
 constexpr int kBwdChunks = kBwdBatch / 32;
 constexpr int kWarps = kBlock / 32;
+constexpr int kGroup = 8;                   // records reduced together by one warp
+constexpr int kTStride = 36;                // floats per transposition row: 32 pixels + 4 (bank spread for LDS.128)
+constexpr int kGStride = 28;                // floats per row of staged dL/dimage: 3 x 8 + 4
+constexpr int kSlot = 9;                    // floats per (warp, record) slot (odd stride: conflict-free flush)
 
 struct BwdSmem {
     Rec rec[kBwdBatch];
-    float slot[kWarps][kBwdBatch][9];       // per-warp partial sums of a record: du, dv, dA, dB, dC, o*do, dr, dg, db
+    float slot[kWarps][kBwdBatch][kSlot];   // m0, m1x, m1y, m2xx, m2xy, m2yy, dr, dg, (db at [8])
+    float tbuf[kWarps][2 * kGroup][kTStride];   // rows 0..7: gp of record k over the warp's 32 pixels; rows 8..15: wgt
+    float gpix[kWarps][4][kGStride];        // dL/dimage of the warp's pixels: row t holds g0[8], g1[8], g2[8]
+    int qlist[kWarps][kGroup];              // position in the batch of the k-th record of the group
     unsigned int vis[kWarps][kBwdChunks];   // which records of the batch a warp wrote
     int max_contrib;
 };
+
+__device__ __forceinline__ void sts32(uint32_t addr, float v) {
+    asm volatile("st.shared.f32 [%0], %1;" :: "r"(addr), "f"(v));
+}
+
+// Reduce the k (<= 8) records of a warp's group; `pyt` = this lane's row offset from the tile centre
+// (lane = 4*g + t: record g, pixel row t), `ox` = x offset of the warp's 8 columns' centre.
+__device__ __forceinline__ void reduce_group(BwdSmem& sm, int warp, int lane, int k, float ox, float pyt) {
+    __syncwarp();
+    const int g = lane >> 2, t = lane & 3;
+    const uint32_t tb = (uint32_t)__cvta_generic_to_shared(&sm.tbuf[warp][g][t * 8]);
+    const float4 p0 = lds128(tb), p1 = lds128(tb + 16);
+    const float4 w0 = lds128(tb + kGroup * kTStride * 4), w1 = lds128(tb + kGroup * kTStride * 4 + 16);
+    const uint32_t gb = (uint32_t)__cvta_generic_to_shared(&sm.gpix[warp][t][0]);
+    // moments of gp over the row, x measured from the centre of the 8 columns (-3.5 .. 3.5)
+    const float a0 = p0.x + p1.w, a1 = p0.y + p1.z, a2 = p0.z + p1.y, a3 = p0.w + p1.x;
+    const float d0 = p1.w - p0.x, d1 = p1.z - p0.y, d2 = p1.y - p0.z, d3 = p1.x - p0.w;
+    const float s0 = (a0 + a1) + (a2 + a3);
+    const float s1 = fmaf(3.5f, d0, fmaf(2.5f, d1, fmaf(1.5f, d2, 0.5f * d3)));
+    const float s2 = fmaf(12.25f, a0, fmaf(6.25f, a1, fmaf(2.25f, a2, 0.25f * a3)));
+    float v[9];
+    // shift to the tile centre: x_t = x + ox, y_t = pyt
+    const float m1x = fmaf(ox, s0, s1);
+    v[0] = s0;
+    v[1] = m1x;
+    v[2] = pyt * s0;
+    v[3] = fmaf(ox, m1x + s1, s2);          // s2 + 2 ox s1 + ox^2 s0
+    v[4] = pyt * m1x;
+    v[5] = pyt * v[2];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float4 ga = lds128(gb + c * 32), gc = lds128(gb + c * 32 + 16);
+        float acc = w0.x * ga.x;
+        acc = fmaf(w0.y, ga.y, acc); acc = fmaf(w0.z, ga.z, acc); acc = fmaf(w0.w, ga.w, acc);
+        acc = fmaf(w1.x, gc.x, acc); acc = fmaf(w1.y, gc.y, acc); acc = fmaf(w1.z, gc.z, acc); acc = fmaf(w1.w, gc.w, acc);
+        v[6 + c] = acc;
+    }
+    // combine the 4 rows (lanes t = 0..3 of the record): values 0..7 split, value 8 plain
+    const bool b1 = t & 2, b0 = t & 1;
+    float c0, c1, c2, c3;
+    {
+        const float s_0 = b1 ? v[0] : v[4], s_1 = b1 ? v[1] : v[5], s_2 = b1 ? v[2] : v[6], s_3 = b1 ? v[3] : v[7];
+        const float k_0 = b1 ? v[4] : v[0], k_1 = b1 ? v[5] : v[1], k_2 = b1 ? v[6] : v[2], k_3 = b1 ? v[7] : v[3];
+        c0 = k_0 + __shfl_xor_sync(0xffffffffu, s_0, 2);
+        c1 = k_1 + __shfl_xor_sync(0xffffffffu, s_1, 2);
+        c2 = k_2 + __shfl_xor_sync(0xffffffffu, s_2, 2);
+        c3 = k_3 + __shfl_xor_sync(0xffffffffu, s_3, 2);
+    }
+    float e0, e1;
+    {
+        const float s_0 = b0 ? c0 : c2, s_1 = b0 ? c1 : c3;
+        const float k_0 = b0 ? c2 : c0, k_1 = b0 ? c3 : c1;
+        e0 = k_0 + __shfl_xor_sync(0xffffffffu, s_0, 1);
+        e1 = k_1 + __shfl_xor_sync(0xffffffffu, s_1, 1);
+    }
+    float w = v[8];
+    w += __shfl_xor_sync(0xffffffffu, w, 2);
+    w += __shfl_xor_sync(0xffffffffu, w, 1);
+    // lane t now holds values (4*b1 + 2*b0, +1) = (2*tt, 2*tt + 1) with tt = 2*b1 + b0 = t
+    if (g < k) {
+        float* slot = &sm.slot[warp][sm.qlist[warp][g]][0];
+        slot[2 * t] = e0;
+        slot[2 * t + 1] = e1;
+        if (t == 0) slot[8] = w;
+    }
+    __syncwarp();
+}
 
 __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, const RasterBwdIO io) {
     extern __shared__ __align__(16) unsigned char bwd_smem_raw[];
@@ -240,8 +286,12 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
     const bool inside = (i < a.height) && (j < a.width);
     const float px = (float)j + 0.5f, py = (float)i + 0.5f;
     const float X0 = (float)bx0 + 0.5f, Y0 = (float)by0 + 0.5f;
+    const float xc = (float)(tx * kTile + kTile / 2), yc = (float)(ty * kTile + kTile / 2);   // tile centre
+    const float ox = (warp & 1) ? 4.0f : -4.0f;                                            // centre of the warp's columns - xc
+    const float pyt = (float)((warp >> 1) * 4 + (lane & 3)) + 0.5f - 8.0f;                 // reduce-phase row (lane & 3) - yc
     const int64_t start = __ldg(a.ranges + 2 * bt);
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.rec);
+    const uint32_t tbase = (uint32_t)__cvta_generic_to_shared(&sm.tbuf[warp][0][lane]);
     const float alpha_min = a.alpha_min, alpha_max = a.alpha_max;
 
     float T = 0.f, g0 = 0.f, g1 = 0.f, g2 = 0.f;
@@ -251,6 +301,10 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
         T = __ldg(io.final_T + pix);
         ncon = __ldg(io.n_contrib + pix);
         g0 = __ldg(io.dL_dimage + 3 * pix); g1 = __ldg(io.dL_dimage + 3 * pix + 1); g2 = __ldg(io.dL_dimage + 3 * pix + 2);
+    }
+    {
+        float* gr = &sm.gpix[warp][lane >> 3][lane & 7];
+        gr[0] = g0; gr[8] = g1; gr[16] = g2;
     }
     if (tid == 0) sm.max_contrib = 0;
     __syncthreads();
@@ -269,16 +323,18 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
         __syncthreads();   // previous batch fully flushed
         if (tid < cnt) stage_record(a, __ldg(a.vals + start + (int64_t)b * kBwdBatch + tid), sm.rec[tid]);
         __syncthreads();
+        int k = 0;         // records in the warp's current group (warp-uniform)
         for (int ch = kBwdChunks - 1; ch >= 0; --ch) {
             const int r = ch * 32 + lane;
-            unsigned int mask = __ballot_sync(0xffffffffu, r < cnt && (b * kBwdBatch + r) < wmax &&
+            const int cbase = b * kBwdBatch + ch * 32;          // list position of bit 0 of this chunk
+            unsigned int mask = __ballot_sync(0xffffffffu, r < cnt && (cbase + lane) < wmax &&
                                                                rect_may_contribute(sm.rec[r].a, sm.rec[r].b, X0, Y0, a.filter_thr));
+            const int nrel = ncon - cbase;                      // this pixel walks bits < nrel
             unsigned int written = 0;
             while (mask) {
                 const int bit = 31 - __clz(mask);
                 mask ^= 1u << bit;
                 const int q = ch * 32 + bit;
-                const int idx = b * kBwdBatch + q;           // position of the record in the tile's list
                 const uint32_t addr = sbase + (uint32_t)q * (uint32_t)sizeof(Rec);
                 const float4 ga = lds128(addr);
                 const float4 gb = lds128(addr + 16);
@@ -286,64 +342,66 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                 const float e = quad_form(ga.z, ga.w, gb.x, dx, dy);
                 const float raw = ex2_approx(e + gb.y);
                 const float alpha = fminf(alpha_max, raw);
-                const bool valid = (idx < ncon) && !(e > 0.0f) && !(alpha < alpha_min);
+                const bool valid = (bit < nrel) && !(e > 0.0f) && !(alpha < alpha_min);
                 if (!__any_sync(0xffffffffu, valid)) continue;
                 const float cb = lds32(addr + 32);
-                float v[9];
                 // quantities of an invalid lane are computed but selected away
                 const float Tf = T * rcp_approx(1.0f - alpha);   // transmittance in front of this record
-                const float wgt = valid ? alpha * Tf : 0.0f;
-                v[6] = wgt * g0; v[7] = wgt * g1; v[8] = wgt * g2;
                 const float d0 = gb.z - S0, d1 = gb.w - S1, d2 = cb - S2;
-                const float dL_dalpha = Tf * (d0 * g0 + d1 * g1 + d2 * g2);
+                const float dL_dalpha = Tf * fmaf(d2, g2, fmaf(d1, g1, d0 * g0));
                 const float am = valid ? alpha : 0.0f;
                 S0 = fmaf(am, d0, S0);
                 S1 = fmaf(am, d1, S1);
                 S2 = fmaf(am, d2, S2);
                 T = valid ? Tf : T;
                 // no gradient through the alpha_max clamp
-                const float gp = (valid && !(raw > alpha_max)) ? alpha * dL_dalpha : 0.0f;   // dL/dpower
-                v[5] = gp;                                       // = o * dL/do  (divided by o at the flush)
-                const float hx = dx * gp, hy = dy * gp;
-                v[2] = -0.5f * dx * hx;
-                v[3] = -dx * hy;
-                v[4] = -0.5f * dy * hy;
-                const float gs = gp * kLn2;                      // A dx + B dy = -(2A' dx + B' dy) ln 2
-                v[0] = fmaf(2.0f * ga.z, dx, ga.w * dy) * gs;
-                v[1] = fmaf(2.0f * gb.x, dy, ga.w * dx) * gs;
-                float r8, r9;
-                warp_reduce9(v, lane, r8, r9);
-                float* slot = &sm.slot[warp][q][0];
-                if ((lane & 3) == 0) slot[lane >> 2] = r8;
-                if (lane == 1) slot[8] = r9;
+                const float gp = (raw > alpha_max) ? 0.0f : am * dL_dalpha;   // dL/dpower
+                sts32(tbase + (uint32_t)k * (kTStride * 4), gp);
+                sts32(tbase + (uint32_t)(k + kGroup) * (kTStride * 4), am * Tf);
+                if (lane == 0) sm.qlist[warp][k] = q;
                 written |= 1u << bit;
+                if (++k == kGroup) {
+                    reduce_group(sm, warp, lane, kGroup, ox, pyt);
+                    k = 0;
+                }
             }
             if (lane == 0) sm.vis[warp][ch] = written;
         }
+        if (k) reduce_group(sm, warp, lane, k, ox, pyt);
         __syncthreads();
         if (tid < cnt) {
-            float acc[9];
+            float m[9];
 #pragma unroll
-            for (int k = 0; k < 9; ++k) acc[k] = 0.f;
+            for (int c = 0; c < 9; ++c) m[c] = 0.f;
             bool any = false;
 #pragma unroll
             for (int w = 0; w < kWarps; ++w)
                 if ((sm.vis[w][tid >> 5] >> (tid & 31)) & 1u) {
                     any = true;
 #pragma unroll
-                    for (int k = 0; k < 9; ++k) acc[k] += sm.slot[w][tid][k];
+                    for (int c = 0; c < 9; ++c) m[c] += sm.slot[w][tid][c];
                 }
             if (any) {
-                const int64_t g = __float_as_int(sm.rec[tid].c.z);
-                if (acc[0] != 0.f) atomicAdd(io.g_means2d + 2 * g, acc[0]);
-                if (acc[1] != 0.f) atomicAdd(io.g_means2d + 2 * g + 1, acc[1]);
-                if (acc[2] != 0.f) atomicAdd(io.g_conics + 3 * g, acc[2]);
-                if (acc[3] != 0.f) atomicAdd(io.g_conics + 3 * g + 1, acc[3]);
-                if (acc[4] != 0.f) atomicAdd(io.g_conics + 3 * g + 2, acc[4]);
-                if (acc[5] != 0.f) atomicAdd(io.g_opacities + g, acc[5] / sm.rec[tid].c.y);
-                if (acc[6] != 0.f) atomicAdd(io.g_rgbs + 3 * g, acc[6]);
-                if (acc[7] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 1, acc[7]);
-                if (acc[8] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 2, acc[8]);
+                const Rec& rc = sm.rec[tid];
+                const int64_t g = __float_as_int(rc.c.z);
+                // moments about the tile centre -> sums of gp*{dx, dy, dx^2, dx dy, dy^2}, dx = u - x
+                const float ut = rc.a.x - xc, vt = rc.a.y - yc;
+                const float Dx = fmaf(ut, m[0], -m[1]), Dy = fmaf(vt, m[0], -m[2]);
+                const float Dxx = fmaf(ut, Dx - m[1], m[3]);                       // ut^2 m0 - 2 ut m1x + m2xx
+                const float Dxy = fmaf(vt, Dx, fmaf(-ut, m[2], m[4]));             // ut vt m0 - vt m1x - ut m1y + m2xy
+                const float Dyy = fmaf(vt, Dy - m[2], m[5]);
+                // A dx + B dy = -(2A' dx + B' dy) ln 2 with the staged log2-domain conic
+                const float gu = fmaf(2.0f * rc.a.z, Dx, rc.a.w * Dy) * kLn2;
+                const float gv = fmaf(2.0f * rc.b.x, Dy, rc.a.w * Dx) * kLn2;
+                if (gu != 0.f) atomicAdd(io.g_means2d + 2 * g, gu);
+                if (gv != 0.f) atomicAdd(io.g_means2d + 2 * g + 1, gv);
+                if (Dxx != 0.f) atomicAdd(io.g_conics + 3 * g, -0.5f * Dxx);
+                if (Dxy != 0.f) atomicAdd(io.g_conics + 3 * g + 1, -Dxy);
+                if (Dyy != 0.f) atomicAdd(io.g_conics + 3 * g + 2, -0.5f * Dyy);
+                if (m[0] != 0.f) atomicAdd(io.g_opacities + g, m[0] / rc.c.y);
+                if (m[6] != 0.f) atomicAdd(io.g_rgbs + 3 * g, m[6]);
+                if (m[7] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 1, m[7]);
+                if (m[8] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 2, m[8]);
             }
         }
     }

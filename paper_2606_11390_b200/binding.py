@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgsplat_b200.so")
+LIB_PATH = os.path.join(_HERE, os.environ.get("GS_LIB_NAME", "libgsplat_b200.so"))   # GS_LIB_NAME: tuning builds
 
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 

@@ -57,6 +57,8 @@ __device__ __forceinline__ float quad_form(float A, float B, float C, float dx, 
 // Can the record contribute to any pixel centre of the rectangle [X0, X0+7] x [Y0, Y0+3]?
 // g0 = (u, v, A', B'), g1.x = C', g1.y = log2(opacity).  Exact maximum of the concave exponent over
 // the rectangle (inside -> 0, otherwise on the edge(s) facing the mean), compared with a margin.
+// The stationary point along an edge uses an approximate reciprocal: an error eps in its position
+// lowers the bound by |C'| eps^2, far inside the margin; a NaN (0/0) falls back to the end points.
 __device__ __forceinline__ bool rect_may_contribute(const float4 g0, const float4 g1, float X0, float Y0, float thr) {
     const float A = g0.z, B = g0.w, C = g1.x;
     const float dx0 = g0.x - (X0 + 7.0f), dx1 = g0.x - X0;
@@ -68,12 +70,12 @@ __device__ __forceinline__ bool rect_may_contribute(const float4 g0, const float
         emax = -3.0e38f;
         if (!inx) {
             const float dxe = dx0 > 0.0f ? dx0 : dx1;
-            const float dys = fminf(fmaxf(-B * dxe / (2.0f * C), dy0), dy1);
+            const float dys = fminf(fmaxf(-0.5f * B * dxe * rcp_approx(C), dy0), dy1);
             emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxe, dys), fmaxf(quad_form(A, B, C, dxe, dy0), quad_form(A, B, C, dxe, dy1))));
         }
         if (!iny) {
             const float dye = dy0 > 0.0f ? dy0 : dy1;
-            const float dxs = fminf(fmaxf(-B * dye / (2.0f * A), dx0), dx1);
+            const float dxs = fminf(fmaxf(-0.5f * B * dye * rcp_approx(A), dx0), dx1);
             emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxs, dye), fmaxf(quad_form(A, B, C, dx0, dye), quad_form(A, B, C, dx1, dye))));
         }
     }
@@ -87,6 +89,12 @@ struct __align__(16) Rec {
     float4 c;   // b, opacity, bit pattern of the entry id, unused
 };
 
+// position of the most significant set bit (x != 0)
+__device__ __forceinline__ int msb(unsigned int x) {
+    int r;
+    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
@@ -188,7 +196,10 @@ struct RasterBwdIO {
 // records into a shared-memory tile, then lane (record g, pixel row t) reads its row of 8 pixels
 // (2+2 LDS.128), accumulates the moments with immediate x offsets (FFMA), and only the 4 lanes of a
 // record are combined by shuffles (value-splitting, 8 shuffles per 8 records).
-constexpr int kBwdBatch = 64;               // records staged per batch in the backward kernel
+#ifndef GS_BWD_BATCH
+#define GS_BWD_BATCH 64
+#endif
+constexpr int kBwdBatch = GS_BWD_BATCH;     // records staged per batch in the backward kernel
 constexpr int kBwdChunks = kBwdBatch / 32;
 constexpr int kWarps = kBlock / 32;
 constexpr int kGroup = 8;                   // records reduced together by one warp
@@ -201,7 +212,6 @@ struct BwdSmem {
     float slot[kWarps][kBwdBatch][kSlot];   // m0, m1x, m1y, m2xx, m2xy, m2yy, dr, dg, (db at [8])
     float tbuf[kWarps][2 * kGroup][kTStride];   // rows 0..7: gp of record k over the warp's 32 pixels; rows 8..15: wgt
     float gpix[kWarps][4][kGStride];        // dL/dimage of the warp's pixels: row t holds g0[8], g1[8], g2[8]
-    int qlist[kWarps][kGroup];              // position in the batch of the k-th record of the group
     unsigned int vis[kWarps][kBwdChunks];   // which records of the batch a warp wrote
     int max_contrib;
 };
@@ -212,7 +222,8 @@ __device__ __forceinline__ void sts32(uint32_t addr, float v) {
 
 // Reduce the k (<= 8) records of a warp's group; `pyt` = this lane's row offset from the tile centre
 // (lane = 4*g + t: record g, pixel row t), `ox` = x offset of the warp's 8 columns' centre.
-__device__ __forceinline__ void reduce_group(BwdSmem& sm, int warp, int lane, int k, float ox, float pyt) {
+// `myq` = position in the batch of record g.
+__device__ __forceinline__ void reduce_group(BwdSmem& sm, int warp, int lane, int k, int myq, float ox, float pyt) {
     __syncwarp();
     const int g = lane >> 2, t = lane & 3;
     const uint32_t tb = (uint32_t)__cvta_generic_to_shared(&sm.tbuf[warp][g][t * 8]);
@@ -265,7 +276,7 @@ __device__ __forceinline__ void reduce_group(BwdSmem& sm, int warp, int lane, in
     w += __shfl_xor_sync(0xffffffffu, w, 1);
     // lane t now holds values (4*b1 + 2*b0, +1) = (2*tt, 2*tt + 1) with tt = 2*b1 + b0 = t
     if (g < k) {
-        float* slot = &sm.slot[warp][sm.qlist[warp][g]][0];
+        float* slot = &sm.slot[warp][myq][0];
         slot[2 * t] = e0;
         slot[2 * t + 1] = e1;
         if (t == 0) slot[8] = w;
@@ -324,6 +335,8 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
         if (tid < cnt) stage_record(a, __ldg(a.vals + start + (int64_t)b * kBwdBatch + tid), sm.rec[tid]);
         __syncthreads();
         int k = 0;         // records in the warp's current group (warp-uniform)
+        int myq = 0;       // batch position of the group's record (lane >> 2)
+        uint32_t taddr = tbase;   // this lane's cell in row k of the transposition tile
         for (int ch = kBwdChunks - 1; ch >= 0; --ch) {
             const int r = ch * 32 + lane;
             const int cbase = b * kBwdBatch + ch * 32;          // list position of bit 0 of this chunk
@@ -331,11 +344,11 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                                                                rect_may_contribute(sm.rec[r].a, sm.rec[r].b, X0, Y0, a.filter_thr));
             const int nrel = ncon - cbase;                      // this pixel walks bits < nrel
             unsigned int written = 0;
+            const uint32_t cbase_addr = sbase + (uint32_t)(ch * 32) * (uint32_t)sizeof(Rec);
             while (mask) {
-                const int bit = 31 - __clz(mask);
+                const int bit = msb(mask);
                 mask ^= 1u << bit;
-                const int q = ch * 32 + bit;
-                const uint32_t addr = sbase + (uint32_t)q * (uint32_t)sizeof(Rec);
+                const uint32_t addr = cbase_addr + (uint32_t)bit * (uint32_t)sizeof(Rec);
                 const float4 ga = lds128(addr);
                 const float4 gb = lds128(addr + 16);
                 const float dx = ga.x - px, dy = ga.y - py;
@@ -356,18 +369,20 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                 T = valid ? Tf : T;
                 // no gradient through the alpha_max clamp
                 const float gp = (raw > alpha_max) ? 0.0f : am * dL_dalpha;   // dL/dpower
-                sts32(tbase + (uint32_t)k * (kTStride * 4), gp);
-                sts32(tbase + (uint32_t)(k + kGroup) * (kTStride * 4), am * Tf);
-                if (lane == 0) sm.qlist[warp][k] = q;
+                sts32(taddr, gp);
+                sts32(taddr + kGroup * kTStride * 4, am * Tf);
+                taddr += kTStride * 4;
+                myq = (k == (lane >> 2)) ? ch * 32 + bit : myq;
                 written |= 1u << bit;
                 if (++k == kGroup) {
-                    reduce_group(sm, warp, lane, kGroup, ox, pyt);
+                    reduce_group(sm, warp, lane, kGroup, myq, ox, pyt);
                     k = 0;
+                    taddr = tbase;
                 }
             }
             if (lane == 0) sm.vis[warp][ch] = written;
         }
-        if (k) reduce_group(sm, warp, lane, k, ox, pyt);
+        if (k) reduce_group(sm, warp, lane, k, myq, ox, pyt);
         __syncthreads();
         if (tid < cnt) {
             float m[9];

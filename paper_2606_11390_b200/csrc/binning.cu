@@ -286,62 +286,142 @@ struct CompactArgs {
     unsigned int n_blocks;
 };
 
+// Warp-striped arrangement: warp w of the block covers 128 * VEC consecutive entries; in iteration
+// j lane l holds entries (j * 128 + l * 4 .. + 3) of that span as one 16-byte load, so that the VEC
+// loads of a thread are all in flight together (memory-level parallelism) and every warp request is
+// 512 contiguous bytes.  Phase 1: visibility (radius > 0 and a non-empty tile rectangle) as one bit
+// per entry, corner differences of the rectangle.  Phase 2 (after the ordered chained scan of the
+// per-block counts): the visible entries' (view | depth, entry) pairs go to their ranks; ranks keep
+// ascending entry order (iteration, lane, component).
+template <int VEC>
 __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs a) {
+    constexpr int TILE = kScanThreads * 4 * VEC;
+    constexpr int WARPS = kScanThreads / 32;
     __shared__ unsigned int s_ticket;
-    __shared__ ChainScanSmem s_scan;
-    const int tid = threadIdx.x;
+    __shared__ unsigned int s_warp[WARPS];
+    __shared__ unsigned long long s_base;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_ticket = atomicAdd(&a.hdr->compact_ticket, 1u);
     __syncthreads();
     const int64_t tile = s_ticket;
-    const int64_t e0 = tile * kScanTile + (int64_t)tid * kScanItems;
+    const int64_t w0 = tile * TILE + (int64_t)warp * (128 * VEC) + lane * 4;
 
-    int rad[kScanItems];
-    if (e0 + kScanItems <= a.n_entries) {
-        const int4 r4 = __ldg(reinterpret_cast<const int4*>(a.radii + e0));
-        rad[0] = r4.x; rad[1] = r4.y; rad[2] = r4.z; rad[3] = r4.w;
-    } else {
+    int4 rad[VEC];
 #pragma unroll
-        for (int k = 0; k < kScanItems; ++k) rad[k] = (e0 + k < a.n_entries) ? __ldg(a.radii + e0 + k) : 0;
+    for (int j = 0; j < VEC; ++j) {
+        const int64_t e = w0 + j * 128;
+        if (e + 4 <= a.n_entries) {
+            rad[j] = __ldg(reinterpret_cast<const int4*>(a.radii + e));
+        } else {
+            rad[j].x = (e < a.n_entries) ? __ldg(a.radii + e) : 0;
+            rad[j].y = (e + 1 < a.n_entries) ? __ldg(a.radii + e + 1) : 0;
+            rad[j].z = (e + 2 < a.n_entries) ? __ldg(a.radii + e + 2) : 0;
+            rad[j].w = 0;
+        }
     }
-    unsigned long long key[kScanItems];
-    unsigned int vis_mask = 0, t_vis = 0;
     const int sx = a.gx + 1, sy = a.gy + 1;
+    unsigned int cand = 0;         // bit 4 j + k: entry w0 + 128 j + k has a positive radius
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        key[k] = 0;
-        if (rad[k] > 0) {
-            const int64_t e = e0 + k;
-            const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + e);
-            int x0, x1, y0, y1;
-            tile_rect(uv.x, uv.y, rad[k], a.gx, a.gy, x0, x1, y0, y1);
-            if (x1 > x0 && y1 > y0) {
-                const int64_t view = e / a.N;
-                key[k] = ((unsigned long long)view << 32) | (unsigned long long)__float_as_uint(__ldg(a.depths + e));
-                vis_mask |= 1u << k;
-                ++t_vis;
-                int* g = a.tdiff + view * (int64_t)sx * sy;
-                atomicAdd(g + y0 * sx + x0, 1);
-                atomicAdd(g + y0 * sx + x1, -1);
-                atomicAdd(g + y1 * sx + x0, -1);
-                atomicAdd(g + y1 * sx + x1, 1);
+    for (int j = 0; j < VEC; ++j)
+        cand |= ((rad[j].x > 0 ? 1u : 0u) | (rad[j].y > 0 ? 2u : 0u) | (rad[j].z > 0 ? 4u : 0u) | (rad[j].w > 0 ? 8u : 0u)) << (4 * j);
+    // one copy of the per-candidate code (a loop over the set bits, not an unrolled chain: in the
+    // large-scene regime a fraction of a per cent of the entries is visible and the instruction
+    // footprint of the skip path is what matters); C * N < 2^31, so 32-bit division gives the view
+    unsigned int vis = 0;          // candidates with a non-empty tile rectangle
+    const unsigned int n32 = (unsigned int)a.N;
+    while (cand) {
+        const int bit = __ffs(cand) - 1;
+        cand &= cand - 1;
+        const int64_t e = w0 + (bit >> 2) * 128 + (bit & 3);
+        const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + e);
+        int x0, x1, y0, y1;
+        tile_rect(uv.x, uv.y, __ldg(a.radii + e), a.gx, a.gy, x0, x1, y0, y1);
+        if (x1 > x0 && y1 > y0) {
+            vis |= 1u << bit;
+            int* g = a.tdiff + (int64_t)((unsigned int)e / n32) * ((int64_t)sx * sy);
+            atomicAdd(g + y0 * sx + x0, 1);
+            atomicAdd(g + y0 * sx + x1, -1);
+            atomicAdd(g + y1 * sx + x0, -1);
+            atomicAdd(g + y1 * sx + x1, 1);
+        }
+    }
+    // inclusive scan over the lanes of the per-iteration counts (<= 4 each, <= 128 per warp: 8-bit
+    // fields, four iterations per word)
+    constexpr int WORDS = (VEC + 3) / 4;
+    unsigned int inc[WORDS];
+#pragma unroll
+    for (int q = 0; q < WORDS; ++q) {
+        unsigned int c = 0;
+#pragma unroll
+        for (int j = 4 * q; j < 4 * q + 4 && j < VEC; ++j) c |= (unsigned int)__popc((vis >> (4 * j)) & 15u) << (8 * (j - 4 * q));
+        // a field can reach 128 only in lane 31 of the inclusive sum: no carry into the next field
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned int o = __shfl_up_sync(0xffffffffu, c, d);
+            if (lane >= d) c += o;
+        }
+        inc[q] = c;
+    }
+    // totals of the iterations (lane 31's fields) -> exclusive bases of the iterations inside the warp
+    unsigned int iter_base[VEC];
+    unsigned int wtotal = 0;
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) {
+        iter_base[j] = wtotal;
+        wtotal += (__shfl_sync(0xffffffffu, inc[j / 4], 31) >> (8 * (j % 4))) & 255u;
+    }
+    if (lane == 0) s_warp[warp] = wtotal;
+    __syncthreads();
+    unsigned int wbase = 0, btotal = 0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) {
+        if (w < warp) wbase += s_warp[w];
+        btotal += s_warp[w];
+    }
+    if (warp == 0) {
+        const unsigned long long excl = chained_scan_lookback(a.status, tile, btotal, lane);
+        if (lane == 0) {
+            s_base = excl;
+            if (tile == (int64_t)a.n_blocks - 1) {
+                const unsigned long long V = excl + btotal;
+                a.hdr->V = V < (unsigned long long)a.vcap ? V : (unsigned long long)a.vcap;
             }
         }
     }
-    unsigned long long block_excl, block_total;
-    unsigned long long pos = block_chained_scan(t_vis, a.status, tile, s_scan, block_excl, block_total);
-    if (tid == 0 && tile == (int64_t)a.n_blocks - 1) {
-        const unsigned long long V = block_excl + block_total;
-        a.hdr->V = V < (unsigned long long)a.vcap ? V : (unsigned long long)a.vcap;
-    }
+    if (btotal == 0) return;       // (block-uniform) nothing to write; warp 0 has published above
+    __syncthreads();
+    const unsigned long long gbase = s_base + wbase;
+    // exclusive rank of the lane's first visible entry of every iteration, 8-bit fields as above
+    unsigned int lane_excl[WORDS];
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k)
-        if ((vis_mask >> k) & 1u) {
-            if (pos < (unsigned long long)a.vcap) {
-                a.ckeys[pos] = key[k];
-                a.cvals[pos] = (int)(e0 + k);
-            }
-            ++pos;
+    for (int q = 0; q < WORDS; ++q) {
+        unsigned int own = 0;
+#pragma unroll
+        for (int j = 4 * q; j < 4 * q + 4 && j < VEC; ++j) own |= (unsigned int)__popc((vis >> (4 * j)) & 15u) << (8 * (j - 4 * q));
+        lane_excl[q] = inc[q] - own;
+    }
+    unsigned int m = vis;
+    int cur_j = -1;
+    unsigned long long pos = 0;
+    while (m) {
+        const int bit = __ffs(m) - 1;
+        m &= m - 1;
+        const int j = bit >> 2;
+        if (j != cur_j) {
+            cur_j = j;
+            unsigned int ib = 0, le = 0;
+#pragma unroll
+            for (int jj = 0; jj < VEC; ++jj)
+                if (jj == j) { ib = iter_base[jj]; le = (lane_excl[jj / 4] >> (8 * (jj % 4))) & 255u; }
+            pos = gbase + ib + le;
         }
+        const int64_t e = w0 + j * 128 + (bit & 3);
+        if (pos < (unsigned long long)a.vcap) {
+            a.ckeys[pos] = ((unsigned long long)((unsigned int)e / n32) << 32) | (unsigned long long)__float_as_uint(__ldg(a.depths + e));
+            a.cvals[pos] = (int)e;
+        }
+        ++pos;
+    }
 }
 
 // ------------------------------------------------------------------------------ B4: counts, ranges, histograms
@@ -1067,7 +1147,10 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
     tv[(tplan.P & 1) ^ 1] = reinterpret_cast<int32_t*>(ws + w.off_vals);
 
     if (cudaMemsetAsync(ws, 0, w.zero_bytes, st) != cudaSuccess) return GS_ERR_CUDA;
-    const int64_t n_blocks = (n_entries + kScanTile - 1) / kScanTile;
+    // compaction tile: the largest of 1, 2, 4, 8 x 1024 entries per block that still gives 8 blocks per SM
+    int cvec = 8;
+    while (cvec > 1 && n_entries < (int64_t)kScanTile * cvec * sms * 8) cvec >>= 1;
+    const int64_t n_blocks = (n_entries + (int64_t)kScanTile * cvec - 1) / ((int64_t)kScanTile * cvec);
     if (n_blocks > 0) {
         CompactArgs a;
         a.n_entries = n_entries; a.N = N; a.gx = gx; a.gy = gy;
@@ -1076,7 +1159,12 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
         a.tdiff = tdiff;
         a.hdr = hdr; a.status = status_at(w.off_compact_status);
         a.n_blocks = (unsigned int)n_blocks;
-        compact_kernel<<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a);
+        switch (cvec) {
+            case 8: compact_kernel<8><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
+            case 4: compact_kernel<4><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
+            case 2: compact_kernel<2><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
+            default: compact_kernel<1><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
+        }
         rc = launch_status();
         if (rc) return rc;
     }

@@ -181,6 +181,185 @@ __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, 
     }
 }
 
+// ---- packed FP32 (two pixels per lane) ---------------------------------------------------------
+// sm_100a has two-wide FP32 instructions (FFMA2 / FMUL2 / FADD2 on 64-bit register pairs; PTX
+// fma/mul/add.rn.f32x2).  The raster kernels are issue bound, so a lane owns two horizontally
+// adjacent pixels and evaluates the exponent, the transmittance update and the colour sums of both
+// with one instruction each.  Records are staged with every field duplicated so that one LDS.128
+// yields two ready-made operand pairs.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ void lds2x64(uint32_t addr, f32x2& a, f32x2& b) {
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
+}
+__device__ __forceinline__ f32x2 lds64(uint32_t addr) {
+    f32x2 a;
+    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(a) : "r"(addr));
+    return a;
+}
+
+// One staged record of the packed kernels: 80 bytes, every operand of the per-pixel arithmetic twice.
+struct __align__(16) Rec2 {
+    float4 a;   // u, u, v, v
+    float4 b;   // A', A', B', B'
+    float4 c;   // C', C', log2(opacity) x 2
+    float4 d;   // r, r, g, g
+    float4 e;   // b, b, bit pattern of the entry id, opacity
+};
+
+__device__ __forceinline__ void stage_record2(const RasterArgs& a, int g, Rec2& r) {
+    const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + g);
+    const float A = -0.5f * kLog2e * __ldg(a.conics + 3 * (int64_t)g), B = -kLog2e * __ldg(a.conics + 3 * (int64_t)g + 1),
+                Cc = -0.5f * kLog2e * __ldg(a.conics + 3 * (int64_t)g + 2);
+    const float op = __ldg(a.opacities + g);
+    const float lo = __log2f(op);
+    const float cr = __ldg(a.rgbs + 3 * (int64_t)g), cg = __ldg(a.rgbs + 3 * (int64_t)g + 1), cb = __ldg(a.rgbs + 3 * (int64_t)g + 2);
+    r.a = make_float4(uv.x, uv.x, uv.y, uv.y);
+    r.b = make_float4(A, A, B, B);
+    r.c = make_float4(Cc, Cc, lo, lo);
+    r.d = make_float4(cr, cr, cg, cg);
+    r.e = make_float4(cb, cb, __int_as_float(g), op);
+}
+
+// rect_may_contribute for a (wx+1) x (wy+1) block of pixel centres starting at (X0, Y0)
+__device__ __forceinline__ bool rect_may_contribute2(float u, float v, float A, float B, float C, float lo, float X0, float Y0, float wx, float wy,
+                                                     float thr) {
+    const float dx0 = u - (X0 + wx), dx1 = u - X0;
+    const float dy0 = v - (Y0 + wy), dy1 = v - Y0;
+    const bool inx = (dx0 <= 0.0f) && (dx1 >= 0.0f), iny = (dy0 <= 0.0f) && (dy1 >= 0.0f);
+    const bool concave = (A <= 0.0f) && (C <= 0.0f) && (4.0f * A * C - B * B >= 0.0f);
+    float emax = 0.0f;
+    if (!(inx && iny)) {
+        emax = -3.0e38f;
+        if (!inx) {
+            const float dxe = dx0 > 0.0f ? dx0 : dx1;
+            const float dys = fminf(fmaxf(-0.5f * B * dxe * rcp_approx(C), dy0), dy1);
+            emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxe, dys), fmaxf(quad_form(A, B, C, dxe, dy0), quad_form(A, B, C, dxe, dy1))));
+        }
+        if (!iny) {
+            const float dye = dy0 > 0.0f ? dy0 : dy1;
+            const float dxs = fminf(fmaxf(-0.5f * B * dye * rcp_approx(A), dx0), dx1);
+            emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxs, dye), fmaxf(quad_form(A, B, C, dx0, dye), quad_form(A, B, C, dx1, dye))));
+        }
+    }
+    return !concave || !(emax + lo < thr);
+}
+
+constexpr int kBlock2 = 128;   // packed kernels: 4 warps per tile, each an 8x8 pixel block, lane = 2 x 1 pixels
+
+__global__ void __launch_bounds__(kBlock2) raster_fwd2_kernel(const RasterArgs a, const RasterFwdOut o) {
+    __shared__ Rec2 s_rec[kBlock2];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t bt = blockIdx.x;                  // view * tiles + tile
+    const int64_t view = bt / a.tiles;
+    const int t = (int)(bt - view * a.tiles);
+    const int ty = t / a.gx, tx = t - ty * a.gx;
+    const int bx0 = tx * kTile + (warp & 1) * 8, by0 = ty * kTile + (warp >> 1) * 8;   // the warp's 8x8 pixel block
+    const int j = bx0 + 2 * (lane & 3), i = by0 + (lane >> 2);                          // pixels (i, j) and (i, j + 1)
+    const bool in0 = (i < a.height) && (j < a.width), in1 = (i < a.height) && (j + 1 < a.width);
+    const f32x2 npx = pk2(-((float)j + 0.5f), -((float)j + 1.5f));
+    const float npy_s = -((float)i + 0.5f);
+    const f32x2 npy = pk2(npy_s, npy_s);
+    const f32x2 one2 = pk2(1.0f, 1.0f), neg2 = pk2(-1.0f, -1.0f);
+    const float X0 = (float)bx0 + 0.5f, Y0 = (float)by0 + 0.5f;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_rec);
+    const float alpha_min = a.alpha_min, alpha_max = a.alpha_max, t_min = a.t_min;
+
+    const int64_t start = __ldg(a.ranges + 2 * bt), end = __ldg(a.ranges + 2 * bt + 1);
+    float T0 = 1.0f, T1 = 1.0f;
+    f32x2 c0 = pk2(0.f, 0.f), c1 = c0, c2 = c0;
+    int last0 = 0, last1 = 0;
+    bool done0 = !in0, done1 = !in1;
+    for (int64_t base = start; base < end; base += kBlock2) {
+        if (__syncthreads_and(done0 && done1)) break;
+        const int64_t k = base + tid;
+        if (k < end) stage_record2(a, __ldg(a.vals + k), s_rec[tid]);
+        __syncthreads();
+        const int cnt = (int)((end - base) < kBlock2 ? (end - base) : kBlock2);
+        const int nbase = (int)(base - start) + 1;
+        bool warp_done = __all_sync(0xffffffffu, done0 && done1);
+        for (int ch = 0; ch * 32 < cnt && !warp_done; ++ch) {
+            const int r = ch * 32 + lane;
+            bool may = false;
+            if (r < cnt) {
+                const Rec2& rc = s_rec[r];
+                may = rect_may_contribute2(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr);
+            }
+            unsigned int mask = __ballot_sync(0xffffffffu, may);
+            while (mask) {
+                const int q = ch * 32 + __ffs(mask) - 1;
+                mask &= mask - 1;
+                const uint32_t addr = sbase + (uint32_t)q * (uint32_t)sizeof(Rec2);
+                f32x2 uu, vv, AA, BB, CC, LL, rr, gg;
+                lds2x64(addr, uu, vv);
+                lds2x64(addr + 16, AA, BB);
+                lds2x64(addr + 32, CC, LL);
+                lds2x64(addr + 48, rr, gg);
+                const f32x2 bb = lds64(addr + 64);
+                const f32x2 dx = add2(uu, npx), dy = add2(vv, npy);
+                // same operation order as quad_form: t = fma(B, dy, A dx); e = fma(C dy, dy, t dx)
+                const f32x2 tq = fma2(BB, dy, mul2(AA, dx));
+                const f32x2 e2 = fma2(mul2(CC, dy), dy, mul2(tq, dx));
+                const f32x2 el = add2(e2, LL);
+                float e_0, e_1, el0, el1;
+                unpk2(e2, e_0, e_1);
+                unpk2(el, el0, el1);
+                const float al0 = fminf(alpha_max, ex2_approx(el0)), al1 = fminf(alpha_max, ex2_approx(el1));
+                const f32x2 al = pk2(al0, al1), Tp = pk2(T0, T1);
+                const f32x2 Tn = mul2(Tp, fma2(al, neg2, one2));      // T (1 - alpha)
+                const f32x2 wg = mul2(al, Tp);
+                float Tn0, Tn1, wg0, wg1;
+                unpk2(Tn, Tn0, Tn1);
+                unpk2(wg, wg0, wg1);
+                const bool ok0 = !done0 && !(e_0 > 0.0f) && !(al0 < alpha_min), ok1 = !done1 && !(e_1 > 0.0f) && !(al1 < alpha_min);
+                const bool term0 = ok0 && (Tn0 < t_min), term1 = ok1 && (Tn1 < t_min);
+                const bool upd0 = ok0 && !term0, upd1 = ok1 && !term1;
+                const f32x2 w2 = pk2(upd0 ? wg0 : 0.0f, upd1 ? wg1 : 0.0f);
+                c0 = fma2(rr, w2, c0);
+                c1 = fma2(gg, w2, c1);
+                c2 = fma2(bb, w2, c2);
+                T0 = upd0 ? Tn0 : T0; T1 = upd1 ? Tn1 : T1;
+                last0 = upd0 ? nbase + q : last0; last1 = upd1 ? nbase + q : last1;
+                done0 = done0 || term0; done1 = done1 || term1;
+                if (__all_sync(0xffffffffu, done0 && done1)) { warp_done = true; break; }
+            }
+        }
+    }
+    float r0, r1, g0, g1, b0, b1;
+    unpk2(c0, r0, r1); unpk2(c1, g0, g1); unpk2(c2, b0, b1);
+    const int64_t pix = (view * a.height + i) * a.width + j;
+    if (in0) {
+        o.image[3 * pix] = r0 + T0 * a.bg0; o.image[3 * pix + 1] = g0 + T0 * a.bg1; o.image[3 * pix + 2] = b0 + T0 * a.bg2;
+        o.final_T[pix] = T0;
+        o.n_contrib[pix] = last0;
+    }
+    if (in1) {
+        o.image[3 * pix + 3] = r1 + T1 * a.bg0; o.image[3 * pix + 4] = g1 + T1 * a.bg1; o.image[3 * pix + 5] = b1 + T1 * a.bg2;
+        o.final_T[pix + 1] = T1;
+        o.n_contrib[pix + 1] = last1;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 struct RasterBwdIO {
     const float* final_T; const int32_t* n_contrib; const float* dL_dimage;
@@ -422,16 +601,314 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
     }
 }
 
-// zero the gradient rows of visible entries only (dense zero-fill when radii == nullptr is a memset)
-__global__ void __launch_bounds__(256) zero_visible_rows_kernel(int64_t n, const int32_t* __restrict__ radii, float* g_means2d,
-                                                                float* g_conics, float* g_opacities, float* g_rgbs) {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n) return;
-    if (__ldg(radii + e) <= 0) return;
+// ---- packed backward -----------------------------------------------------------------------------
+// Same scheme as raster_bwd_kernel with two pixels per lane: 4 warps per tile, each an 8x8 pixel
+// block (lane = row l >> 2, columns 2 (l & 3) and 2 (l & 3) + 1).  Transposition tile: one row per
+// record, 64 pixels in row-major order of the 8x8 block, 4 floats of padding after pixel 31 and a
+// row stride of 72 floats, so that both the 64-bit stores of the evaluation phase and the 128-bit
+// loads of the reduction phase (lane (record g, row pair t) reads pixels 16 t .. 16 t + 15) are free
+// of bank conflicts.
+#ifndef GS_BWD2_BATCH
+#define GS_BWD2_BATCH 64
+#endif
+constexpr int kBwd2Batch = GS_BWD2_BATCH;
+constexpr int kBwd2Chunks = kBwd2Batch / 32;
+constexpr int kWarps2 = kBlock2 / 32;
+constexpr int kT2Stride = 72;
+
+struct Bwd2Smem {
+    Rec2 rec[kBwd2Batch];
+    float slot[kWarps2][kBwd2Batch][kSlot];     // m0, m1x, m1y, m2xx, m2xy, m2yy, dr, dg, (db at [8])
+    float tbuf[kWarps2][2 * kGroup][kT2Stride]; // rows 0..7: gp of record k over the warp's 64 pixels; rows 8..15: wgt
+    float gpix[kWarps2][3][kT2Stride];          // dL/dimage of the warp's pixels, one row per channel, same pixel layout
+    unsigned int vis[kWarps2][kBwd2Chunks];
+    int max_contrib;
+};
+
+__device__ __forceinline__ void sts64(uint32_t addr, f32x2 v) { asm volatile("st.shared.b64 [%0], %1;" :: "r"(addr), "l"(v)); }
+
+// moments of one row of 8 values about the centre of the 8 columns (x = -3.5 .. 3.5)
+__device__ __forceinline__ void row_moments(const float4 p0, const float4 p1, float& s0, float& s1, float& s2) {
+    const float a0 = p0.x + p1.w, a1 = p0.y + p1.z, a2 = p0.z + p1.y, a3 = p0.w + p1.x;
+    const float d0 = p1.w - p0.x, d1 = p1.z - p0.y, d2 = p1.y - p0.z, d3 = p1.x - p0.w;
+    s0 = (a0 + a1) + (a2 + a3);
+    s1 = fmaf(3.5f, d0, fmaf(2.5f, d1, fmaf(1.5f, d2, 0.5f * d3)));
+    s2 = fmaf(12.25f, a0, fmaf(6.25f, a1, fmaf(2.25f, a2, 0.25f * a3)));
+}
+__device__ __forceinline__ float dot8(const float4 w0, const float4 w1, const float4 g0, const float4 g1, float acc) {
+    acc = fmaf(w0.x, g0.x, acc); acc = fmaf(w0.y, g0.y, acc); acc = fmaf(w0.z, g0.z, acc); acc = fmaf(w0.w, g0.w, acc);
+    acc = fmaf(w1.x, g1.x, acc); acc = fmaf(w1.y, g1.y, acc); acc = fmaf(w1.z, g1.z, acc); acc = fmaf(w1.w, g1.w, acc);
+    return acc;
+}
+
+// Reduce the k (<= 8) records of a warp's group.  lane = 4 g + t: record g, pixel rows 2 t and 2 t + 1
+// of the warp's block; `pya` = offset of row 2 t from the tile centre, `ox` = offset of the centre of
+// the warp's 8 columns; `myq` = batch position of record g.
+__device__ __forceinline__ void reduce_group2(Bwd2Smem& sm, int warp, int lane, int k, int myq, float ox, float pya) {
+    __syncwarp();
+    const int g = lane >> 2, t = lane & 3;
+    const int poff = 16 * t + ((t >> 1) << 2);
+    const uint32_t tb = (uint32_t)__cvta_generic_to_shared(&sm.tbuf[warp][g][poff]);
+    const uint32_t wb = tb + kGroup * kT2Stride * 4;
+    const uint32_t gb = (uint32_t)__cvta_generic_to_shared(&sm.gpix[warp][0][poff]);
+    const float pyb = pya + 1.0f;
+    float s0a, s1a, s2a, s0b, s1b, s2b;
+    row_moments(lds128(tb), lds128(tb + 16), s0a, s1a, s2a);
+    row_moments(lds128(tb + 32), lds128(tb + 48), s0b, s1b, s2b);
+    float v[9];
+    const float s0 = s0a + s0b, s1 = s1a + s1b, s2 = s2a + s2b;
+    const float m1xa = fmaf(ox, s0a, s1a), m1xb = fmaf(ox, s0b, s1b);
+    const float m1x = m1xa + m1xb;
+    const float ya = pya * s0a, yb = pyb * s0b;
+    v[0] = s0;
+    v[1] = m1x;
+    v[2] = ya + yb;
+    v[3] = fmaf(ox, m1x + s1, s2);            // s2 + 2 ox s1 + ox^2 s0
+    v[4] = fmaf(pya, m1xa, pyb * m1xb);
+    v[5] = fmaf(pya, ya, pyb * yb);
+    const float4 w0 = lds128(wb), w1 = lds128(wb + 16), w2 = lds128(wb + 32), w3 = lds128(wb + 48);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const uint32_t ga = gb + c * kT2Stride * 4;
+        float acc = dot8(w0, w1, lds128(ga), lds128(ga + 16), 0.0f);
+        v[6 + c] = dot8(w2, w3, lds128(ga + 32), lds128(ga + 48), acc);
+    }
+    // combine the 4 lanes of a record: values 0..7 split, value 8 plain
+    const bool b1 = t & 2, b0 = t & 1;
+    float c0, c1, c2, c3;
+    {
+        const float s_0 = b1 ? v[0] : v[4], s_1 = b1 ? v[1] : v[5], s_2 = b1 ? v[2] : v[6], s_3 = b1 ? v[3] : v[7];
+        const float k_0 = b1 ? v[4] : v[0], k_1 = b1 ? v[5] : v[1], k_2 = b1 ? v[6] : v[2], k_3 = b1 ? v[7] : v[3];
+        c0 = k_0 + __shfl_xor_sync(0xffffffffu, s_0, 2);
+        c1 = k_1 + __shfl_xor_sync(0xffffffffu, s_1, 2);
+        c2 = k_2 + __shfl_xor_sync(0xffffffffu, s_2, 2);
+        c3 = k_3 + __shfl_xor_sync(0xffffffffu, s_3, 2);
+    }
+    float e0, e1;
+    {
+        const float s_0 = b0 ? c0 : c2, s_1 = b0 ? c1 : c3;
+        const float k_0 = b0 ? c2 : c0, k_1 = b0 ? c3 : c1;
+        e0 = k_0 + __shfl_xor_sync(0xffffffffu, s_0, 1);
+        e1 = k_1 + __shfl_xor_sync(0xffffffffu, s_1, 1);
+    }
+    float w = v[8];
+    w += __shfl_xor_sync(0xffffffffu, w, 2);
+    w += __shfl_xor_sync(0xffffffffu, w, 1);
+    if (g < k) {
+        float* slot = &sm.slot[warp][myq][0];
+        slot[2 * t] = e0;
+        slot[2 * t + 1] = e1;
+        if (t == 0) slot[8] = w;
+    }
+    __syncwarp();
+}
+
+__global__ void __launch_bounds__(kBlock2) raster_bwd2_kernel(const RasterArgs a, const RasterBwdIO io) {
+    extern __shared__ __align__(16) unsigned char bwd_smem_raw[];
+    Bwd2Smem& sm = *reinterpret_cast<Bwd2Smem*>(bwd_smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t bt = blockIdx.x;
+    const int64_t view = bt / a.tiles;
+    const int t = (int)(bt - view * a.tiles);
+    const int ty = t / a.gx, tx = t - ty * a.gx;
+    const int bx0 = tx * kTile + (warp & 1) * 8, by0 = ty * kTile + (warp >> 1) * 8;
+    const int j = bx0 + 2 * (lane & 3), i = by0 + (lane >> 2);
+    const bool in0 = (i < a.height) && (j < a.width), in1 = (i < a.height) && (j + 1 < a.width);
+    const f32x2 npx = pk2(-((float)j + 0.5f), -((float)j + 1.5f));
+    const float npy_s = -((float)i + 0.5f);
+    const f32x2 npy = pk2(npy_s, npy_s);
+    const f32x2 one2 = pk2(1.0f, 1.0f), neg2 = pk2(-1.0f, -1.0f);
+    const float X0 = (float)bx0 + 0.5f, Y0 = (float)by0 + 0.5f;
+    const float xc = (float)(tx * kTile + kTile / 2), yc = (float)(ty * kTile + kTile / 2);   // tile centre
+    const float ox = (warp & 1) ? 4.0f : -4.0f;                                            // centre of the warp's columns - xc
+    const float pya = (float)((warp >> 1) * 8 + 2 * (lane & 3)) + 0.5f - 8.0f;             // reduce-phase row 2 (lane & 3) - yc
+    const int64_t start = __ldg(a.ranges + 2 * bt);
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.rec);
+    const int ppos = 2 * lane + ((lane >> 4) << 2);                                        // this lane's pixel pair in a tile row
+    const uint32_t tbase = (uint32_t)__cvta_generic_to_shared(&sm.tbuf[warp][0][ppos]);
+    const float alpha_min = a.alpha_min, alpha_max = a.alpha_max;
+
+    float T0 = 0.f, T1 = 0.f;
+    float gr0 = 0.f, gg0 = 0.f, gb0 = 0.f, gr1 = 0.f, gg1 = 0.f, gb1 = 0.f;
+    int ncon0 = 0, ncon1 = 0;
+    const int64_t pix = (view * a.height + i) * a.width + j;
+    if (in0) {
+        T0 = __ldg(io.final_T + pix);
+        ncon0 = __ldg(io.n_contrib + pix);
+        gr0 = __ldg(io.dL_dimage + 3 * pix); gg0 = __ldg(io.dL_dimage + 3 * pix + 1); gb0 = __ldg(io.dL_dimage + 3 * pix + 2);
+    }
+    if (in1) {
+        T1 = __ldg(io.final_T + pix + 1);
+        ncon1 = __ldg(io.n_contrib + pix + 1);
+        gr1 = __ldg(io.dL_dimage + 3 * pix + 3); gg1 = __ldg(io.dL_dimage + 3 * pix + 4); gb1 = __ldg(io.dL_dimage + 3 * pix + 5);
+    }
+    {
+        float* gp = &sm.gpix[warp][0][ppos];
+        gp[0] = gr0; gp[1] = gr1;
+        gp[kT2Stride] = gg0; gp[kT2Stride + 1] = gg1;
+        gp[2 * kT2Stride] = gb0; gp[2 * kT2Stride + 1] = gb1;
+    }
+    const f32x2 G0 = pk2(gr0, gr1), G1 = pk2(gg0, gg1), G2 = pk2(gb0, gb1);
+    if (tid == 0) sm.max_contrib = 0;
+    __syncthreads();
+    int wmax = max(ncon0, ncon1);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, d));
+    if (lane == 0 && wmax > 0) atomicMax(&sm.max_contrib, wmax);
+    __syncthreads();
+    const int maxn = sm.max_contrib;
+    if (maxn == 0) return;
+    // colour accumulated behind the current record
+    f32x2 S0 = pk2(a.bg0, a.bg0), S1 = pk2(a.bg1, a.bg1), S2 = pk2(a.bg2, a.bg2);
+    const int nb = (maxn + kBwd2Batch - 1) / kBwd2Batch;
+    for (int b = nb - 1; b >= 0; --b) {
+        const int cnt = min(kBwd2Batch, maxn - b * kBwd2Batch);
+        __syncthreads();   // previous batch fully flushed
+        if (tid < cnt) stage_record2(a, __ldg(a.vals + start + (int64_t)b * kBwd2Batch + tid), sm.rec[tid]);
+        __syncthreads();
+        int k = 0;         // records in the warp's current group (warp-uniform)
+        int myq = 0;       // batch position of the group's record (lane >> 2)
+        uint32_t taddr = tbase;   // this lane's cell in row k of the transposition tile
+        for (int ch = kBwd2Chunks - 1; ch >= 0; --ch) {
+            const int r = ch * 32 + lane;
+            const int cbase = b * kBwd2Batch + ch * 32;         // list position of bit 0 of this chunk
+            bool may = false;
+            if (r < cnt && (cbase + lane) < wmax) {
+                const Rec2& rc = sm.rec[r];
+                may = rect_may_contribute2(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr);
+            }
+            unsigned int mask = __ballot_sync(0xffffffffu, may);
+            const int nrel0 = ncon0 - cbase, nrel1 = ncon1 - cbase;   // pixel j walks bits < nrel_j
+            unsigned int written = 0;
+            const uint32_t cbase_addr = sbase + (uint32_t)(ch * 32) * (uint32_t)sizeof(Rec2);
+            while (mask) {
+                const int bit = msb(mask);
+                mask ^= 1u << bit;
+                const uint32_t addr = cbase_addr + (uint32_t)bit * (uint32_t)sizeof(Rec2);
+                f32x2 uu, vv, AA, BB, CC, LL;
+                lds2x64(addr, uu, vv);
+                lds2x64(addr + 16, AA, BB);
+                lds2x64(addr + 32, CC, LL);
+                const f32x2 dx = add2(uu, npx), dy = add2(vv, npy);
+                const f32x2 tq = fma2(BB, dy, mul2(AA, dx));
+                const f32x2 e2 = fma2(mul2(CC, dy), dy, mul2(tq, dx));
+                const f32x2 el = add2(e2, LL);
+                float e_0, e_1, el0, el1;
+                unpk2(e2, e_0, e_1);
+                unpk2(el, el0, el1);
+                const float raw0 = ex2_approx(el0), raw1 = ex2_approx(el1);
+                const float al0 = fminf(alpha_max, raw0), al1 = fminf(alpha_max, raw1);
+                const bool valid0 = (bit < nrel0) && !(e_0 > 0.0f) && !(al0 < alpha_min);
+                const bool valid1 = (bit < nrel1) && !(e_1 > 0.0f) && !(al1 < alpha_min);
+                if (!__any_sync(0xffffffffu, valid0 || valid1)) continue;
+                f32x2 rr, gg;
+                lds2x64(addr + 48, rr, gg);
+                const f32x2 bb = lds64(addr + 64);
+                // quantities of an invalid pixel are computed but selected away
+                const f32x2 al = pk2(al0, al1);
+                float om0, om1;
+                unpk2(fma2(al, neg2, one2), om0, om1);
+                const f32x2 Tp = pk2(T0, T1);
+                const f32x2 Tf = mul2(Tp, pk2(rcp_approx(om0), rcp_approx(om1)));   // transmittance in front of this record
+                const f32x2 d0 = fma2(S0, neg2, rr), d1 = fma2(S1, neg2, gg), d2 = fma2(S2, neg2, bb);
+                const f32x2 dLda = mul2(Tf, fma2(d2, G2, fma2(d1, G1, mul2(d0, G0))));
+                const f32x2 am = pk2(valid0 ? al0 : 0.0f, valid1 ? al1 : 0.0f);
+                S0 = fma2(am, d0, S0);
+                S1 = fma2(am, d1, S1);
+                S2 = fma2(am, d2, S2);
+                float Tf0, Tf1;
+                unpk2(Tf, Tf0, Tf1);
+                T0 = valid0 ? Tf0 : T0; T1 = valid1 ? Tf1 : T1;
+                // no gradient through the alpha_max clamp
+                float gp0, gp1;
+                unpk2(mul2(am, dLda), gp0, gp1);
+                gp0 = (raw0 > alpha_max) ? 0.0f : gp0;
+                gp1 = (raw1 > alpha_max) ? 0.0f : gp1;
+                sts64(taddr, pk2(gp0, gp1));
+                sts64(taddr + kGroup * kT2Stride * 4, mul2(am, Tf));
+                taddr += kT2Stride * 4;
+                myq = (k == (lane >> 2)) ? ch * 32 + bit : myq;
+                written |= 1u << bit;
+                if (++k == kGroup) {
+                    reduce_group2(sm, warp, lane, kGroup, myq, ox, pya);
+                    k = 0;
+                    taddr = tbase;
+                }
+            }
+            if (lane == 0) sm.vis[warp][ch] = written;
+        }
+        if (k) reduce_group2(sm, warp, lane, k, myq, ox, pya);
+        __syncthreads();
+        if (tid < cnt) {
+            float m[9];
+#pragma unroll
+            for (int c = 0; c < 9; ++c) m[c] = 0.f;
+            bool any = false;
+#pragma unroll
+            for (int w = 0; w < kWarps2; ++w)
+                if ((sm.vis[w][tid >> 5] >> (tid & 31)) & 1u) {
+                    any = true;
+#pragma unroll
+                    for (int c = 0; c < 9; ++c) m[c] += sm.slot[w][tid][c];
+                }
+            if (any) {
+                const Rec2& rc = sm.rec[tid];
+                const int64_t g = __float_as_int(rc.e.z);
+                const float Aq = rc.b.x, Bq = rc.b.z, Cq = rc.c.x;
+                // moments about the tile centre -> sums of gp*{dx, dy, dx^2, dx dy, dy^2}, dx = u - x
+                const float ut = rc.a.x - xc, vt = rc.a.z - yc;
+                const float Dx = fmaf(ut, m[0], -m[1]), Dy = fmaf(vt, m[0], -m[2]);
+                const float Dxx = fmaf(ut, Dx - m[1], m[3]);
+                const float Dxy = fmaf(vt, Dx, fmaf(-ut, m[2], m[4]));
+                const float Dyy = fmaf(vt, Dy - m[2], m[5]);
+                const float gu = fmaf(2.0f * Aq, Dx, Bq * Dy) * kLn2;
+                const float gv = fmaf(2.0f * Cq, Dy, Bq * Dx) * kLn2;
+                if (gu != 0.f) atomicAdd(io.g_means2d + 2 * g, gu);
+                if (gv != 0.f) atomicAdd(io.g_means2d + 2 * g + 1, gv);
+                if (Dxx != 0.f) atomicAdd(io.g_conics + 3 * g, -0.5f * Dxx);
+                if (Dxy != 0.f) atomicAdd(io.g_conics + 3 * g + 1, -Dxy);
+                if (Dyy != 0.f) atomicAdd(io.g_conics + 3 * g + 2, -0.5f * Dyy);
+                if (m[0] != 0.f) atomicAdd(io.g_opacities + g, m[0] / rc.e.w);
+                if (m[6] != 0.f) atomicAdd(io.g_rgbs + 3 * g, m[6]);
+                if (m[7] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 1, m[7]);
+                if (m[8] != 0.f) atomicAdd(io.g_rgbs + 3 * g + 2, m[8]);
+            }
+        }
+    }
+}
+
+// zero the gradient rows of visible entries only (dense zero-fill when radii == nullptr is a memset);
+// four entries per thread and load (one 16-byte load when `vec`), two loads in flight per thread
+__device__ __forceinline__ void zero_row(int64_t e, float* g_means2d, float* g_conics, float* g_opacities, float* g_rgbs) {
     reinterpret_cast<float2*>(g_means2d)[e] = make_float2(0.f, 0.f);
     g_conics[3 * e] = 0.f; g_conics[3 * e + 1] = 0.f; g_conics[3 * e + 2] = 0.f;
     g_opacities[e] = 0.f;
     g_rgbs[3 * e] = 0.f; g_rgbs[3 * e + 1] = 0.f; g_rgbs[3 * e + 2] = 0.f;
+}
+__global__ void __launch_bounds__(256) zero_visible_rows_kernel(int64_t n, const int32_t* __restrict__ radii, int vec, float* g_means2d,
+                                                                float* g_conics, float* g_opacities, float* g_rgbs) {
+    const int64_t q0 = ((int64_t)blockIdx.x * 512 + threadIdx.x) * 4;
+    int4 r[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int64_t e = q0 + h * 1024;
+        if (vec && e + 4 <= n) {
+            r[h] = __ldg(reinterpret_cast<const int4*>(radii + e));
+        } else {
+            r[h].x = (e < n) ? __ldg(radii + e) : 0;
+            r[h].y = (e + 1 < n) ? __ldg(radii + e + 1) : 0;
+            r[h].z = (e + 2 < n) ? __ldg(radii + e + 2) : 0;
+            r[h].w = (e + 3 < n) ? __ldg(radii + e + 3) : 0;
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int64_t e = q0 + h * 1024;
+        if (r[h].x > 0) zero_row(e, g_means2d, g_conics, g_opacities, g_rgbs);
+        if (r[h].y > 0) zero_row(e + 1, g_means2d, g_conics, g_opacities, g_rgbs);
+        if (r[h].z > 0) zero_row(e + 2, g_means2d, g_conics, g_opacities, g_rgbs);
+        if (r[h].w > 0) zero_row(e + 3, g_means2d, g_conics, g_opacities, g_rgbs);
+    }
 }
 
 __global__ void __launch_bounds__(256) l1_loss_kernel(int64_t n, const float* __restrict__ image, const float* __restrict__ target,
@@ -485,7 +962,11 @@ extern "C" int gs_raster_fwd(const gs_config* cfg, int32_t C, const gs_camera* c
     if (rc) return rc;
     if (!image || !final_T || !n_contrib) return GS_ERR_INVALID_ARGUMENT;
     RasterFwdOut o{image, final_T, n_contrib};
+#ifdef GS_FWD_SCALAR
     raster_fwd_kernel<<<(unsigned)(C * a.tiles), kBlock, 0, (cudaStream_t)stream>>>(a, o);
+#else
+    raster_fwd2_kernel<<<(unsigned)(C * a.tiles), kBlock2, 0, (cudaStream_t)stream>>>(a, o);
+#endif
     return launch_status();
 }
 
@@ -503,8 +984,8 @@ extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* c
     cudaStream_t st = (cudaStream_t)stream;
     if (N_total > 0) {
         if (radii) {
-            zero_visible_rows_kernel<<<(unsigned)((N_total + 255) / 256), 256, 0, st>>>(N_total, radii, dL_dmeans2d, dL_dconics,
-                                                                                         dL_dopacities, dL_drgbs);
+            zero_visible_rows_kernel<<<(unsigned)((N_total + 2047) / 2048), 256, 0, st>>>(N_total, radii, aligned(radii, 16) ? 1 : 0,
+                                                                                           dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs);
             rc = launch_status();
             if (rc) return rc;
         } else {
@@ -517,12 +998,21 @@ extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* c
     }
     RasterBwdIO io{final_T, n_contrib, dL_dimage, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs};
     static bool attr_set = false;
+#ifdef GS_BWD_SCALAR
     if (!attr_set) {
         if (cudaFuncSetAttribute(raster_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BwdSmem)) != cudaSuccess)
             return GS_ERR_CUDA;
         attr_set = true;
     }
     raster_bwd_kernel<<<(unsigned)(C * a.tiles), kBlock, sizeof(BwdSmem), st>>>(a, io);
+#else
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(raster_bwd2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Bwd2Smem)) != cudaSuccess)
+            return GS_ERR_CUDA;
+        attr_set = true;
+    }
+    raster_bwd2_kernel<<<(unsigned)(C * a.tiles), kBlock2, sizeof(Bwd2Smem), st>>>(a, io);
+#endif
     return launch_status();
 }
 

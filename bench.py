@@ -311,14 +311,21 @@ def run_b200(args):
     M_now = int(st.M_dev.item())
     pairs_bwd = int(st.n_contrib.to(torch.int64).sum().item())
     lens = (st.tile_ranges[:, 1] - st.tile_ranges[:, 0])
+    # binning plan (mirrors gs_bin_tiles): depth sort = 4 passes over bits 0..30 plus the view bits; tile sort =
+    # P_t passes of 8 or 9 bits over the tile id; the generating pass writes (key, value), the last pass values only
     tile_bits = max(1, int(np.ceil(np.log2(C * st.gx * st.gy))))
-    P = 4 + (tile_bits + 7) // 8
+    view_bits = int(np.ceil(np.log2(C))) if C > 1 else 0
+    P_d = 4 + (view_bits + 7) // 8
+    P_t = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
+    cells = C * (st.gx + 1) * (st.gy + 1)
+    tsort_bytes = 4 * M_now if P_t == 1 else (8 + 16 * (P_t - 2) + 12) * M_now
     K3 = 3 * st.K
     par_b = 4 * (3 + 3 + 4 + 1 + K3)
     work = {
         # bytes
         "project_fwd": 12 * N + (par_b - 12) * V_any + 48 * V_sum + 8 * N * C,
-        "bin_tiles": 4 * N * C + 12 * V_sum + 12 * M_now + (8 * M_now + 24 * M_now * P) + (8 * M_now + 16 * C * st.gx * st.gy),
+        # compaction (radii; uv, depth -> key, id) + depth sort (histogram, P_d passes) + entry table + tile sort + grid scans, ranges
+        "bin_tiles": 4 * N * C + 24 * V_sum + (8 + 24 * P_d) * V_sum + (32 + 16) * V_sum + tsort_bytes + 24 * cells + 16 * C * st.gx * st.gy,
         "project_bwd": 4 * N * C + 36 * V_sum + par_b * V_any + par_b * N,
         "l1_loss": 12 * C * W * H * 3,
         # flops (per evaluated (pixel, record) pair: DESIGN.md "algorithmic flops per pair")

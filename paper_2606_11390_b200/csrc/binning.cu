@@ -272,6 +272,48 @@ __device__ __forceinline__ unsigned long long block_chained_scan(unsigned long l
     return sm.base + wbase + inc - thread_sum;
 }
 
+// Block-wide variant of the look-back: all kScanThreads threads inspect one predecessor each per
+// round trip (nearest first), so a chain of several thousand in-flight blocks is walked in a handful
+// of L2 round trips instead of one per 32 blocks.  Every thread returns the exclusive prefix.
+struct WideLookSmem {
+    unsigned long long sum[kScanThreads / 32];
+    unsigned int has[kScanThreads / 32];
+};
+__device__ __forceinline__ unsigned long long block_lookback(unsigned long long* status, int64_t tile, unsigned long long block_total,
+                                                             WideLookSmem& sm) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tile == 0) {
+        if (tid == 0) st_volatile_u64(status, kFlagIncl | (block_total & kValMask));
+        return 0;
+    }
+    if (tid == 0) st_volatile_u64(status + tile, kFlagAgg | (block_total & kValMask));
+    unsigned long long excl = 0;
+    int64_t look = tile - 1;
+    while (true) {
+        const int64_t idx = look - tid;
+        unsigned long long st = kFlagIncl;   // virtual predecessor of block 0: inclusive 0
+        if (idx >= 0) {
+            do { st = ld_volatile_u64(status + idx); } while ((st >> 62) == 0);
+        }
+        const unsigned int incl = __ballot_sync(0xffffffffu, (st >> 62) == 2);
+        unsigned long long v = st & kValMask;
+        if (incl && lane > __ffs(incl) - 1) v = 0;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) v += shfl_u64(v, lane ^ d);
+        if (lane == 0) { sm.sum[warp] = v; sm.has[warp] = incl; }
+        __syncthreads();
+        bool found = false;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w)
+            if (!found) { excl += sm.sum[w]; found = sm.has[w] != 0u; }
+        if (found) break;
+        look -= kScanThreads;
+        __syncthreads();   // the round's partial sums have been read
+    }
+    if (tid == 0) st_volatile_u64(status + tile, kFlagIncl | ((excl + block_total) & kValMask));
+    return excl;
+}
+
 // ------------------------------------------------------------------------------ B1a: compaction
 struct CompactArgs {
     int64_t n_entries;      // C * N
@@ -299,7 +341,7 @@ __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs
     constexpr int WARPS = kScanThreads / 32;
     __shared__ unsigned int s_ticket;
     __shared__ unsigned int s_warp[WARPS];
-    __shared__ unsigned long long s_base;
+    __shared__ WideLookSmem s_look;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_ticket = atomicAdd(&a.hdr->compact_ticket, 1u);
     __syncthreads();
@@ -378,19 +420,13 @@ __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs
         if (w < warp) wbase += s_warp[w];
         btotal += s_warp[w];
     }
-    if (warp == 0) {
-        const unsigned long long excl = chained_scan_lookback(a.status, tile, btotal, lane);
-        if (lane == 0) {
-            s_base = excl;
-            if (tile == (int64_t)a.n_blocks - 1) {
-                const unsigned long long V = excl + btotal;
-                a.hdr->V = V < (unsigned long long)a.vcap ? V : (unsigned long long)a.vcap;
-            }
-        }
+    const unsigned long long excl = block_lookback(a.status, tile, btotal, s_look);
+    if (tid == 0 && tile == (int64_t)a.n_blocks - 1) {
+        const unsigned long long V = excl + btotal;
+        a.hdr->V = V < (unsigned long long)a.vcap ? V : (unsigned long long)a.vcap;
     }
-    if (btotal == 0) return;       // (block-uniform) nothing to write; warp 0 has published above
-    __syncthreads();
-    const unsigned long long gbase = s_base + wbase;
+    if (btotal == 0) return;       // (block-uniform) nothing to write
+    const unsigned long long gbase = excl + wbase;
     // exclusive rank of the lane's first visible entry of every iteration, 8-bit fields as above
     unsigned int lane_excl[WORDS];
 #pragma unroll

@@ -364,12 +364,9 @@ def run_b200(args):
         d2h = 4
 
         def e2e_step():
-            for k in st.param_names:
-                st.params[k].copy_(host_params[k], non_blocking=True)
-            st.target.copy_(host_tgt, non_blocking=True)
-            st.step(sync=False)
-            host_loss.copy_(st.loss, non_blocking=True)
-            stream.synchronize()
+            # the public end-to-end call: H2D of parameters and targets (the target copy overlaps P1..R1 on a
+            # second stream), the step, D2H of the loss, stream drained
+            st.step_from_host(host_params, host_tgt, host_loss)
 
         for _ in range(3):
             e2e_step()

@@ -138,6 +138,30 @@ class SplatStep:
         self.l1_loss()
         self.backward()
 
+    def step_from_host(self, host_params, host_target, host_loss):
+        """End-to-end step: parameters and target images come from (pinned) host tensors, the loss goes back
+        to ``host_loss``.  The parameters are copied on the compute stream; the target images, which only
+        the loss needs, are copied on a second stream while P1, binning and R1 run, and the loss kernel waits
+        for that copy.  Returns after the stream has drained (the loss value is then valid on the host)."""
+        main = torch.cuda.current_stream(self.device)
+        if getattr(self, "_copy_stream", None) is None:
+            self._copy_stream = torch.cuda.Stream(self.device)
+            self._target_ready = torch.cuda.Event()
+        if self.target is None:
+            self.target = torch.empty(tuple(host_target.shape), dtype=torch.float32, device=self.device)
+        self._copy_stream.wait_stream(main)          # the previous step's loss kernel has read the old target
+        with torch.cuda.stream(self._copy_stream):
+            self.target.copy_(host_target, non_blocking=True)
+            self._target_ready.record(self._copy_stream)
+        for k in self.param_names:
+            self.params[k].copy_(host_params[k], non_blocking=True)
+        self.forward(sync=False)
+        main.wait_event(self._target_ready)
+        self.l1_loss()
+        self.backward()
+        host_loss.copy_(self.loss, non_blocking=True)
+        main.synchronize()
+
     # launches of this library's kernels in one step (memsets excluded): P1; compact, tile y-scan, x-scan,
     # ranges, histogram scan, depth-sort histogram + passes, entry offsets, tile-sort passes (+ keys); R1, L1,
     # zero rows, R2, P5

@@ -234,6 +234,29 @@ def test_bin_tiles_tile_sort_pass_plans(B, oracle, W, H, C):
     np.testing.assert_array_equal(gr, ranges)
 
 
+@pytest.mark.parametrize("N,C,vis_frac", [(1_300_003, 2, 0.02), (2_000_001, 3, 0.01), (5_000_005, 2, 0.004)])
+def test_bin_tiles_compaction_tile_widths(B, oracle, N, C, vis_frac):
+    """Entry counts that select the 2 048-, 4 096- and 8 192-entry compaction tiles (the small scenes use
+    1 024), sparse visibility as in the street scenes, N not a multiple of 4 (ragged 16-byte loads), some
+    positive radii whose tile rectangle is empty (must not count), exact depth ties."""
+    W, H = 1920, 1080
+    cams = [scenes.make_camera(W, H, 1000.0, 1000.0, (0, 0, -3), (0, 0, 0), (0, -1, 0))] * C
+    sc = {"cameras": cams, "sh_degree": 0}
+    rng = np.random.default_rng(N)
+    m2d = np.stack([rng.uniform(-300, W + 300, (C, N)), rng.uniform(-300, H + 300, (C, N))], axis=-1).astype(np.float32)
+    dep = rng.uniform(0.3, 50.0, (C, N)).astype(np.float32)
+    dep[:, ::5] = np.float32(7.25)
+    rad = np.where(rng.random((C, N)) < vis_frac, rng.integers(1, 60, (C, N)), 0).astype(np.int32)
+    rad[:, -3:] = 9                                                            # the ragged tail is visible
+    cfg = oracle.make_cfg(sh_degree=0)
+    keys, vals, ranges = oracle.bin_tiles(cfg, cams, m2d, dep, rad)
+    M, M_dev, gk, gv, gr = run_bin(B, sc, {"means2d": m2d, "depths": dep}, rad, capacity=len(keys) + 5)
+    assert M == len(keys) == M_dev
+    np.testing.assert_array_equal(gk[:M], keys)
+    np.testing.assert_array_equal(gv[:M], vals)
+    np.testing.assert_array_equal(gr, ranges)
+
+
 @pytest.mark.parametrize("n,end_bit,skip", [(1, 64, 0), (255, 40, 1), (4096, 64, 0), (4097, 47, 1), (100_003, 64, 0),
                                             (1_000_000, 49, 1), (3_000_001, 33, 1)])
 def test_sort_pairs_matches_stable_library_sort(B, n, end_bit, skip):
@@ -421,3 +444,28 @@ def test_end_to_end_step_against_oracle(B, oracle, name, sc):
     print(f"[{name}] M {st.M} image err>1e-4 frac {frac_bad:.2e}; grad rel L2 {errs}")
     for k, e in errs.items():
         assert e <= 1e-3, (k, e)
+
+
+def test_step_from_host_equals_resident_step(B):
+    """The end-to-end call (pinned host inputs, target copied on a second stream, loss read back) computes
+    the same integers and, up to the order of the float atomics, the same gradients as the resident step."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    name, sc = SCENES[0]
+    tgt = scenes.target_image(sc)
+    ref = SplatStep(sc)
+    ref.set_target(tgt)
+    ref.step(sync=True)
+    torch.cuda.synchronize()
+    st = SplatStep(sc, upload=False, capacity_M=ref.capacity_M)
+    host_params = {k: torch.from_numpy(np.ascontiguousarray(sc[k], dtype=np.float32)).pin_memory() for k in st.param_names}
+    host_tgt = torch.from_numpy(tgt).pin_memory()
+    host_loss = torch.zeros((1,), dtype=torch.float32).pin_memory()
+    for _ in range(2):                       # twice: the second call reuses the copy stream and the target buffer
+        st.step_from_host(host_params, host_tgt, host_loss)
+    assert int(st.M_dev.item()) == ref.M
+    assert torch.equal(st.isect_vals[: ref.M], ref.isect_vals[: ref.M])
+    assert torch.equal(st.n_contrib, ref.n_contrib)
+    assert torch.equal(st.image, ref.image)
+    assert abs(float(host_loss.item()) - float(ref.loss.item())) <= 1e-6
+    for k in st.param_names:
+        assert rel_l2(st.grads[k].cpu().numpy(), ref.grads[k].cpu().numpy()) <= 1e-5, k

@@ -847,8 +847,8 @@ template <int BITS>
 struct TileSweepSmem {
     static constexpr int BINS = 1 << BITS;
     unsigned short warp_hist[kTsWarps][BINS];   // <= 32 * kTsItems items per warp
-    unsigned int keys[kTsTile];
-    int vals[kTsTile];
+    unsigned int keys[kTsTile + kTsTile / 32];   // + padding of the generating pass (one word per 32: the blocked
+    int vals[kTsTile + kTsTile / 32];            //   writes, 16 words apart between lanes, stay conflict-free)
     int goff[BINS];                  // global base of the digit minus its start inside the tile
     unsigned int bin_start[BINS];
     unsigned short head[kTsTile];    // generating pass: 1 + (entry - first entry) at the entry's first record
@@ -857,7 +857,10 @@ struct TileSweepSmem {
 };
 
 template <int BITS, bool GEN>
-__global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSweepArgs a) {
+#ifndef GS_TS_MINB
+#define GS_TS_MINB 2
+#endif
+__global__ void __launch_bounds__(kTsThreads, GS_TS_MINB) tile_sweep_kernel(const TileSweepArgs a) {
     using Smem = TileSweepSmem<BITS>;
     constexpr int BINS = Smem::BINS;
     static_assert(kTsItems % 8 == 0, "blocked generation reads 8 heads per vector");
@@ -942,8 +945,8 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
                     int rx = (int)(kk - ry * en.w);
                     if (rx < 0) { --ry; rx += (int)en.w; }
                     else if (rx >= (int)en.w) { ++ry; rx -= (int)en.w; }
-                    sm.keys[p] = en.t0 + ry * (unsigned int)a.gx + (unsigned int)rx;
-                    sm.vals[p] = en.id;
+                    sm.keys[p + (p >> 5)] = en.t0 + ry * (unsigned int)a.gx + (unsigned int)rx;
+                    sm.vals[p + (p >> 5)] = en.id;
                 }
             }
             __syncthreads();
@@ -951,8 +954,8 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
 #pragma unroll
             for (int j = 0; j < kTsItems; ++j) {
                 const int idx = warp * (32 * kTsItems) + j * 32 + lane;
-                key[j] = idx < valid ? sm.keys[idx] : 0xffffffffu;
-                val[j] = idx < valid ? sm.vals[idx] : 0;
+                key[j] = idx < valid ? sm.keys[idx + (idx >> 5)] : 0xffffffffu;
+                val[j] = idx < valid ? sm.vals[idx + (idx >> 5)] : 0;
             }
         } else {
 #pragma unroll

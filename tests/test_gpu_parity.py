@@ -234,10 +234,10 @@ def test_bin_tiles_tile_sort_pass_plans(B, oracle, W, H, C):
     np.testing.assert_array_equal(gr, ranges)
 
 
-@pytest.mark.parametrize("N,C,vis_frac", [(1_300_003, 2, 0.02), (2_000_001, 3, 0.01), (5_000_005, 2, 0.004)])
+@pytest.mark.parametrize("N,C,vis_frac", [(1_300_003, 2, 0.02), (2_000_001, 3, 0.01), (5_000_005, 2, 0.004), (8_500_001, 2, 0.003)])
 def test_bin_tiles_compaction_tile_widths(B, oracle, N, C, vis_frac):
     """Entry counts that select the 2 048-, 4 096- and 8 192-entry compaction tiles (the small scenes use
-    1 024), sparse visibility as in the street scenes, N not a multiple of 4 (ragged 16-byte loads), some
+    1 024) and, from 2^24 entries, the two-kernel path (visibility bit mask + scan over the mask); sparse visibility as in the street scenes, N not a multiple of 4 (ragged 16-byte loads), some
     positive radii whose tile rectangle is empty (must not count), exact depth ties."""
     W, H = 1920, 1080
     cams = [scenes.make_camera(W, H, 1000.0, 1000.0, (0, 0, -3), (0, 0, 0), (0, -1, 0))] * C

@@ -170,4 +170,5 @@ class SplatStep:
         view_bits = int(np.ceil(np.log2(self.C))) if self.C > 1 else 0
         depth_passes = 4 + (view_bits + 7) // 8
         tile_passes = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
-        return 1 + 5 + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1
+        compact = 2 if self.C * self.N >= (1 << 24) else 1          # visibility mask + scan over the mask for large inputs
+        return 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

@@ -224,6 +224,23 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ----------------------------------------------------------------------------- replicas (multi-GPU) arithmetic
+def max_over_ranks(ms, world, device=None):
+    """Device time of the job = the slowest rank's (all-reduce MAX over the default process group)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world, units_per_rank_per_step, ms_per_step):
+    """Replicas only: every rank processes the same units; whole-job rate = all ranks' units / max time."""
+    return world * units_per_rank_per_step / (ms_per_step * 1e-3)
+
+
 # ----------------------------------------------------------------------------- B200 leg
 STAGES = ("project_fwd", "bin_tiles", "raster_fwd", "l1_loss", "raster_bwd", "project_bwd")
 
@@ -294,15 +311,11 @@ def run_b200(args):
     clocks = sampler.stop()
     step_ms = np.array([ev[0].elapsed_time(ev[-1]) for ev in events])
     stage_ms = {s: float(np.mean([ev[i].elapsed_time(ev[i + 1]) for ev in events])) for i, s in enumerate(STAGES)}
-    total_ms = float(step_ms.sum())
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(float(step_ms.sum()), world, dev)
     ms_per_step = total_ms / args.steps
     mpix_step = C * W * H / 1e6
-    value = world * mpix_step / (ms_per_step * 1e-3)
-    gauss_per_s = world * C * N / (ms_per_step * 1e-3)
+    value = whole_job_rate(world, mpix_step, ms_per_step)
+    gauss_per_s = whole_job_rate(world, C * N, ms_per_step)
 
     # ---- algorithmic work of this step (harness-side counting, outside the timed region)
     vis = st.radii > 0
@@ -378,12 +391,8 @@ def run_b200(args):
             e2e_step()
         e1.record(stream)
         barrier()
-        e_ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([e_ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_ms = float(t.item())
-        e2e = {"value": world * mpix_step / (e_ms / n_e2e * 1e-3), "unit": "MP/s", "h2d_bytes_per_step": int(h2d),
+        e_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
+        e2e = {"value": whole_job_rate(world, mpix_step, e_ms / n_e2e), "unit": "MP/s", "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms / n_e2e, "steps": n_e2e, "loss": float(host_loss.item())}
 
     if rank != 0:

@@ -3,7 +3,7 @@
 
 * object (configs[1]: 100 k Gaussians, 8 x 1080p, SH degree 3): the whole chained step against the
   oracle chained the same way -- every pixel and every gradient row (the oracle needs ~1 min).
-* room / block (1 M Gaussians x 4 x 4K; 10 M Gaussians x 4K): sampled outputs.  P1 on every entry;
+* room / block / city (1 M Gaussians x 4 x 4K; 10 M Gaussians x 4K; 6 M of the city's 60 M Gaussians x 4 x 4K): sampled outputs.  P1 on every entry;
   binning by properties that hold at any size (ranges partition [0, M), every list sorted by depth) plus
   the exact list of sampled tiles rebuilt one by one from the definition (rectangle overlap, stable order
   by (depth bits, entry)); R1 / R2 on sampled tiles with the oracle's tile mask (stage isolation: the oracle
@@ -174,9 +174,11 @@ def tile_list_from_definition(t, view, N, gx, gy, means2d, depths, radii):
     return (view * N + idx[order]).astype(np.int32)
 
 
-@pytest.mark.parametrize("workload,stride", [("room", 211), ("block", 97)])
-def test_full_size_sampled(B, oracle, workload, stride):
-    sc = scenes.make_scene(workload)
+@pytest.mark.parametrize("workload,stride,n", [("room", 211, None), ("block", 97, None), ("city", 503, 6_000_000)])
+def test_full_size_sampled(B, oracle, workload, stride, n):
+    # city: the scene's four 4K street views over 6 M of its 60 M Gaussians (same distribution): 24 M entries, which is
+    # past the 2^24-entry switch to the two-kernel compaction and keeps the oracle's P1 within a minute
+    sc = scenes.make_scene(workload, n=n)
     cfg = oracle.make_cfg(sh_degree=sc["sh_degree"])
     cams = sc["cameras"]
     C, N = len(cams), sc["means"].shape[0]

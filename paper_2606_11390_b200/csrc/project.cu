@@ -33,6 +33,8 @@ struct ProjFwdArgs {
 
 constexpr int kProjThreads = 128;   // P1 block
 constexpr int kBwdThreads = 128;    // P5 block (168 registers per thread)
+constexpr int64_t kZeroFillMinN = 1 << 22;   // from here the dense zero-fill of P5 runs as its own streaming kernels (measured:
+                                             // slower at 1 M Gaussians, 0.555 -> 0.44 ms at 10 M, 2.98 -> 2.34 ms at 60 M)
 #ifndef GS_PROJ_ITEMS
 #define GS_PROJ_ITEMS 8
 #endif
@@ -288,6 +290,7 @@ struct ProjBwdArgs {
     float dilation;
     int32_t accumulate;
     int32_t vec_in, vec_out;   // 16-byte vector access allowed on the radii rows / on the five gradient arrays
+    int32_t prezeroed;         // the gradient arrays were zero-filled by zero_fill_kernel: phase A only reads the radii
 };
 
 template <int DEG>
@@ -517,17 +520,20 @@ __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjB
             for (int k = 0; k < ITEMS; ++k) vis[k] = 0;
             for (int c = 0; c < a.C; ++c) {
                 const int64_t e0 = (int64_t)c * a.N + i0;
-                if (ITEMS == 4 && a.vec_in && full) {
-                    const int4 r = __ldg(reinterpret_cast<const int4*>(a.radii + e0));
-                    vis[0] |= (r.x > 0 ? 1u : 0u) << c; vis[1 % ITEMS] |= (r.y > 0 ? 1u : 0u) << c;
-                    vis[2 % ITEMS] |= (r.z > 0 ? 1u : 0u) << c; vis[3 % ITEMS] |= (r.w > 0 ? 1u : 0u) << c;
+                if (ITEMS % 4 == 0 && a.vec_in && full) {
+#pragma unroll
+                    for (int q = 0; q < ITEMS / 4; ++q) {
+                        const int4 r = __ldg(reinterpret_cast<const int4*>(a.radii + e0) + q);
+                        vis[(4 * q) % ITEMS] |= (r.x > 0 ? 1u : 0u) << c; vis[(4 * q + 1) % ITEMS] |= (r.y > 0 ? 1u : 0u) << c;
+                        vis[(4 * q + 2) % ITEMS] |= (r.z > 0 ? 1u : 0u) << c; vis[(4 * q + 3) % ITEMS] |= (r.w > 0 ? 1u : 0u) << c;
+                    }
                 } else {
 #pragma unroll
                     for (int k = 0; k < ITEMS; ++k)
                         if (i0 + k < a.N && __ldg(a.radii + e0 + k) > 0) vis[k] |= 1u << c;
                 }
             }
-            if (!a.accumulate) {
+            if (!a.accumulate && !a.prezeroed) {
                 const int64_t n = (a.N - base) < CHUNK ? (a.N - base) : CHUNK;
                 const bool vec = a.vec_out != 0;
                 zero_span(a.d_sh + base * K3, n * K3, vec, lane);
@@ -549,6 +555,21 @@ __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjB
         cnt -= n;
         __syncwarp();          // the popped entries have been read
     }
+}
+
+// Dense zero-fill of the five gradient arrays as one streaming kernel (16-byte stores, full occupancy).  For large N
+// this is where P5's bytes go (236 B per Gaussian at SH degree 3); measured on B200 a plain store stream reaches
+// 7.5 TB/s, the same stores issued from the 168-register persistent kernel's phase A 4.8 TB/s.
+// one array: every thread zeroes four 16-byte units a block-width apart (coalesced, four stores in flight)
+__global__ void __launch_bounds__(256) zero_fill_kernel(float* __restrict__ p, int64_t count) {
+    const int64_t n4 = count >> 2;
+    const int64_t i0 = (int64_t)blockIdx.x * 1024 + threadIdx.x;
+    float4* p4 = reinterpret_cast<float4*>(p);
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (i0 + k * 256 < n4) p4[i0 + k * 256] = zero;
+    if (blockIdx.x == 0 && threadIdx.x < 4 && (n4 << 2) + threadIdx.x < count) p[(n4 << 2) + threadIdx.x] = 0.f;
 }
 
 static int sm_count() {
@@ -586,6 +607,16 @@ template <int DEG>
 int launch_bwd(const ProjBwdArgs& a, const CamBatch& cb, cudaStream_t st) {
     const int sms = sm_count();
     constexpr int warps = kBwdThreads / 32;
+    if (a.prezeroed) {
+        // phase A only scans the radii: 16 Gaussians per lane keep 4 C 16-byte loads in flight per lane
+        // (only when every resident warp still gets >= 8 such chunks; else the narrower variants below)
+        const int64_t scan = (a.N + 32 * 16 - 1) / (32 * 16);
+        const unsigned scan_grid = persistent_grid(project_bwd_kernel<DEG, 16>, kBwdThreads, (scan + warps - 1) / warps, sms);
+        if (scan >= 8 * (int64_t)scan_grid * warps) {
+            project_bwd_kernel<DEG, 16><<<scan_grid, kBwdThreads, 0, st>>>(a, cb);
+            return launch_status();
+        }
+    }
     const int64_t wide = (a.N + 32 * 4 - 1) / (32 * 4);
     const unsigned wide_grid = persistent_grid(project_bwd_kernel<DEG, 4>, kBwdThreads, (wide + warps - 1) / warps, sms);
     if (wide >= 8 * (int64_t)wide_grid * warps) {
@@ -679,6 +710,19 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
         a.vec_in = (aligned(a.radii, 16) && (N % 4 == 0 || nc == 1)) ? 1 : 0;
         a.vec_out = (aligned(dL_dmeans, 16) && aligned(dL_dlog_scales, 16) && aligned(dL_dquats, 16) &&
                      aligned(dL_dopacity_logits, 16) && aligned(dL_dsh, 16)) ? 1 : 0;
+        a.prezeroed = 0;
+        if (!a.accumulate && a.vec_out && N >= kZeroFillMinN) {
+            const int64_t K3 = 3 * (int64_t)(cfg->sh_degree + 1) * (cfg->sh_degree + 1);
+            float* ptrs[5] = {dL_dsh, dL_dquats, dL_dmeans, dL_dlog_scales, dL_dopacity_logits};
+            const int64_t counts[5] = {K3 * N, 4 * N, 3 * N, 3 * N, N};
+            for (int k = 0; k < 5; ++k) {
+                const int64_t blocks = ((counts[k] >> 2) + 1023) / 1024;
+                zero_fill_kernel<<<(unsigned)(blocks > 0 ? blocks : 1), 256, 0, st>>>(ptrs[k], counts[k]);
+            }
+            rc = launch_status();
+            if (rc) return rc;
+            a.prezeroed = 1;
+        }
         switch (cfg->sh_degree) {
             case 0: rc = launch_bwd<0>(a, cb, st); break;
             case 1: rc = launch_bwd<1>(a, cb, st); break;

@@ -171,4 +171,5 @@ class SplatStep:
         depth_passes = 4 + (view_bits + 7) // 8
         tile_passes = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
         compact = 2 if self.C * self.N >= (1 << 24) else 1          # visibility mask + scan over the mask for large inputs
-        return 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1
+        p5 = 6 if self.N >= (1 << 22) else 1                         # dense zero-fill as five streaming launches for large N
+        return (p5 - 1) + 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

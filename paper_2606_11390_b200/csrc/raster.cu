@@ -18,6 +18,8 @@
 // record go to the warp's own shared-memory slot (shared-memory float atomics are CAS loops on
 // this hardware), are summed across the 4 warps at the end of the batch and flushed with one
 // device-scope red.add per value and (tile, record).
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace gs {
@@ -130,7 +132,7 @@ __device__ __forceinline__ void stage_record(const RasterArgs& a, int g, Rec& r)
 
 // rect_may_contribute for a (wx+1) x (wy+1) block of pixel centres starting at (X0, Y0)
 __device__ __forceinline__ bool rect_may_contribute(float u, float v, float A, float B, float C, float lo, float X0, float Y0, float wx, float wy,
-                                                     float thr) {
+                                                     float thr, bool* is_concave = nullptr) {
     const float dx0 = u - (X0 + wx), dx1 = u - X0;
     const float dy0 = v - (Y0 + wy), dy1 = v - Y0;
     const bool inx = (dx0 <= 0.0f) && (dx1 >= 0.0f), iny = (dy0 <= 0.0f) && (dy1 >= 0.0f);
@@ -149,6 +151,7 @@ __device__ __forceinline__ bool rect_may_contribute(float u, float v, float A, f
             emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxs, dye), fmaxf(quad_form(A, B, C, dx0, dye), quad_form(A, B, C, dx1, dye))));
         }
     }
+    if (is_concave) *is_concave = concave;
     return !concave || !(emax + lo < thr);
 }
 
@@ -173,29 +176,33 @@ __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, 
     const float alpha_min = a.alpha_min, alpha_max = a.alpha_max, t_min = a.t_min;
 
     const int64_t start = __ldg(a.ranges + 2 * bt), end = __ldg(a.ranges + 2 * bt + 1);
-    float T0 = 1.0f, T1 = 1.0f;
+    // A pixel that has terminated (or lies outside the image) carries its transmittance NEGATED: T (1 - alpha) is then
+    // negative, fails the T' >= t_min test and nothing updates any more -- the sticky "done" flag costs no predicate
+    // register and no select of its own (the ALU pipe, half as wide as the FMA pipe, is the busiest unit of this loop).
+    float T0 = in0 ? 1.0f : -1.0f, T1 = in1 ? 1.0f : -1.0f;
     f32x2 c0 = pk2(0.f, 0.f), c1 = c0, c2 = c0;
     int last0 = 0, last1 = 0;
-    bool done0 = !in0, done1 = !in1;
     for (int64_t base = start; base < end; base += kBlock) {
-        if (__syncthreads_and(done0 && done1)) break;
+        if (__syncthreads_and(T0 < 0.0f && T1 < 0.0f)) break;
         const int64_t k = base + tid;
         if (k < end) stage_record(a, __ldg(a.vals + k), s_rec[tid]);
         __syncthreads();
         const int cnt = (int)((end - base) < kBlock ? (end - base) : kBlock);
         const int nbase = (int)(base - start) + 1;
-        bool warp_done = __all_sync(0xffffffffu, done0 && done1);
+        bool warp_done = __all_sync(0xffffffffu, T0 < 0.0f && T1 < 0.0f);
         for (int ch = 0; ch * 32 < cnt && !warp_done; ++ch) {
             const int r = ch * 32 + lane;
-            bool may = false;
+            bool may = false, concave = true;
             if (r < cnt) {
                 const Rec& rc = s_rec[r];
-                may = rect_may_contribute(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr);
+                may = rect_may_contribute(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr, &concave);
             }
+            // the exponent of a concave (valid) conic cannot be positive: its "power > 0" test is dropped (a rounding
+            // residue of +1e-7 changes alpha by 1e-7); chunks that hold any other record take the checked body
+            const bool check_e = __any_sync(0xffffffffu, !concave);
             unsigned int mask = __ballot_sync(0xffffffffu, may);
-            while (mask) {
-                const int q = ch * 32 + __ffs(mask) - 1;
-                mask &= mask - 1;
+            auto composite = [&](auto checked, int q) {
+                constexpr bool CHECK = decltype(checked)::value;
                 const uint32_t addr = sbase + (uint32_t)q * (uint32_t)sizeof(Rec);
                 f32x2 uu, vv, AA, BB, CC, LL, rr, gg;
                 lds2x64(addr, uu, vv);
@@ -218,23 +225,38 @@ __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, 
                 float Tn0, Tn1, wg0, wg1;
                 unpk2(Tn, Tn0, Tn1);
                 unpk2(wg, wg0, wg1);
-                const bool ok0 = !done0 && !(e_0 > 0.0f) && !(al0 < alpha_min), ok1 = !done1 && !(e_1 > 0.0f) && !(al1 < alpha_min);
-                const bool term0 = ok0 && (Tn0 < t_min), term1 = ok1 && (Tn1 < t_min);
-                const bool upd0 = ok0 && !term0, upd1 = ok1 && !term1;
+                const bool ok0 = !(CHECK && e_0 > 0.0f) && !(al0 < alpha_min), ok1 = !(CHECK && e_1 > 0.0f) && !(al1 < alpha_min);
+                const bool term0 = ok0 && (Tn0 < t_min), term1 = ok1 && (Tn1 < t_min);      // also true again for a finished pixel
+                const bool upd0 = ok0 && !(Tn0 < t_min), upd1 = ok1 && !(Tn1 < t_min);
                 const f32x2 w2 = pk2(upd0 ? wg0 : 0.0f, upd1 ? wg1 : 0.0f);
                 c0 = fma2(rr, w2, c0);
                 c1 = fma2(gg, w2, c1);
                 c2 = fma2(bb, w2, c2);
-                T0 = upd0 ? Tn0 : T0; T1 = upd1 ? Tn1 : T1;
+                T0 = upd0 ? Tn0 : (term0 ? -fabsf(T0) : T0);
+                T1 = upd1 ? Tn1 : (term1 ? -fabsf(T1) : T1);
                 last0 = upd0 ? nbase + q : last0; last1 = upd1 ? nbase + q : last1;
-                done0 = done0 || term0; done1 = done1 || term1;
-                if (__all_sync(0xffffffffu, done0 && done1)) { warp_done = true; break; }
+            };
+            if (check_e) {
+                while (mask) {
+                    const int q = ch * 32 + __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    composite(std::true_type{}, q);
+                    if (__all_sync(0xffffffffu, T0 < 0.0f && T1 < 0.0f)) { warp_done = true; break; }
+                }
+            } else {
+                while (mask) {
+                    const int q = ch * 32 + __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    composite(std::false_type{}, q);
+                    if (__all_sync(0xffffffffu, T0 < 0.0f && T1 < 0.0f)) { warp_done = true; break; }
+                }
             }
         }
     }
     float r0, r1, g0, g1, b0, b1;
     unpk2(c0, r0, r1); unpk2(c1, g0, g1); unpk2(c2, b0, b1);
     const int64_t pix = (view * a.height + i) * a.width + j;
+    T0 = fabsf(T0); T1 = fabsf(T1);
     if (in0) {
         o.image[3 * pix] = r0 + T0 * a.bg0; o.image[3 * pix + 1] = g0 + T0 * a.bg1; o.image[3 * pix + 2] = b0 + T0 * a.bg2;
         o.final_T[pix] = T0;

@@ -149,6 +149,18 @@ int gs_project_bwd(const gs_config* cfg /*host*/, int64_t N, const float* means,
  * dL_dimage[n] = sign(image - target) / n; *loss_sum (device, float, caller-zeroed) += sum |image - target| / n. */
 int gs_l1_loss(int64_t n, const float* image, const float* target, float* dL_dimage, float* loss_sum, void* stream);
 
+/* Fused L1 + SSIM image loss, forward and backward ("computes the loss", refs [31],
+ * [20]):  L = (1 - lambda) mean|x - y| + lambda (1 - mean SSIM(x, y)), SSIM per channel with the 11 x 11 Gaussian window
+ * (sigma 1.5, sum 1), zero padding (window not renormalised at the border), biased window variances, C1 = 0.01^2,
+ * C2 = 0.03^2, means over all C * H * W * 3 values.
+ * in : image, target [C, H, W, 3] fp32 (device), 0 <= lambda <= 1.
+ * out: dL_dimage [C, H, W, 3] = dL/dimage (overwritten); *loss_sum (device, float, caller-zeroed) += L.
+ * workspace (device, caller-owned): 3 * C * H * W * 3 floats; with workspace == NULL the call only writes the needed
+ * size to *workspace_bytes.  Asynchronous on `stream`; no allocation, no host synchronisation.
+ * Errors: GS_ERR_INVALID_ARGUMENT (null pointers, sizes < 1, lambda outside [0, 1], workspace too small), GS_ERR_CUDA. */
+int gs_l1_ssim_loss(int32_t C, int32_t height, int32_t width, const float* image, const float* target, float lambda,
+                    float* dL_dimage, float* loss_sum, void* workspace, size_t* workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, os.environ.get("GS_LIB_NAME", "libgsplat_b200.so"
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
-           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss"]
+           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss"]
 
 
 class gs_camera(C.Structure):
@@ -219,3 +219,23 @@ def gs_l1_loss(image, target, dL_dimage, loss_sum, stream=None):
     rc = lib().gs_l1_loss(C.c_int64(image.numel()), _ptr(image, torch.float32), _ptr(target, torch.float32),
                           _ptr(dL_dimage, torch.float32), _ptr(loss_sum, torch.float32), _stream(stream))
     _check(rc, "gs_l1_loss")
+
+
+def gs_l1_ssim_loss_workspace_bytes(C_views, height, width):
+    nbytes = C.c_size_t(0)
+    rc = lib().gs_l1_ssim_loss(C.c_int32(C_views), C.c_int32(height), C.c_int32(width), None, None, C.c_float(0.2), None, None,
+                               None, C.byref(nbytes), None)
+    _check(rc, "gs_l1_ssim_loss")
+    return int(nbytes.value)
+
+
+def gs_l1_ssim_loss(image, target, lam, dL_dimage, loss_sum, workspace, stream=None):
+    """image, target, dL_dimage: [C, H, W, 3] float32 CUDA tensors; loss_sum: 1 float (caller-zeroed, added to)."""
+    import torch
+    Cv, H, W, ch = image.shape
+    assert ch == 3 and tuple(target.shape) == tuple(image.shape) == tuple(dL_dimage.shape)
+    nbytes = C.c_size_t(workspace.numel() * workspace.element_size())
+    rc = lib().gs_l1_ssim_loss(C.c_int32(Cv), C.c_int32(H), C.c_int32(W), _ptr(image, torch.float32), _ptr(target, torch.float32),
+                               C.c_float(lam), _ptr(dL_dimage, torch.float32), _ptr(loss_sum, torch.float32),
+                               _ptr(workspace, torch.uint8), C.byref(nbytes), _stream(stream))
+    _check(rc, "gs_l1_ssim_loss")

@@ -1,0 +1,109 @@
+"""GPU parity of the fused L1 + SSIM loss (gs_l1_ssim_loss) against oracle/ssim_oracle.py
+through the C ABI.  Bars: loss within 1e-5 absolute (fp32 sums of values in [0, 1]); dL/dimage within relative L2
+1e-3 (the north_star's gradient bar) and, element by element, within 1e-3 of the largest gradient magnitude."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_11390_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    from oracle import ssim_oracle
+    return ssim_oracle
+
+
+def run(B, x, y, lam):
+    dx, dy = torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()
+    dL = torch.full_like(dx, float("nan"))
+    loss = torch.zeros((1,), dtype=torch.float32, device="cuda")
+    C, H, W, _ = x.shape
+    ws = torch.empty((B.gs_l1_ssim_loss_workspace_bytes(C, H, W),), dtype=torch.uint8, device="cuda")
+    B.gs_l1_ssim_loss(dx, dy, lam, dL, loss, ws)
+    torch.cuda.synchronize()
+    return float(loss.item()), dL.cpu().numpy()
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, np.float64).ravel(); b = np.asarray(b, np.float64).ravel()
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-30))
+
+
+def images(shape, seed, smooth=False):
+    rng = np.random.default_rng(seed)
+    x = rng.random(shape, dtype=np.float32)
+    y = rng.random(shape, dtype=np.float32)
+    if smooth:                                  # correlated pair, like a render and its target
+        y = np.clip(0.8 * x + 0.2 * y, 0.0, 1.0).astype(np.float32)
+    return x, y
+
+
+@pytest.mark.parametrize("shape,lam,smooth", [
+    ((1, 16, 16, 3), 0.2, False),               # exactly one tile
+    ((2, 37, 45, 3), 0.2, False),               # several tiles, ragged in both directions, two views
+    ((1, 5, 7, 3), 0.2, False),                 # smaller than the window: every window is cut by the padding
+    ((3, 64, 80, 3), 1.0, True),                # SSIM term only, correlated images
+    ((1, 33, 17, 3), 0.0, False),               # L1 term only
+    ((1, 1, 1, 3), 0.2, False),                 # a single pixel
+])
+def test_l1_ssim_parity(B, oracle, shape, lam, smooth):
+    x, y = images(shape, sum(shape) + int(lam * 10), smooth)
+    L_ref, g_ref = oracle.l1_ssim_loss_grad(x, y, lam)
+    L, g = run(B, x, y, lam)
+    assert np.isfinite(g).all()
+    assert abs(L - L_ref) <= 1e-5, (L, L_ref)
+    assert rel_l2(g, g_ref) <= 1e-3
+    assert np.abs(g - g_ref).max() <= 1e-3 * np.abs(g_ref).max()
+    print(f"{shape} lam {lam}: loss err {abs(L - L_ref):.1e}, grad rel L2 {rel_l2(g, g_ref):.1e}")
+
+
+def test_identical_images(B):
+    x, _ = images((1, 40, 24, 3), 3)
+    L, g = run(B, x, x.copy(), 0.2)
+    assert abs(L) <= 1e-6                       # SSIM(x, x) = 1, |x - x| = 0
+    assert np.abs(g).max() <= 1e-6              # stationary point of the SSIM term; sign(0) = 0 for the L1 term
+
+
+def test_loss_accumulates_and_gradient_is_overwritten(B):
+    x, y = images((1, 20, 20, 3), 4)
+    dx, dy = torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()
+    dL = torch.full_like(dx, 7.0)
+    loss = torch.full((1,), 2.0, dtype=torch.float32, device="cuda")
+    ws = torch.empty((B.gs_l1_ssim_loss_workspace_bytes(1, 20, 20),), dtype=torch.uint8, device="cuda")
+    B.gs_l1_ssim_loss(dx, dy, 0.2, dL, loss, ws)
+    first = dL.clone()
+    B.gs_l1_ssim_loss(dx, dy, 0.2, dL, loss, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(first, dL)
+    from oracle import ssim_oracle
+    L_ref = ssim_oracle.l1_ssim_loss(x, y, 0.2)
+    assert abs(float(loss.item()) - (2.0 + 2 * L_ref)) <= 1e-5
+
+
+def test_full_hd_view_sampled_rows(B, oracle):
+    """One 1920 x 1080 view (the object workload's image size, the launch configuration bench.py times): the oracle
+    evaluates a horizontal band exactly (a band's values depend only on rows within 10 of it, and the loss weight 1 / n
+    is that of the full image)."""
+    H, W = 1080, 1920
+    x, y = images((1, H, W, 3), 11, smooth=True)
+    L, g = run(B, x, y, 0.2)
+    lo, hi = 500, 560                            # rows checked
+    a, b = lo - 10, hi + 10
+    n_full, n_band = x.size, x[:, a:b].size
+    _, g_band = oracle.l1_ssim_loss_grad(x[:, a:b], y[:, a:b], 0.2)
+    g_ref = g_band[:, 10:-10] * (n_band / n_full)
+    assert rel_l2(g[:, lo:hi], g_ref) <= 1e-3
+    assert np.isfinite(L) and 0.0 < L < 1.0
+    # first and last rows of the image are cut by the zero padding: compare them too
+    _, g_top = oracle.l1_ssim_loss_grad(x[:, :40], y[:, :40], 0.2)
+    assert rel_l2(g[:, :30], g_top[:, :30] * (x[:, :40].size / n_full)) <= 1e-3

@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="object", choices=["tiny", "object", "room", "block", "city"])
     ap.add_argument("--n", type=int, default=None, help="override the Gaussian count (debugging only)")
+    ap.add_argument("--loss", default="l1", choices=["l1", "l1ssim"],
+                    help="loss of the step: mean L1 (BASELINE.json configs, default) or the fused 0.8 L1 + 0.2 (1 - SSIM) (SURVEY 8(f) NEXT-1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
@@ -270,6 +272,7 @@ def run_b200(args):
     tgt_host = scenes.target_image(sc)
     st = SplatStep(sc, device=dev)
     st.set_target(tgt_host)
+    st.loss_mode = args.loss
     C, N, W, H = st.C, st.N, st.W, st.H
     # size the intersection buffers once (one synchronising pass), then run without host syncs
     st.forward(sync=True)
@@ -340,7 +343,8 @@ def run_b200(args):
         # compaction (radii; uv, depth -> key, id) + depth sort (histogram, P_d passes) + entry table + tile sort + grid scans, ranges
         "bin_tiles": 4 * N * C + 24 * V_sum + (8 + 24 * P_d) * V_sum + (32 + 16) * V_sum + tsort_bytes + 24 * cells + 16 * C * st.gx * st.gy,
         "project_bwd": 4 * N * C + 36 * V_sum + par_b * V_any + par_b * N,
-        "l1_loss": 12 * C * W * H * 3,
+        # L1: read image, target, write dL; L1 + SSIM: + three derivative maps written and read, image and target read twice
+        "l1_loss": (12 if args.loss == "l1" else 44) * C * W * H * 3,
         # flops (per evaluated (pixel, record) pair: DESIGN.md "algorithmic flops per pair")
         "raster_fwd": 22 * pairs_bwd,
         "raster_bwd": 60 * pairs_bwd,
@@ -406,7 +410,7 @@ def run_b200(args):
         "metric": METRIC, "value": value, "unit": "MP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": args.workload, "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
+        "config": {"workload": args.workload, "loss": args.loss, "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
                    "intersections": M_now, "visible_entries": V_sum, "pairs_bwd": pairs_bwd,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},

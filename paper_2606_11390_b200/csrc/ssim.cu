@@ -32,15 +32,31 @@ struct SsimArgs {
     float win[kSsimWin];
 };
 
-// rows i0-5 .. i0+20, pixels j0-5 .. j0+20 of view v, all three channels, zero outside the image
-__device__ __forceinline__ void load_halo(const float* __restrict__ img, int v, int i0, int j0, int H, int W, float (*s)[kSsimRowPad]) {
-    for (int k = threadIdx.x; k < kSsimHalo * kSsimRow; k += blockDim.x) {
-        const int r = k / kSsimRow, c = k - r * kSsimRow;
-        const int gi = i0 - kSsimR + r, gj = j0 - kSsimR + c / 3;
-        float val = 0.0f;
-        if (gi >= 0 && gi < H && gj >= 0 && gj < W) val = __ldg(img + ((int64_t)(v * (int64_t)H + gi) * W + (j0 - kSsimR)) * 3 + c);
-        s[r][c] = val;
+// rows i0-5 .. i0+20, pixels j0-5 .. j0+20 of view v, all three channels, zero outside the image; a warp takes whole
+// rows (78 contiguous floats: three coalesced requests).  The elements go global -> shared with cp.async (4 bytes each,
+// zero-filled outside the image), so every load of every halo tile of a block is in flight before the first wait.
+__device__ __forceinline__ void load_halo_async(const float* __restrict__ img, int v, int i0, int j0, int H, int W, float (*s)[kSsimRowPad]) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int r = warp; r < kSsimHalo; r += 8) {
+        const int gi = i0 - kSsimR + r;
+        const bool row_in = gi >= 0 && gi < H;
+        const float* row = img + ((int64_t)(v * (int64_t)H + gi) * W + (j0 - kSsimR)) * 3;
+#pragma unroll
+        for (int it = 0; it < 3; ++it) {
+            const int c = lane + 32 * it;
+            if (c < kSsimRow) {
+                const int gj = j0 - kSsimR + c / 3;
+                const bool in = row_in && gj >= 0 && gj < W;
+                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&s[r][c]);
+                const float* src = in ? row + c : img;          // not read when the source size is 0
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(in ? 4 : 0) : "memory");
+            }
+        }
     }
+}
+__device__ __forceinline__ void halo_wait() {
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
 }
 
 __device__ __forceinline__ float block_sum(float v, float* s_red) {
@@ -55,60 +71,105 @@ __device__ __forceinline__ float block_sum(float v, float* s_red) {
     return t;               // valid in thread 0
 }
 
+// Both passes of the separable window keep a run of outputs in registers and stream over the inputs (4 outputs from 14
+// inputs), so an input is read from shared memory once per run instead of once per tap; the three channels are processed
+// together.  Horizontal tasks: (row, column group of 4, channel); vertical tasks: (row group of 4, column, channel) with
+// the channel fastest, so that consecutive threads write consecutive addresses of the interleaved [.., 3] layout.
+constexpr int kSsimRun = 4;
+constexpr int kSsimIn = kSsimRun + kSsimWin - 1;        // 14 inputs feed 4 outputs
+constexpr int kHzRow = kSsimTile + 1;
+
+template <int Q>
+struct HzBuf {
+    // per-channel stride = 11 (mod 32) words: the vertical pass reads (channel, column) across a warp -> banks column + 11 channel
+    static constexpr int kPad = (11 - (Q * kSsimHalo * kHzRow) % 32 + 32) % 32;
+    float v[3][Q * kSsimHalo * kHzRow + kPad];
+    __device__ __forceinline__ float& at(int ch, int q, int r, int c) { return v[ch][(q * kSsimHalo + r) * kHzRow + c]; }
+};
+
 __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
     __shared__ float sx[kSsimHalo][kSsimRowPad], sy[kSsimHalo][kSsimRowPad];
-    __shared__ float hz[5][kSsimHalo][kSsimTile + 1];
+    __shared__ HzBuf<5> hz;
     __shared__ float s_red[8];
     const int v = blockIdx.z, i0 = blockIdx.y * kSsimTile, j0 = blockIdx.x * kSsimTile;
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-    load_halo(a.x, v, i0, j0, a.H, a.W, sx);
-    load_halo(a.y, v, i0, j0, a.H, a.W, sy);
+    load_halo_async(a.x, v, i0, j0, a.H, a.W, sx);
+    load_halo_async(a.y, v, i0, j0, a.H, a.W, sy);
+    halo_wait();
+    // horizontal pass
+    for (int task = threadIdx.x; task < kSsimHalo * 3 * (kSsimTile / kSsimRun); task += 256) {
+        const int r = task / 12, rem = task - r * 12, cg = rem / 3, ch = rem - cg * 3;
+        float acc[kSsimRun][5];
+#pragma unroll
+        for (int o = 0; o < kSsimRun; ++o)
+#pragma unroll
+            for (int q = 0; q < 5; ++q) acc[o][q] = 0.0f;
+#pragma unroll
+        for (int p = 0; p < kSsimIn; ++p) {
+            const float xv = sx[r][(kSsimRun * cg + p) * 3 + ch], yv = sy[r][(kSsimRun * cg + p) * 3 + ch];
+            const float xx = xv * xv, yy = yv * yv, xy = xv * yv;
+#pragma unroll
+            for (int o = 0; o < kSsimRun; ++o) {
+                const int t = p - o;
+                if (t >= 0 && t < kSsimWin) {
+                    const float w = a.win[t];
+                    acc[o][0] = fmaf(w, xv, acc[o][0]); acc[o][1] = fmaf(w, yv, acc[o][1]);
+                    acc[o][2] = fmaf(w, xx, acc[o][2]); acc[o][3] = fmaf(w, yy, acc[o][3]); acc[o][4] = fmaf(w, xy, acc[o][4]);
+                }
+            }
+        }
+#pragma unroll
+        for (int o = 0; o < kSsimRun; ++o)
+#pragma unroll
+            for (int q = 0; q < 5; ++q) hz.at(ch, q, r, kSsimRun * cg + o) = acc[o][q];
+    }
     __syncthreads();
-    const int gi = i0 + ty, gj = j0 + tx;
-    const bool inside = gi < a.H && gj < a.W;
-    const int64_t pix = ((int64_t)v * a.H + gi) * a.W + gj;
+    // vertical pass, SSIM and its derivatives
     const float wgt = -a.lambda * a.inv_n;
     float ssim_sum = 0.0f, l1_sum = 0.0f;
-    for (int ch = 0; ch < 3; ++ch) {
-        // horizontal pass: 26 rows x 16 columns, five quantities
-        for (int k = threadIdx.x; k < kSsimHalo * kSsimTile; k += 256) {
-            const int r = k >> 4, c = k & 15;
-            float m1 = 0.f, m2 = 0.f, e11 = 0.f, e22 = 0.f, e12 = 0.f;
+    if (threadIdx.x < 3 * kSsimTile * (kSsimTile / kSsimRun)) {
+        const int ch = threadIdx.x % 3, col = (threadIdx.x / 3) % kSsimTile, g = threadIdx.x / (3 * kSsimTile);
+        float acc[kSsimRun][5];
 #pragma unroll
-            for (int t = 0; t < kSsimWin; ++t) {
-                const float w = a.win[t];
-                const float xv = sx[r][(c + t) * 3 + ch], yv = sy[r][(c + t) * 3 + ch];
-                m1 = fmaf(w, xv, m1); m2 = fmaf(w, yv, m2);
-                e11 = fmaf(w * xv, xv, e11); e22 = fmaf(w * yv, yv, e22); e12 = fmaf(w * xv, yv, e12);
+        for (int o = 0; o < kSsimRun; ++o)
+#pragma unroll
+            for (int q = 0; q < 5; ++q) acc[o][q] = 0.0f;
+#pragma unroll
+        for (int p = 0; p < kSsimIn; ++p) {
+            float in[5];
+#pragma unroll
+            for (int q = 0; q < 5; ++q) in[q] = hz.at(ch, q, kSsimRun * g + p, col);
+#pragma unroll
+            for (int o = 0; o < kSsimRun; ++o) {
+                const int t = p - o;
+                if (t >= 0 && t < kSsimWin) {
+                    const float w = a.win[t];
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) acc[o][q] = fmaf(w, in[q], acc[o][q]);
+                }
             }
-            hz[0][r][c] = m1; hz[1][r][c] = m2; hz[2][r][c] = e11; hz[3][r][c] = e22; hz[4][r][c] = e12;
         }
-        __syncthreads();
-        // vertical pass at this thread's pixel
-        float mu1 = 0.f, mu2 = 0.f, e11 = 0.f, e22 = 0.f, e12 = 0.f;
+        const int gj = j0 + col;
 #pragma unroll
-        for (int t = 0; t < kSsimWin; ++t) {
-            const float w = a.win[t];
-            mu1 = fmaf(w, hz[0][ty + t][tx], mu1); mu2 = fmaf(w, hz[1][ty + t][tx], mu2);
-            e11 = fmaf(w, hz[2][ty + t][tx], e11); e22 = fmaf(w, hz[3][ty + t][tx], e22); e12 = fmaf(w, hz[4][ty + t][tx], e12);
+        for (int o = 0; o < kSsimRun; ++o) {
+            const int ty = kSsimRun * g + o, gi = i0 + ty;
+            if (gi < a.H && gj < a.W) {
+                const float mu1 = acc[o][0], mu2 = acc[o][1];
+                const float s11 = acc[o][2] - mu1 * mu1, s22 = acc[o][3] - mu2 * mu2, s12 = acc[o][4] - mu1 * mu2;
+                const float A1 = fmaf(2.0f * mu1, mu2, kSsimC1), A2 = fmaf(2.0f, s12, kSsimC2);
+                const float B1 = fmaf(mu1, mu1, fmaf(mu2, mu2, kSsimC1)), B2 = s11 + s22 + kSsimC2;
+                const float inv = 1.0f / (B1 * B2);
+                const float S = A1 * A2 * inv;
+                const float d11 = -S / B2;                                   // dS/ds11
+                const float d12 = 2.0f * A1 * inv;                           // dS/ds12
+                const float dmu = 2.0f * mu2 * A2 * inv - 2.0f * mu1 * S / B1 - 2.0f * mu1 * d11 - mu2 * d12;   // total dS/dmu1
+                const int64_t o3 = 3 * (((int64_t)v * a.H + gi) * a.W + gj) + ch;
+                a.maps[o3] = wgt * dmu;
+                a.maps[a.n + o3] = wgt * d11;
+                a.maps[2 * a.n + o3] = wgt * d12;
+                ssim_sum += S;
+                l1_sum += fabsf(sx[ty + kSsimR][(col + kSsimR) * 3 + ch] - sy[ty + kSsimR][(col + kSsimR) * 3 + ch]);
+            }
         }
-        if (inside) {
-            const float s11 = e11 - mu1 * mu1, s22 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
-            const float A1 = fmaf(2.0f * mu1, mu2, kSsimC1), A2 = fmaf(2.0f, s12, kSsimC2);
-            const float B1 = fmaf(mu1, mu1, fmaf(mu2, mu2, kSsimC1)), B2 = s11 + s22 + kSsimC2;
-            const float inv = 1.0f / (B1 * B2);
-            const float S = A1 * A2 * inv;
-            const float d11 = -S / B2;                                   // dS/ds11
-            const float d12 = 2.0f * A1 * inv;                           // dS/ds12
-            const float dmu = 2.0f * mu2 * A2 * inv - 2.0f * mu1 * S / B1 - 2.0f * mu1 * d11 - mu2 * d12;   // total dS/dmu1
-            const int64_t o = 3 * pix + ch;
-            a.maps[o] = wgt * dmu;
-            a.maps[a.n + o] = wgt * d11;
-            a.maps[2 * a.n + o] = wgt * d12;
-            ssim_sum += S;
-            l1_sum += fabsf(sx[ty + kSsimR][(tx + kSsimR) * 3 + ch] - sy[ty + kSsimR][(tx + kSsimR) * 3 + ch]);
-        }
-        __syncthreads();        // hz is rewritten for the next channel
     }
     const float part = (1.0f - a.lambda) * l1_sum * a.inv_n - a.lambda * ssim_sum * a.inv_n;
     float tot = block_sum(part, s_red);
@@ -120,44 +181,70 @@ __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
 
 __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
     __shared__ float sm[3][kSsimHalo][kSsimRowPad];
-    __shared__ float hz[3][kSsimHalo][kSsimTile + 1];
+    __shared__ HzBuf<3> hz;
     const int v = blockIdx.z, i0 = blockIdx.y * kSsimTile, j0 = blockIdx.x * kSsimTile;
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
 #pragma unroll
-    for (int q = 0; q < 3; ++q) load_halo(a.maps + q * a.n, v, i0, j0, a.H, a.W, sm[q]);
-    __syncthreads();
-    const int gi = i0 + ty, gj = j0 + tx;
-    const bool inside = gi < a.H && gj < a.W;
-    const int64_t pix = ((int64_t)v * a.H + gi) * a.W + gj;
-    const float l1w = (1.0f - a.lambda) * a.inv_n;
-    for (int ch = 0; ch < 3; ++ch) {
-        for (int k = threadIdx.x; k < kSsimHalo * kSsimTile; k += 256) {
-            const int r = k >> 4, c = k & 15;
-            float g0 = 0.f, g1 = 0.f, g2 = 0.f;
+    for (int q = 0; q < 3; ++q) load_halo_async(a.maps + q * a.n, v, i0, j0, a.H, a.W, sm[q]);
+    halo_wait();
+    for (int task = threadIdx.x; task < kSsimHalo * 3 * (kSsimTile / kSsimRun); task += 256) {
+        const int r = task / 12, rem = task - r * 12, cg = rem / 3, ch = rem - cg * 3;
+        float acc[kSsimRun][3];
 #pragma unroll
-            for (int t = 0; t < kSsimWin; ++t) {
-                const float w = a.win[t];
-                g0 = fmaf(w, sm[0][r][(c + t) * 3 + ch], g0);
-                g1 = fmaf(w, sm[1][r][(c + t) * 3 + ch], g1);
-                g2 = fmaf(w, sm[2][r][(c + t) * 3 + ch], g2);
+        for (int o = 0; o < kSsimRun; ++o) acc[o][0] = acc[o][1] = acc[o][2] = 0.0f;
+#pragma unroll
+        for (int p = 0; p < kSsimIn; ++p) {
+            float in[3];
+#pragma unroll
+            for (int q = 0; q < 3; ++q) in[q] = sm[q][r][(kSsimRun * cg + p) * 3 + ch];
+#pragma unroll
+            for (int o = 0; o < kSsimRun; ++o) {
+                const int t = p - o;
+                if (t >= 0 && t < kSsimWin) {
+                    const float w = a.win[t];
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) acc[o][q] = fmaf(w, in[q], acc[o][q]);
+                }
             }
-            hz[0][r][c] = g0; hz[1][r][c] = g1; hz[2][r][c] = g2;
         }
-        __syncthreads();
-        float g0 = 0.f, g1 = 0.f, g2 = 0.f;
 #pragma unroll
-        for (int t = 0; t < kSsimWin; ++t) {
-            const float w = a.win[t];
-            g0 = fmaf(w, hz[0][ty + t][tx], g0); g1 = fmaf(w, hz[1][ty + t][tx], g1); g2 = fmaf(w, hz[2][ty + t][tx], g2);
+        for (int o = 0; o < kSsimRun; ++o)
+#pragma unroll
+            for (int q = 0; q < 3; ++q) hz.at(ch, q, r, kSsimRun * cg + o) = acc[o][q];
+    }
+    __syncthreads();
+    if (threadIdx.x < 3 * kSsimTile * (kSsimTile / kSsimRun)) {
+        const int ch = threadIdx.x % 3, col = (threadIdx.x / 3) % kSsimTile, g = threadIdx.x / (3 * kSsimTile);
+        float acc[kSsimRun][3];
+#pragma unroll
+        for (int o = 0; o < kSsimRun; ++o) acc[o][0] = acc[o][1] = acc[o][2] = 0.0f;
+#pragma unroll
+        for (int p = 0; p < kSsimIn; ++p) {
+            float in[3];
+#pragma unroll
+            for (int q = 0; q < 3; ++q) in[q] = hz.at(ch, q, kSsimRun * g + p, col);
+#pragma unroll
+            for (int o = 0; o < kSsimRun; ++o) {
+                const int t = p - o;
+                if (t >= 0 && t < kSsimWin) {
+                    const float w = a.win[t];
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) acc[o][q] = fmaf(w, in[q], acc[o][q]);
+                }
+            }
         }
-        if (inside) {
-            const int64_t o = 3 * pix + ch;
-            const float xv = __ldg(a.x + o), yv = __ldg(a.y + o);
-            const float d = xv - yv;
-            const float l1 = d > 0.f ? l1w : (d < 0.f ? -l1w : 0.f);
-            a.dL[o] = fmaf(2.0f * xv, g1, fmaf(yv, g2, g0)) + l1;
+        const float l1w = (1.0f - a.lambda) * a.inv_n;
+        const int gj = j0 + col;
+#pragma unroll
+        for (int o = 0; o < kSsimRun; ++o) {
+            const int gi = i0 + kSsimRun * g + o;
+            if (gi < a.H && gj < a.W) {
+                const int64_t o3 = 3 * (((int64_t)v * a.H + gi) * a.W + gj) + ch;
+                const float xv = __ldg(a.x + o3), yv = __ldg(a.y + o3);
+                const float d = xv - yv;
+                const float l1 = d > 0.f ? l1w : (d < 0.f ? -l1w : 0.f);
+                a.dL[o3] = fmaf(2.0f * xv, acc[o][1], fmaf(yv, acc[o][2], acc[o][0])) + l1;
+            }
         }
-        __syncthreads();
     }
 }
 

@@ -108,8 +108,16 @@ class SplatStep:
                         self.rgbs, self.bg, self.image, self.final_T, self.n_contrib)
 
     def l1_loss(self):
+        """The step's loss: mean L1 (reading A18, default) or, with ``loss_mode = "l1ssim"``, the fused
+        0.8 L1 + 0.2 (1 - SSIM) loss of the paper's reference method (gs_l1_ssim_loss)."""
         self.loss.zero_()
-        B.gs_l1_loss(self.image, self.target, self.dL_dimage, self.loss)
+        if getattr(self, "loss_mode", "l1") == "l1ssim":
+            if getattr(self, "_ssim_ws", None) is None:
+                nbytes = B.gs_l1_ssim_loss_workspace_bytes(self.C, self.H, self.W)
+                self._ssim_ws = torch.empty((nbytes,), dtype=torch.uint8, device=self.device)
+            B.gs_l1_ssim_loss(self.image, self.target, 0.2, self.dL_dimage, self.loss, self._ssim_ws)
+        else:
+            B.gs_l1_loss(self.image, self.target, self.dL_dimage, self.loss)
 
     def raster_bwd(self):
         B.gs_raster_bwd(self.cfg, self.cams, self.C * self.N, self.isect_vals, self.tile_ranges, self.means2d, self.conics,
@@ -172,4 +180,5 @@ class SplatStep:
         tile_passes = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
         compact = 2 if self.C * self.N >= (1 << 24) else 1          # visibility mask + scan over the mask for large inputs
         p5 = 6 if self.N >= (1 << 22) else 1                         # dense zero-fill as five streaming launches for large N
-        return (p5 - 1) + 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1
+        loss = 2 if getattr(self, "loss_mode", "l1") == "l1ssim" else 1
+        return (loss - 1) + (p5 - 1) + 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

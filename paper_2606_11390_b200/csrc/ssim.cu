@@ -37,19 +37,32 @@ struct SsimArgs {
 // zero-filled outside the image), so every load of every halo tile of a block is in flight before the first wait.
 __device__ __forceinline__ void load_halo_async(const float* __restrict__ img, int v, int i0, int j0, int H, int W, float (*s)[kSsimRowPad]) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int r = warp; r < kSsimHalo; r += 8) {
-        const int gi = i0 - kSsimR + r;
-        const bool row_in = gi >= 0 && gi < H;
-        const float* row = img + ((int64_t)(v * (int64_t)H + gi) * W + (j0 - kSsimR)) * 3;
+    // per-thread column state (the same for every row): three elements c = lane + 32 it of the 78-float row
+    bool col_in[3];
 #pragma unroll
-        for (int it = 0; it < 3; ++it) {
-            const int c = lane + 32 * it;
-            if (c < kSsimRow) {
-                const int gj = j0 - kSsimR + c / 3;
-                const bool in = row_in && gj >= 0 && gj < W;
-                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&s[r][c]);
-                const float* src = in ? row + c : img;          // not read when the source size is 0
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(in ? 4 : 0) : "memory");
+    for (int it = 0; it < 3; ++it) {
+        const int c = lane + 32 * it;
+        const int gj = j0 - kSsimR + c / 3;
+        col_in[it] = c < kSsimRow && gj >= 0 && gj < W;
+    }
+    const uint32_t dst0 = (uint32_t)__cvta_generic_to_shared(&s[0][lane]);
+    const float* src0 = img + ((int64_t)(v * (int64_t)H + (i0 - kSsimR)) * W + (j0 - kSsimR)) * 3 + lane;
+    const int64_t row_stride = (int64_t)W * 3;
+#pragma unroll
+    for (int k = 0; k < (kSsimHalo + 7) / 8; ++k) {
+        const int r = warp + 8 * k;
+        if (r < kSsimHalo) {
+            const int gi = i0 - kSsimR + r;
+            const bool row_in = gi >= 0 && gi < H;
+            const float* row = src0 + r * row_stride;
+            const uint32_t drow = dst0 + (uint32_t)(r * kSsimRowPad * 4);
+#pragma unroll
+            for (int it = 0; it < 3; ++it) {
+                if (lane + 32 * it < kSsimRow) {
+                    const bool in = row_in && col_in[it];
+                    const float* src = in ? row + 32 * it : img;     // not read when the source size is 0
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(drow + 128 * it), "l"(src), "r"(in ? 4 : 0) : "memory");
+                }
             }
         }
     }
@@ -185,6 +198,19 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
     const int v = blockIdx.z, i0 = blockIdx.y * kSsimTile, j0 = blockIdx.x * kSsimTile;
 #pragma unroll
     for (int q = 0; q < 3; ++q) load_halo_async(a.maps + q * a.n, v, i0, j0, a.H, a.W, sm[q]);
+    // x and y at this thread's four output values travel while the window passes run
+    const bool vtask = threadIdx.x < 3 * kSsimTile * (kSsimTile / kSsimRun);
+    const int vch = threadIdx.x % 3, vcol = (threadIdx.x / 3) % kSsimTile, vg = threadIdx.x / (3 * kSsimTile);
+    float xo[kSsimRun], yo[kSsimRun];
+#pragma unroll
+    for (int o = 0; o < kSsimRun; ++o) {
+        const int gi = i0 + kSsimRun * vg + o, gj = j0 + vcol;
+        xo[o] = 0.0f; yo[o] = 0.0f;
+        if (vtask && gi < a.H && gj < a.W) {
+            const int64_t o3 = 3 * (((int64_t)v * a.H + gi) * a.W + gj) + vch;
+            xo[o] = __ldg(a.x + o3); yo[o] = __ldg(a.y + o3);
+        }
+    }
     halo_wait();
     for (int task = threadIdx.x; task < kSsimHalo * 3 * (kSsimTile / kSsimRun); task += 256) {
         const int r = task / 12, rem = task - r * 12, cg = rem / 3, ch = rem - cg * 3;
@@ -212,8 +238,8 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
             for (int q = 0; q < 3; ++q) hz.at(ch, q, r, kSsimRun * cg + o) = acc[o][q];
     }
     __syncthreads();
-    if (threadIdx.x < 3 * kSsimTile * (kSsimTile / kSsimRun)) {
-        const int ch = threadIdx.x % 3, col = (threadIdx.x / 3) % kSsimTile, g = threadIdx.x / (3 * kSsimTile);
+    if (vtask) {
+        const int ch = vch, col = vcol, g = vg;
         float acc[kSsimRun][3];
 #pragma unroll
         for (int o = 0; o < kSsimRun; ++o) acc[o][0] = acc[o][1] = acc[o][2] = 0.0f;
@@ -239,7 +265,7 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
             const int gi = i0 + kSsimRun * g + o;
             if (gi < a.H && gj < a.W) {
                 const int64_t o3 = 3 * (((int64_t)v * a.H + gi) * a.W + gj) + ch;
-                const float xv = __ldg(a.x + o3), yv = __ldg(a.y + o3);
+                const float xv = xo[o], yv = yo[o];
                 const float d = xv - yv;
                 const float l1 = d > 0.f ? l1w : (d < 0.f ? -l1w : 0.f);
                 a.dL[o3] = fmaf(2.0f * xv, acc[o][1], fmaf(yv, acc[o][2], acc[o][0])) + l1;

@@ -161,6 +161,21 @@ int gs_l1_loss(int64_t n, const float* image, const float* target, float* dL_dim
 int gs_l1_ssim_loss(int32_t C, int32_t height, int32_t width, const float* image, const float* target, float lambda,
                     float* dL_dimage, float* loss_sum, void* workspace, size_t* workspace_bytes, void* stream);
 
+/* 3-D Morton ordering of the Gaussian arrays ("sorted along a Morton curve").
+ * Sequence: gs_bounds -> gs_morton_codes -> gs_sort_pairs(N, 63, 0, codes, index, ...) -> gs_gather_rows per array.
+ * All pointers are device pointers; everything is asynchronous on `stream`; no allocation, no host synchronisation.
+ *
+ * gs_bounds: lo_hi[6] (device) = min x, y, z, max x, y, z of means[N,3] (N >= 1; NaNs order as their bit patterns).
+ * gs_morton_codes: per Gaussian q_a = clamp(floor((p_a - lo_a) * (2^21 / (hi_a - lo_a))), 0, 2^21 - 1) in fp32 with one
+ *   rounding per operation (scale 1 for a degenerate axis, q = 0 for a non-finite product); codes[i] = bits of
+ *   (qx, qy, qz) interleaved, bit k of qx at 3k+2, qy at 3k+1, qz at 3k (63 bits); index[i] = i.  N < 2^31.
+ * gs_gather_rows: dst[i, :] = src[perm[i], :] for rows of row_floats floats (src != dst; 16-byte accesses when
+ *   row_floats % 4 == 0 and both pointers are 16-byte aligned).
+ * Errors: GS_ERR_INVALID_ARGUMENT (null pointers, sizes out of range, src == dst), GS_ERR_CUDA. */
+int gs_bounds(int64_t N, const float* means, float* lo_hi, void* stream);
+int gs_morton_codes(int64_t N, const float* means, const float* lo_hi, uint64_t* codes, int32_t* index, void* stream);
+int gs_gather_rows(int64_t N, int32_t row_floats, const float* src, const int32_t* perm, float* dst, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

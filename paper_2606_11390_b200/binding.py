@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, os.environ.get("GS_LIB_NAME", "libgsplat_b200.so"
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
-           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss"]
+           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows"]
 
 
 class gs_camera(C.Structure):
@@ -239,3 +239,48 @@ def gs_l1_ssim_loss(image, target, lam, dL_dimage, loss_sum, workspace, stream=N
                                C.c_float(lam), _ptr(dL_dimage, torch.float32), _ptr(loss_sum, torch.float32),
                                _ptr(workspace, torch.uint8), C.byref(nbytes), _stream(stream))
     _check(rc, "gs_l1_ssim_loss")
+
+
+def gs_bounds(means, lo_hi, stream=None):
+    import torch
+    rc = lib().gs_bounds(C.c_int64(means.shape[0]), _ptr(means, torch.float32), _ptr(lo_hi, torch.float32), _stream(stream))
+    _check(rc, "gs_bounds")
+
+
+def gs_morton_codes(means, lo_hi, codes, index, stream=None):
+    """codes: int64 tensor holding the uint64 bit patterns; index: int32."""
+    import torch
+    rc = lib().gs_morton_codes(C.c_int64(means.shape[0]), _ptr(means, torch.float32), _ptr(lo_hi, torch.float32),
+                               _ptr(codes, torch.int64), _ptr(index, torch.int32), _stream(stream))
+    _check(rc, "gs_morton_codes")
+
+
+def gs_gather_rows(src, perm, dst, stream=None):
+    import torch
+    N = src.shape[0]
+    row = src.numel() // max(N, 1)
+    rc = lib().gs_gather_rows(C.c_int64(N), C.c_int32(row), _ptr(src, torch.float32), _ptr(perm, torch.int32),
+                              _ptr(dst, torch.float32), _stream(stream))
+    _check(rc, "gs_gather_rows")
+
+
+def morton_sort(params, stream=None):
+    """Reorder the parameter tensors (dict of [N, ...] float32 CUDA tensors with key "means") along the Morton curve of the
+    means.  Returns (sorted dict, perm int32[N]).  Orchestration only: bounds, codes, radix sort and gathers are kernels."""
+    import torch
+    means = params["means"]
+    N = means.shape[0]
+    dev = means.device
+    lo_hi = torch.empty((6,), dtype=torch.float32, device=dev)
+    codes = torch.empty((N,), dtype=torch.int64, device=dev)
+    perm = torch.empty((N,), dtype=torch.int32, device=dev)
+    gs_bounds(means, lo_hi, stream)
+    gs_morton_codes(means, lo_hi, codes, perm, stream)
+    ws = torch.empty((gs_sort_pairs_workspace_bytes(N),), dtype=torch.uint8, device=dev)
+    gs_sort_pairs(N, 63, 0, codes, perm, ws, stream)
+    out = {}
+    for k, t in params.items():
+        d = torch.empty_like(t)
+        gs_gather_rows(t, perm, d, stream)
+        out[k] = d
+    return out, perm

@@ -43,6 +43,9 @@ def parse_args():
     ap.add_argument("--n", type=int, default=None, help="override the Gaussian count (debugging only)")
     ap.add_argument("--loss", default="l1", choices=["l1", "l1ssim"],
                     help="loss of the step: mean L1 (BASELINE.json configs, default) or the fused 0.8 L1 + 0.2 (1 - SSIM) (SURVEY 8(f) NEXT-1)")
+    ap.add_argument("--morton", action="store_true",
+                    help="reorder the Gaussian arrays along the Morton curve of the means before timing (SURVEY 8(f) NEXT-2; "
+                         "one-time preprocessing, its device time is reported as morton_sort_ms, not part of a step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
@@ -273,6 +276,19 @@ def run_b200(args):
     st = SplatStep(sc, device=dev)
     st.set_target(tgt_host)
     st.loss_mode = args.loss
+    morton_ms = None
+    if args.morton:
+        B.morton_sort({k: st.params[k] for k in st.param_names})          # warm-up (allocations, first launches)
+        torch.cuda.synchronize()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record()
+        sorted_params, _ = B.morton_sort({k: st.params[k] for k in st.param_names})
+        m1.record()
+        torch.cuda.synchronize()
+        morton_ms = m0.elapsed_time(m1)
+        for k in st.param_names:
+            st.params[k].copy_(sorted_params[k])
+        del sorted_params
     C, N, W, H = st.C, st.N, st.W, st.H
     # size the intersection buffers once (one synchronising pass), then run without host syncs
     st.forward(sync=True)
@@ -410,11 +426,12 @@ def run_b200(args):
         "metric": METRIC, "value": value, "unit": "MP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": args.workload, "loss": args.loss, "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
+        "config": {"workload": args.workload, "loss": args.loss, "morton": bool(args.morton), "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
                    "intersections": M_now, "visible_entries": V_sum, "pairs_bwd": pairs_bwd,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},
         "gaussians_per_s": gauss_per_s,
+        "morton_sort_ms": morton_ms,
         "clocks": clocks,
         "e2e": e2e,
         "gpu_launches": st.launches_per_step() * args.steps,

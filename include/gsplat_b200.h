@@ -176,6 +176,17 @@ int gs_bounds(int64_t N, const float* means, float* lo_hi, void* stream);
 int gs_morton_codes(int64_t N, const float* means, const float* lo_hi, uint64_t* codes, int32_t* index, void* stream);
 int gs_gather_rows(int64_t N, int32_t row_floats, const float* src, const int32_t* perm, float* dst, void* stream);
 
+/* Fused Adam step over one parameter array, in place:
+ *   m <- beta1 m + (1 - beta1) g;  v <- beta2 v + (1 - beta2) g^2;
+ *   p <- p - lr (m / (1 - beta1^step)) / (sqrt(v / (1 - beta2^step)) + eps)         (no weight decay, no amsgrad)
+ * param, grad, m, v: [N, row_floats] fp32 (device); step >= 1.
+ * radii == NULL: every element is updated (16-byte accesses when all four pointers are 16-byte aligned).
+ * radii != NULL ([C, N] int32 as saved by gs_project_fwd): only the rows of Gaussians with radius > 0 in at least one
+ * of the C views are updated; parameter and moments of every other row are left untouched.
+ * Asynchronous on `stream`.  Errors: GS_ERR_INVALID_ARGUMENT, GS_ERR_CUDA. */
+int gs_adam_step(int64_t N, int32_t row_floats, float* param, const float* grad, float* m, float* v, float lr, float beta1,
+                 float beta2, float eps, int32_t step, const int32_t* radii, int32_t C, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

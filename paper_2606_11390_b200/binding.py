@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, os.environ.get("GS_LIB_NAME", "libgsplat_b200.so"
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
-           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows"]
+           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step"]
 
 
 class gs_camera(C.Structure):
@@ -284,3 +284,16 @@ def morton_sort(params, stream=None):
         gs_gather_rows(t, perm, d, stream)
         out[k] = d
     return out, perm
+
+
+def gs_adam_step(param, grad, m, v, lr, beta1, beta2, eps, step, radii=None, stream=None):
+    """In-place Adam step on one [N, ...] float32 array; with ``radii`` ([C, N] int32) only rows visible in >= 1 view."""
+    import torch
+    N = param.shape[0]
+    row = param.numel() // max(N, 1)
+    Cv = int(radii.shape[0]) if radii is not None else 0
+    rc = lib().gs_adam_step(C.c_int64(N), C.c_int32(row), _ptr(param, torch.float32), _ptr(grad, torch.float32),
+                            _ptr(m, torch.float32), _ptr(v, torch.float32), C.c_float(lr), C.c_float(beta1), C.c_float(beta2),
+                            C.c_float(eps), C.c_int32(step), _ptr(radii, torch.int32) if radii is not None else None,
+                            C.c_int32(Cv), _stream(stream))
+    _check(rc, "gs_adam_step")

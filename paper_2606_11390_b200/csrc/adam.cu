@@ -1,0 +1,100 @@
+// adam.cu -- fused Adam step over one parameter array of the Gaussians.
+// m <- b1 m + (1 - b1) g;  v <- b2 v + (1 - b2) g^2;  p <- p - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps)
+// (readings A27, A28).  One streaming pass: 16 bytes read and 12 written per element, 16-byte accesses.  With the saved
+// radii[C, N] the "visible-only" variant touches only the rows of Gaussians visible in >= 1 view of the batch: at street
+// scale that is a fraction of a per cent of the 28 x 59 bytes per Gaussian.
+#include "common.cuh"
+
+namespace gs {
+
+struct AdamArgs {
+    int64_t N;
+    int32_t row;            // floats per Gaussian in this array
+    float* p; const float* g; float* m; float* v;
+    float lr, b1, b2, eps, c1, c2;      // c1 = 1 / (1 - b1^t), c2 = 1 / (1 - b2^t)
+    const int32_t* radii; int32_t C;
+};
+
+__device__ __forceinline__ void adam1(float& p, float g, float& m, float& v, const AdamArgs& a) {
+    m = fmaf(a.b1, m, (1.0f - a.b1) * g);
+    v = fmaf(a.b2, v, (1.0f - a.b2) * g * g);
+    p -= a.lr * (m * a.c1) / (sqrtf(v * a.c2) + a.eps);
+}
+
+// dense: one thread per 16-byte unit
+__global__ void __launch_bounds__(256) adam_dense_kernel(const AdamArgs a, int64_t n4, int64_t n) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n4; k += stride) {
+        float4 p = reinterpret_cast<float4*>(a.p)[k], m = reinterpret_cast<float4*>(a.m)[k], v = reinterpret_cast<float4*>(a.v)[k];
+        const float4 g = __ldg(reinterpret_cast<const float4*>(a.g) + k);
+        adam1(p.x, g.x, m.x, v.x, a); adam1(p.y, g.y, m.y, v.y, a); adam1(p.z, g.z, m.z, v.z, a); adam1(p.w, g.w, m.w, v.w, a);
+        reinterpret_cast<float4*>(a.p)[k] = p; reinterpret_cast<float4*>(a.m)[k] = m; reinterpret_cast<float4*>(a.v)[k] = v;
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (int)(n - 4 * n4)) {
+        const int64_t k = 4 * n4 + threadIdx.x;
+        float p = a.p[k], m = a.m[k], v = a.v[k];
+        adam1(p, a.g[k], m, v, a);
+        a.p[k] = p; a.m[k] = m; a.v[k] = v;
+    }
+}
+
+// scalar fall-back for unaligned arrays, and the visible-only variant: a warp scans 32 Gaussians' radii over the C views
+// and then walks the visible rows, lanes across the row's floats
+__global__ void __launch_bounds__(256) adam_rows_kernel(const AdamArgs a) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t base = warp * 32; base < a.N; base += nwarps * 32) {
+        const int64_t i = base + lane;
+        bool vis = false;
+        if (i < a.N) {
+            vis = a.radii == nullptr;
+            for (int c = 0; c < a.C && !vis; ++c) vis = __ldg(a.radii + (int64_t)c * a.N + i) > 0;
+        }
+        unsigned int mask = __ballot_sync(0xffffffffu, vis);
+        while (mask) {
+            const int s = __ffs(mask) - 1;
+            mask &= mask - 1;
+            const int64_t r0 = (base + s) * a.row;
+            for (int k = lane; k < a.row; k += 32) {
+                float p = a.p[r0 + k], m = a.m[r0 + k], v = a.v[r0 + k];
+                adam1(p, __ldg(a.g + r0 + k), m, v, a);
+                a.p[r0 + k] = p; a.m[r0 + k] = m; a.v[r0 + k] = v;
+            }
+        }
+    }
+}
+
+}  // namespace gs
+
+using namespace gs;
+
+extern "C" int gs_adam_step(int64_t N, int32_t row_floats, float* param, const float* grad, float* m, float* v, float lr, float beta1,
+                            float beta2, float eps, int32_t step, const int32_t* radii, int32_t C, void* stream) {
+    if (N < 0 || row_floats < 1 || row_floats > 4096 || step < 1) return GS_ERR_INVALID_ARGUMENT;
+    if (!(beta1 >= 0.0f && beta1 < 1.0f) || !(beta2 >= 0.0f && beta2 < 1.0f) || !finite_f(lr) || !(eps >= 0.0f)) return GS_ERR_INVALID_ARGUMENT;
+    if (radii && (C < 1 || C > GS_MAX_VIEWS)) return GS_ERR_INVALID_ARGUMENT;
+    if (N == 0) return GS_OK;
+    if (!param || !grad || !m || !v) return GS_ERR_INVALID_ARGUMENT;
+    AdamArgs a;
+    a.N = N; a.row = row_floats; a.p = param; a.g = grad; a.m = m; a.v = v;
+    a.lr = lr; a.b1 = beta1; a.b2 = beta2; a.eps = eps;
+    a.c1 = (float)(1.0 / (1.0 - pow((double)beta1, (double)step)));
+    a.c2 = (float)(1.0 / (1.0 - pow((double)beta2, (double)step)));
+    a.radii = radii; a.C = radii ? C : 0;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t n = N * row_floats;
+    if (!radii && aligned(param, 16) && aligned(grad, 16) && aligned(m, 16) && aligned(v, 16)) {
+        const int64_t n4 = n >> 2;
+        int64_t blocks = (n4 + 255) / 256;
+        if (blocks > (int64_t)sms * 32) blocks = (int64_t)sms * 32;
+        adam_dense_kernel<<<(unsigned)(blocks < 1 ? 1 : blocks), 256, 0, st>>>(a, n4, n);
+    } else {
+        int64_t blocks = (N + 255) / 256;
+        if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
+        adam_rows_kernel<<<(unsigned)blocks, 256, 0, st>>>(a);
+    }
+    return launch_status();
+}

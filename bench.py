@@ -46,6 +46,9 @@ def parse_args():
     ap.add_argument("--morton", action="store_true",
                     help="reorder the Gaussian arrays along the Morton curve of the means before timing (SURVEY 8(f) NEXT-2; "
                          "one-time preprocessing, its device time is reported as morton_sort_ms, not part of a step)")
+    ap.add_argument("--adam", default="none", choices=["none", "dense", "sparse"],
+                    help="append the fused Adam step (SURVEY 8(f) NEXT-3) to the step, with lr = 0 so that the scene stays the same: "
+                         "dense, or sparse = only Gaussians visible in the batch")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
@@ -248,6 +251,7 @@ def whole_job_rate(world, units_per_rank_per_step, ms_per_step):
 
 # ----------------------------------------------------------------------------- B200 leg
 STAGES = ("project_fwd", "bin_tiles", "raster_fwd", "l1_loss", "raster_bwd", "project_bwd")
+STAGES_ADAM = STAGES + ("adam",)
 
 
 def run_b200(args):
@@ -306,8 +310,12 @@ def run_b200(args):
 
     stream = torch.cuda.current_stream()
 
+    STAGES = STAGES_ADAM if args.adam != "none" else globals()["STAGES"]
+
     def timed_step(ev):
         calls = (st.project_fwd, lambda: st.bin_tiles(sync=False), st.raster_fwd, st.l1_loss, st.raster_bwd, st.project_bwd)
+        if args.adam != "none":
+            calls = calls + (lambda: st.adam(args.adam),)
         ev[0].record(stream)
         for k, fn in enumerate(calls):
             fn()
@@ -362,6 +370,8 @@ def run_b200(args):
         # L1: read image, target, write dL; L1 + SSIM: + three derivative maps written and read, image and target read twice
         "l1_loss": (12 if args.loss == "l1" else 44) * C * W * H * 3,
         # flops (per evaluated (pixel, record) pair: DESIGN.md "algorithmic flops per pair")
+        # Adam: p, g, m, v read, p, m, v written, per float; sparse: radii scan + the same for visible rows only
+        "adam": (28 * (par_b // 4) * N if args.adam == "dense" else 4 * N * C + 28 * (par_b // 4) * V_any),
         "raster_fwd": 22 * pairs_bwd,
         "raster_bwd": 60 * pairs_bwd,
     }
@@ -381,7 +391,8 @@ def run_b200(args):
     roof = dict(stage_roof[dominant])
     roof.pop("ms")
     roof["kernel"] = {"raster_bwd": "raster_bwd_kernel", "raster_fwd": "raster_fwd_kernel", "project_fwd": "project_fwd_kernel",
-                      "project_bwd": "project_bwd_kernel", "bin_tiles": "tile_sweep_kernel", "l1_loss": "l1_loss_kernel"}[dominant]
+                      "project_bwd": "project_bwd_kernel", "bin_tiles": "tile_sweep_kernel", "l1_loss": "l1_loss_kernel" if args.loss == "l1" else "ssim_stats_kernel",
+                      "adam": "adam_dense_kernel" if args.adam == "dense" else "adam_visible_multi_kernel"}[dominant]
     roof["share_of_step"] = round(stage_ms[dominant] / (ms_per_step if world == 1 else float(step_ms.mean())), 4)
     roof["peak_source"] = ("MEASURED_PEAKS.json (%s)" % peaks["source"]) if roof["bound"] == "hbm" else \
         f"{sms} SMs x 128 FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)"
@@ -426,7 +437,7 @@ def run_b200(args):
         "metric": METRIC, "value": value, "unit": "MP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": args.workload, "loss": args.loss, "morton": bool(args.morton), "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
+        "config": {"workload": args.workload, "loss": args.loss, "morton": bool(args.morton), "adam": args.adam, "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
                    "intersections": M_now, "visible_entries": V_sum, "pairs_bwd": pairs_bwd,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},
@@ -434,7 +445,7 @@ def run_b200(args):
         "morton_sort_ms": morton_ms,
         "clocks": clocks,
         "e2e": e2e,
-        "gpu_launches": st.launches_per_step() * args.steps,
+        "gpu_launches": (st.launches_per_step() + {"none": 0, "dense": 5, "sparse": 1}[args.adam]) * args.steps,
         "roofline": roof,
         "stages": stage_roof,
         "cpu_baseline": cpu,

@@ -187,6 +187,13 @@ int gs_gather_rows(int64_t N, int32_t row_floats, const float* src, const int32_
 int gs_adam_step(int64_t N, int32_t row_floats, float* param, const float* grad, float* m, float* v, float lr, float beta1,
                  float beta2, float eps, int32_t step, const int32_t* radii, int32_t C, void* stream);
 
+/* The visible-only Adam step over n_arrays (<= 8) parameter arrays in ONE launch: the radii [C, N] are scanned once.
+ * row_floats, params, grads, ms, vs: HOST arrays of n_arrays entries (row sizes; device pointers to [N, row] arrays).
+ * Same update and same row selection as gs_adam_step with radii != NULL. */
+int gs_adam_step_visible(int64_t N, int32_t n_arrays, const int32_t* row_floats, float* const* params, const float* const* grads,
+                         float* const* ms, float* const* vs, float lr, float beta1, float beta2, float eps, int32_t step,
+                         const int32_t* radii, int32_t C, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, os.environ.get("GS_LIB_NAME", "libgsplat_b200.so"
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
-           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step"]
+           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
 
 
 class gs_camera(C.Structure):
@@ -297,3 +297,17 @@ def gs_adam_step(param, grad, m, v, lr, beta1, beta2, eps, step, radii=None, str
                             C.c_float(eps), C.c_int32(step), _ptr(radii, torch.int32) if radii is not None else None,
                             C.c_int32(Cv), _stream(stream))
     _check(rc, "gs_adam_step")
+
+
+def gs_adam_step_visible(params, grads, ms, vs, lr, beta1, beta2, eps, step, radii, stream=None):
+    """Visible-only Adam step over several [N, ...] float32 arrays (lists of tensors) in one launch."""
+    import torch
+    n = len(params)
+    N = params[0].shape[0]
+    rows = (C.c_int32 * n)(*[t.numel() // max(N, 1) for t in params])
+    def ptrs(ts):
+        return (C.c_void_p * n)(*[_ptr(t, torch.float32).value for t in ts])
+    rc = lib().gs_adam_step_visible(C.c_int64(N), C.c_int32(n), rows, ptrs(params), ptrs(grads), ptrs(ms), ptrs(vs), C.c_float(lr),
+                                    C.c_float(beta1), C.c_float(beta2), C.c_float(eps), C.c_int32(step), _ptr(radii, torch.int32),
+                                    C.c_int32(int(radii.shape[0])), _stream(stream))
+    _check(rc, "gs_adam_step_visible")

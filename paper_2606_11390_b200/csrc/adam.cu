@@ -64,9 +64,87 @@ __global__ void __launch_bounds__(256) adam_rows_kernel(const AdamArgs a) {
     }
 }
 
+// Visible-only step over up to 8 arrays at once: the radii are scanned ONCE (16-byte loads, 4 Gaussians per lane and view),
+// then the warp walks the visible Gaussians and, for each, the rows of all arrays with the lanes across the floats.
+constexpr int kAdamMaxArrays = 8;
+struct AdamMultiArgs {
+    int64_t N;
+    int32_t n_arrays, C, vec;
+    int32_t row[kAdamMaxArrays];
+    float* p[kAdamMaxArrays]; const float* g[kAdamMaxArrays]; float* m[kAdamMaxArrays]; float* v[kAdamMaxArrays];
+    float lr, b1, b2, eps, c1, c2;
+    const int32_t* radii;
+};
+
+__global__ void __launch_bounds__(256) adam_visible_multi_kernel(const AdamMultiArgs a) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    AdamArgs h;
+    h.lr = a.lr; h.b1 = a.b1; h.b2 = a.b2; h.eps = a.eps; h.c1 = a.c1; h.c2 = a.c2;
+    for (int64_t base = warp * 128; base < a.N; base += nwarps * 128) {
+        const int64_t i0 = base + 4 * lane;
+        unsigned int vis = 0;                       // bit k: Gaussian i0 + k is visible in some view
+        for (int c = 0; c < a.C; ++c) {
+            const int32_t* r = a.radii + (int64_t)c * a.N + i0;
+            if (a.vec && i0 + 4 <= a.N) {
+                const int4 q = __ldg(reinterpret_cast<const int4*>(r));
+                vis |= (q.x > 0 ? 1u : 0u) | (q.y > 0 ? 2u : 0u) | (q.z > 0 ? 4u : 0u) | (q.w > 0 ? 8u : 0u);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (i0 + k < a.N && __ldg(r + k) > 0) vis |= 1u << k;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            unsigned int mask = __ballot_sync(0xffffffffu, (vis >> k) & 1u);
+            while (mask) {
+                const int s = __ffs(mask) - 1;
+                mask &= mask - 1;
+                const int64_t i = base + 4 * s + k;
+                for (int q = 0; q < a.n_arrays; ++q) {
+                    const int64_t r0 = i * a.row[q];
+                    for (int e = lane; e < a.row[q]; e += 32) {
+                        float p = a.p[q][r0 + e], m = a.m[q][r0 + e], v = a.v[q][r0 + e];
+                        adam1(p, __ldg(a.g[q] + r0 + e), m, v, h);
+                        a.p[q][r0 + e] = p; a.m[q][r0 + e] = m; a.v[q][r0 + e] = v;
+                    }
+                }
+            }
+        }
+    }
+}
+
 }  // namespace gs
 
 using namespace gs;
+
+extern "C" int gs_adam_step_visible(int64_t N, int32_t n_arrays, const int32_t* row_floats, float* const* params, const float* const* grads,
+                                    float* const* ms, float* const* vs, float lr, float beta1, float beta2, float eps, int32_t step,
+                                    const int32_t* radii, int32_t C, void* stream) {
+    if (N < 0 || n_arrays < 1 || n_arrays > kAdamMaxArrays || step < 1 || !row_floats || !params || !grads || !ms || !vs) return GS_ERR_INVALID_ARGUMENT;
+    if (!(beta1 >= 0.0f && beta1 < 1.0f) || !(beta2 >= 0.0f && beta2 < 1.0f) || !finite_f(lr) || !(eps >= 0.0f)) return GS_ERR_INVALID_ARGUMENT;
+    if (!radii || C < 1 || C > GS_MAX_VIEWS) return GS_ERR_INVALID_ARGUMENT;
+    if (N == 0) return GS_OK;
+    AdamMultiArgs a;
+    a.N = N; a.n_arrays = n_arrays; a.C = C; a.radii = radii;
+    a.vec = (aligned(radii, 16) && (N % 4 == 0 || C == 1)) ? 1 : 0;
+    for (int q = 0; q < n_arrays; ++q) {
+        if (row_floats[q] < 1 || row_floats[q] > 4096 || !params[q] || !grads[q] || !ms[q] || !vs[q]) return GS_ERR_INVALID_ARGUMENT;
+        a.row[q] = row_floats[q]; a.p[q] = params[q]; a.g[q] = grads[q]; a.m[q] = ms[q]; a.v[q] = vs[q];
+    }
+    a.lr = lr; a.b1 = beta1; a.b2 = beta2; a.eps = eps;
+    a.c1 = (float)(1.0 / (1.0 - pow((double)beta1, (double)step)));
+    a.c2 = (float)(1.0 / (1.0 - pow((double)beta2, (double)step)));
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int64_t blocks = (N + 1023) / 1024;
+    if (blocks > (int64_t)sms * 8) blocks = (int64_t)sms * 8;
+    adam_visible_multi_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(a);
+    return launch_status();
+}
+
 
 extern "C" int gs_adam_step(int64_t N, int32_t row_floats, float* param, const float* grad, float* m, float* v, float lr, float beta1,
                             float beta2, float eps, int32_t step, const int32_t* radii, int32_t C, void* stream) {

@@ -130,6 +130,22 @@ class SplatStep:
                          self.radii, self.g_means2d, self.g_conics, self.g_opacities, self.g_rgbs, g["means"],
                          g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], accumulate)
 
+    def adam(self, mode="dense", lr=0.0, beta1=0.9, beta2=0.999, eps=1e-15):
+        """One fused Adam step over the five parameter arrays (gs_adam_step); ``mode`` "dense" or "sparse" (only Gaussians
+        visible in >= 1 view of the batch, from the saved radii)."""
+        if getattr(self, "_adam_m", None) is None:
+            self._adam_m = {k: torch.zeros_like(v) for k, v in self.params.items()}
+            self._adam_v = {k: torch.zeros_like(v) for k, v in self.params.items()}
+            self._adam_t = 0
+        self._adam_t += 1
+        if mode == "sparse":
+            ks = self.param_names
+            B.gs_adam_step_visible([self.params[k] for k in ks], [self.grads[k] for k in ks], [self._adam_m[k] for k in ks],
+                                   [self._adam_v[k] for k in ks], lr, beta1, beta2, eps, self._adam_t, self.radii)
+            return
+        for k in self.param_names:
+            B.gs_adam_step(self.params[k], self.grads[k], self._adam_m[k], self._adam_v[k], lr, beta1, beta2, eps, self._adam_t)
+
     # -- whole passes -------------------------------------------------------------------
     def forward(self, sync=True):
         self.project_fwd()

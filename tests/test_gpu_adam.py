@@ -77,3 +77,29 @@ def test_visible_only_rows(B, N, row, C, frac):
         assert np.array_equal(got[~vis], old[~vis])                        # untouched rows: bit-exact
         if vis.any():
             assert close(got[vis], r[vis], np.abs(r).max())
+
+
+@pytest.mark.parametrize("N,C,frac", [(4000, 4, 0.03), (10_001, 3, 0.3), (130, 1, 1.0), (5000, 2, 0.0)])
+def test_visible_only_multi_array_step(B, N, C, frac):
+    """gs_adam_step_visible: the five Gaussian arrays in one launch, radii scanned once; N not a multiple of 4 included."""
+    from oracle import adam_oracle as A
+    rng = np.random.default_rng(N * 7 + C)
+    rows = (3, 3, 4, 1, 48)
+    P = [rng.standard_normal((N, r)).astype(np.float32) for r in rows]
+    G = [rng.standard_normal((N, r)).astype(np.float32) for r in rows]
+    Ms = [rng.standard_normal((N, r)).astype(np.float32) for r in rows]
+    Vs = [np.abs(rng.standard_normal((N, r))).astype(np.float32) for r in rows]
+    radii = np.where(rng.random((C, N)) < frac, rng.integers(1, 50, (C, N)), 0).astype(np.int32)
+    vis = (radii > 0).any(axis=0)
+    hp = (f32(2e-3), f32(0.9), f32(0.999), f32(1e-15))
+    dev = lambda xs: [torch.from_numpy(x.copy()).cuda() for x in xs]
+    dP, dG, dM, dV = dev(P), dev(G), dev(Ms), dev(Vs)
+    B.gs_adam_step_visible(dP, dG, dM, dV, *hp, 4, torch.from_numpy(radii).cuda())
+    torch.cuda.synchronize()
+    for q in range(5):
+        ref = A.adam_step(P[q], G[q], Ms[q], Vs[q], *hp, 4, visible=vis)
+        for got, r, old in zip((dP[q], dM[q], dV[q]), ref, (P[q], Ms[q], Vs[q])):
+            got = got.cpu().numpy()
+            assert np.array_equal(got[~vis], old[~vis])
+            if vis.any():
+                assert close(got[vis], r[vis], np.abs(r).max())

@@ -49,6 +49,9 @@ def parse_args():
     ap.add_argument("--adam", default="none", choices=["none", "dense", "sparse"],
                     help="append the fused Adam step (SURVEY 8(f) NEXT-3) to the step, with lr = 0 so that the scene stays the same: "
                          "dense, or sparse = only Gaussians visible in the batch")
+    ap.add_argument("--sparse-grads", action="store_true",
+                    help="P5 writes only the rows of Gaussians visible in the batch (gs_project_bwd accumulate = 2) instead of the dense "
+                         "overwrite; goes with --adam sparse")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
@@ -313,7 +316,8 @@ def run_b200(args):
     STAGES = STAGES_ADAM if args.adam != "none" else globals()["STAGES"]
 
     def timed_step(ev):
-        calls = (st.project_fwd, lambda: st.bin_tiles(sync=False), st.raster_fwd, st.l1_loss, st.raster_bwd, st.project_bwd)
+        p5 = (lambda: st.project_bwd(accumulate=2)) if args.sparse_grads else st.project_bwd
+        calls = (st.project_fwd, lambda: st.bin_tiles(sync=False), st.raster_fwd, st.l1_loss, st.raster_bwd, p5)
         if args.adam != "none":
             calls = calls + (lambda: st.adam(args.adam),)
         ev[0].record(stream)
@@ -366,7 +370,7 @@ def run_b200(args):
         "project_fwd": 12 * N + (par_b - 12) * V_any + 48 * V_sum + 8 * N * C,
         # compaction (radii; uv, depth -> key, id) + depth sort (histogram, P_d passes) + entry table + tile sort + grid scans, ranges
         "bin_tiles": 4 * N * C + 24 * V_sum + (8 + 24 * P_d) * V_sum + (32 + 16) * V_sum + tsort_bytes + 24 * cells + 16 * C * st.gx * st.gy,
-        "project_bwd": 4 * N * C + 36 * V_sum + par_b * V_any + par_b * N,
+        "project_bwd": 4 * N * C + 36 * V_sum + par_b * V_any + par_b * (V_any if args.sparse_grads else N),
         # L1: read image, target, write dL; L1 + SSIM: + three derivative maps written and read, image and target read twice
         "l1_loss": (12 if args.loss == "l1" else 44) * C * W * H * 3,
         # flops (per evaluated (pixel, record) pair: DESIGN.md "algorithmic flops per pair")
@@ -437,7 +441,7 @@ def run_b200(args):
         "metric": METRIC, "value": value, "unit": "MP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": args.workload, "loss": args.loss, "morton": bool(args.morton), "adam": args.adam, "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
+        "config": {"workload": args.workload, "loss": args.loss, "morton": bool(args.morton), "adam": args.adam, "sparse_grads": bool(args.sparse_grads), "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
                    "intersections": M_now, "visible_entries": V_sum, "pairs_bwd": pairs_bwd,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},

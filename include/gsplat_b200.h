@@ -136,7 +136,9 @@ int gs_raster_bwd(const gs_config* cfg /*host*/, int32_t C, const gs_camera* cam
  * coefficients and view direction -> mean, opacity -> logit; summed over the C views.  Gradients
  * are with respect to the RAW parameters (reading A1).
  * accumulate == 0: every row of every output is overwritten (zeros for Gaussians visible nowhere);
- * accumulate != 0: rows of Gaussians visible in >= 1 view are added to, other rows untouched.
+ * accumulate == 1: rows of Gaussians visible in >= 1 view are added to, other rows untouched;
+ * accumulate == 2: rows of Gaussians visible in >= 1 view are OVERWRITTEN, other rows untouched (the visible-only
+ *                  gradient that goes with gs_adam_step_visible; C <= 16, else GS_ERR_UNSUPPORTED).
  * out: dL_dmeans[N,3] dL_dlog_scales[N,3] dL_dquats[N,4] dL_dopacity_logits[N] dL_dsh[N,K,3]. */
 int gs_project_bwd(const gs_config* cfg /*host*/, int64_t N, const float* means, const float* log_scales,
                    const float* quats, const float* opacity_logits, const float* sh, int32_t C,

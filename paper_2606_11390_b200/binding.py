@@ -210,7 +210,7 @@ def gs_project_bwd(cfg, means, log_scales, quats, opacity_logits, sh, cams, radi
                               _ptr(dL_drgbs, torch.float32), _ptr(dL_dmeans, torch.float32),
                               _ptr(dL_dlog_scales, torch.float32), _ptr(dL_dquats, torch.float32),
                               _ptr(dL_dopacity_logits, torch.float32), _ptr(dL_dsh, torch.float32),
-                              C.c_int32(1 if accumulate else 0), _stream(stream))
+                              C.c_int32(int(accumulate)), _stream(stream))
     _check(rc, "gs_project_bwd")
 
 

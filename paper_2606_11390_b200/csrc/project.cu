@@ -690,6 +690,8 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
     if (!aligned(quats, 16) || !aligned(sh, 16) || !aligned(dL_dquats, 16) || !aligned(dL_dsh, 16) || !aligned(dL_dmeans2d, 8))
         return GS_ERR_INVALID_ARGUMENT;
     if ((int64_t)C * N >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
+    if (accumulate < 0 || accumulate > 2) return GS_ERR_INVALID_ARGUMENT;
+    if (accumulate == 2 && C > kMaxCamsPerLaunch) return GS_ERR_UNSUPPORTED;   // one launch must see every view of the batch
     cudaStream_t st = (cudaStream_t)stream;
     for (int c0 = 0; c0 < C; c0 += kMaxCamsPerLaunch) {
         const int nc = C - c0 < kMaxCamsPerLaunch ? C - c0 : kMaxCamsPerLaunch;
@@ -706,12 +708,14 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
         a.d_logits = dL_dopacity_logits; a.d_sh = dL_dsh;
         a.dilation = cfg->dilation;
         // the first chunk of cameras overwrites (unless the caller accumulates), later chunks add
-        a.accumulate = (accumulate != 0 || c0 > 0) ? 1 : 0;
+        // accumulate == 2 ("visible rows only"): the rows of Gaussians visible in this batch are overwritten, all other rows
+        // are left untouched (no dense zero-fill: the caller's optimizer reads only visible rows, gs_adam_step_visible)
+        a.accumulate = (accumulate == 1 || c0 > 0) ? 1 : 0;
         a.vec_in = (aligned(a.radii, 16) && (N % 4 == 0 || nc == 1)) ? 1 : 0;
         a.vec_out = (aligned(dL_dmeans, 16) && aligned(dL_dlog_scales, 16) && aligned(dL_dquats, 16) &&
                      aligned(dL_dopacity_logits, 16) && aligned(dL_dsh, 16)) ? 1 : 0;
-        a.prezeroed = 0;
-        if (!a.accumulate && a.vec_out && N >= kZeroFillMinN) {
+        a.prezeroed = (accumulate == 2) ? 1 : 0;
+        if (!a.accumulate && accumulate != 2 && a.vec_out && N >= kZeroFillMinN) {
             const int64_t K3 = 3 * (int64_t)(cfg->sh_degree + 1) * (cfg->sh_degree + 1);
             float* ptrs[5] = {dL_dsh, dL_dquats, dL_dmeans, dL_dlog_scales, dL_dopacity_logits};
             const int64_t counts[5] = {K3 * N, 4 * N, 3 * N, 3 * N, N};

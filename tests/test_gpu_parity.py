@@ -469,3 +469,24 @@ def test_step_from_host_equals_resident_step(B):
     assert abs(float(host_loss.item()) - float(ref.loss.item())) <= 1e-6
     for k in st.param_names:
         assert rel_l2(st.grads[k].cpu().numpy(), ref.grads[k].cpu().numpy()) <= 1e-5, k
+
+
+@pytest.mark.parametrize("name,sc", SCENES[1:], ids=[s[0] for s in SCENES[1:]])
+def test_project_bwd_visible_rows_only(B, name, sc):
+    """accumulate = 2: rows of Gaussians visible in the batch equal the dense overwrite bit for bit, all other rows keep
+    their previous contents (a sentinel here)."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    st = SplatStep(sc)
+    st.set_target(scenes.target_image(sc))
+    st.step(sync=True)
+    torch.cuda.synchronize()
+    dense = {k: v.clone() for k, v in st.grads.items()}
+    for v in st.grads.values():
+        v.fill_(123.0)
+    st.project_bwd(accumulate=2)
+    torch.cuda.synchronize()
+    vis = (st.radii > 0).any(dim=0)
+    assert 0 < int(vis.sum()) < st.N
+    for k, v in st.grads.items():
+        assert torch.equal(v[vis], dense[k][vis]), k
+        assert bool((v[~vis] == 123.0).all()), k

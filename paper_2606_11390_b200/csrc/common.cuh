@@ -108,6 +108,30 @@ __device__ __forceinline__ void tile_rect(float u, float v, int radius, int gx, 
     y1 = clampi(floor_to_int_sat(__fmul_rn(__fadd_rn(v, r_hi), inv)), 0, gy);
 }
 
+// Two-wide FP32 (sm_100a FFMA2 / FMUL2 / FADD2; PTX fma/mul/add.rn.f32x2 on 64-bit register pairs): one issue slot for two
+// lanes of arithmetic.  Used by the issue-bound raster and SSIM kernels.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
 // Real spherical-harmonic constants, degrees 0..3 (closed forms evaluated in double, rounded once).
 constexpr float kC0 = 0.28209479177387814f;   // 1/(2 sqrt(pi))
 constexpr float kC1 = 0.4886025119029199f;    // sqrt(3/(4 pi))

@@ -111,29 +111,34 @@ __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
     // horizontal pass
     for (int task = threadIdx.x; task < kSsimHalo * 3 * (kSsimTile / kSsimRun); task += 256) {
         const int r = task / 12, rem = task - r * 12, cg = rem / 3, ch = rem - cg * 3;
-        float acc[kSsimRun][5];
+        // (x, y) and (x^2, y^2) travel as two-wide pairs: three instructions per tap and output instead of five
+        f32x2 accA[kSsimRun], accB[kSsimRun];
+        float accC[kSsimRun];
 #pragma unroll
-        for (int o = 0; o < kSsimRun; ++o)
-#pragma unroll
-            for (int q = 0; q < 5; ++q) acc[o][q] = 0.0f;
+        for (int o = 0; o < kSsimRun; ++o) { accA[o] = pk2(0.f, 0.f); accB[o] = accA[o]; accC[o] = 0.0f; }
 #pragma unroll
         for (int p = 0; p < kSsimIn; ++p) {
             const float xv = sx[r][(kSsimRun * cg + p) * 3 + ch], yv = sy[r][(kSsimRun * cg + p) * 3 + ch];
-            const float xx = xv * xv, yy = yv * yv, xy = xv * yv;
+            const f32x2 X = pk2(xv, yv);
+            const f32x2 P = mul2(X, X);
+            const float xy = xv * yv;
 #pragma unroll
             for (int o = 0; o < kSsimRun; ++o) {
                 const int t = p - o;
                 if (t >= 0 && t < kSsimWin) {
                     const float w = a.win[t];
-                    acc[o][0] = fmaf(w, xv, acc[o][0]); acc[o][1] = fmaf(w, yv, acc[o][1]);
-                    acc[o][2] = fmaf(w, xx, acc[o][2]); acc[o][3] = fmaf(w, yy, acc[o][3]); acc[o][4] = fmaf(w, xy, acc[o][4]);
+                    const f32x2 W2 = pk2(w, w);
+                    accA[o] = fma2(W2, X, accA[o]); accB[o] = fma2(W2, P, accB[o]); accC[o] = fmaf(w, xy, accC[o]);
                 }
             }
         }
 #pragma unroll
-        for (int o = 0; o < kSsimRun; ++o)
-#pragma unroll
-            for (int q = 0; q < 5; ++q) hz.at(ch, q, r, kSsimRun * cg + o) = acc[o][q];
+        for (int o = 0; o < kSsimRun; ++o) {
+            float m1, m2, e11, e22;
+            unpk2(accA[o], m1, m2); unpk2(accB[o], e11, e22);
+            const int c = kSsimRun * cg + o;
+            hz.at(ch, 0, r, c) = m1; hz.at(ch, 1, r, c) = m2; hz.at(ch, 2, r, c) = e11; hz.at(ch, 3, r, c) = e22; hz.at(ch, 4, r, c) = accC[o];
+        }
     }
     __syncthreads();
     // vertical pass, SSIM and its derivatives
@@ -141,25 +146,31 @@ __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
     float ssim_sum = 0.0f, l1_sum = 0.0f;
     if (threadIdx.x < 3 * kSsimTile * (kSsimTile / kSsimRun)) {
         const int ch = threadIdx.x % 3, col = (threadIdx.x / 3) % kSsimTile, g = threadIdx.x / (3 * kSsimTile);
-        float acc[kSsimRun][5];
+        f32x2 accA[kSsimRun], accB[kSsimRun];
+        float accC[kSsimRun];
 #pragma unroll
-        for (int o = 0; o < kSsimRun; ++o)
-#pragma unroll
-            for (int q = 0; q < 5; ++q) acc[o][q] = 0.0f;
+        for (int o = 0; o < kSsimRun; ++o) { accA[o] = pk2(0.f, 0.f); accB[o] = accA[o]; accC[o] = 0.0f; }
 #pragma unroll
         for (int p = 0; p < kSsimIn; ++p) {
             float in[5];
 #pragma unroll
             for (int q = 0; q < 5; ++q) in[q] = hz.at(ch, q, kSsimRun * g + p, col);
+            const f32x2 A2 = pk2(in[0], in[1]), B2 = pk2(in[2], in[3]);
 #pragma unroll
             for (int o = 0; o < kSsimRun; ++o) {
                 const int t = p - o;
                 if (t >= 0 && t < kSsimWin) {
                     const float w = a.win[t];
-#pragma unroll
-                    for (int q = 0; q < 5; ++q) acc[o][q] = fmaf(w, in[q], acc[o][q]);
+                    const f32x2 W2 = pk2(w, w);
+                    accA[o] = fma2(W2, A2, accA[o]); accB[o] = fma2(W2, B2, accB[o]); accC[o] = fmaf(w, in[4], accC[o]);
                 }
             }
+        }
+        float acc[kSsimRun][5];
+#pragma unroll
+        for (int o = 0; o < kSsimRun; ++o) {
+            unpk2(accA[o], acc[o][0], acc[o][1]); unpk2(accB[o], acc[o][2], acc[o][3]);
+            acc[o][4] = accC[o];
         }
         const int gj = j0 + col;
 #pragma unroll
@@ -214,50 +225,58 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
     halo_wait();
     for (int task = threadIdx.x; task < kSsimHalo * 3 * (kSsimTile / kSsimRun); task += 256) {
         const int r = task / 12, rem = task - r * 12, cg = rem / 3, ch = rem - cg * 3;
-        float acc[kSsimRun][3];
+        f32x2 accA[kSsimRun];
+        float accC[kSsimRun];
 #pragma unroll
-        for (int o = 0; o < kSsimRun; ++o) acc[o][0] = acc[o][1] = acc[o][2] = 0.0f;
+        for (int o = 0; o < kSsimRun; ++o) { accA[o] = pk2(0.f, 0.f); accC[o] = 0.0f; }
 #pragma unroll
         for (int p = 0; p < kSsimIn; ++p) {
             float in[3];
 #pragma unroll
             for (int q = 0; q < 3; ++q) in[q] = sm[q][r][(kSsimRun * cg + p) * 3 + ch];
+            const f32x2 A2 = pk2(in[0], in[1]);
 #pragma unroll
             for (int o = 0; o < kSsimRun; ++o) {
                 const int t = p - o;
                 if (t >= 0 && t < kSsimWin) {
                     const float w = a.win[t];
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) acc[o][q] = fmaf(w, in[q], acc[o][q]);
+                    accA[o] = fma2(pk2(w, w), A2, accA[o]); accC[o] = fmaf(w, in[2], accC[o]);
                 }
             }
         }
 #pragma unroll
-        for (int o = 0; o < kSsimRun; ++o)
-#pragma unroll
-            for (int q = 0; q < 3; ++q) hz.at(ch, q, r, kSsimRun * cg + o) = acc[o][q];
+        for (int o = 0; o < kSsimRun; ++o) {
+            float g0, g1;
+            unpk2(accA[o], g0, g1);
+            const int c = kSsimRun * cg + o;
+            hz.at(ch, 0, r, c) = g0; hz.at(ch, 1, r, c) = g1; hz.at(ch, 2, r, c) = accC[o];
+        }
     }
     __syncthreads();
     if (vtask) {
         const int ch = vch, col = vcol, g = vg;
-        float acc[kSsimRun][3];
+        f32x2 accA[kSsimRun];
+        float accC[kSsimRun];
 #pragma unroll
-        for (int o = 0; o < kSsimRun; ++o) acc[o][0] = acc[o][1] = acc[o][2] = 0.0f;
+        for (int o = 0; o < kSsimRun; ++o) { accA[o] = pk2(0.f, 0.f); accC[o] = 0.0f; }
 #pragma unroll
         for (int p = 0; p < kSsimIn; ++p) {
             float in[3];
 #pragma unroll
             for (int q = 0; q < 3; ++q) in[q] = hz.at(ch, q, kSsimRun * g + p, col);
+            const f32x2 A2 = pk2(in[0], in[1]);
 #pragma unroll
             for (int o = 0; o < kSsimRun; ++o) {
                 const int t = p - o;
                 if (t >= 0 && t < kSsimWin) {
                     const float w = a.win[t];
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) acc[o][q] = fmaf(w, in[q], acc[o][q]);
+                    accA[o] = fma2(pk2(w, w), A2, accA[o]); accC[o] = fmaf(w, in[2], accC[o]);
                 }
             }
         }
+        float acc[kSsimRun][3];
+#pragma unroll
+        for (int o = 0; o < kSsimRun; ++o) { unpk2(accA[o], acc[o][0], acc[o][1]); acc[o][2] = accC[o]; }
         const float l1w = (1.0f - a.lambda) * a.inv_n;
         const int gj = j0 + col;
 #pragma unroll

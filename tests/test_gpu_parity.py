@@ -56,6 +56,16 @@ def small_scenes():
                      for e in [(2.5, 1.6, 2.5), (7.5, 1.6, 7.5)]]
     sc["bg"] = np.array([0.1, 0.3, 0.2], np.float32)
     out.append(("room-small", sc))
+    # SH degrees 1 and 2 (the kernels are instantiated per degree): the object scene with truncated coefficients
+    for deg in (1, 2):
+        sc = scenes.make_scene("object", n=6_007)
+        sc["cameras"] = [scenes.make_camera(320, 180, 250.0, 250.0, np.asarray(c["viewmat"])[:, :3].T @ -np.asarray(c["viewmat"])[:, 3],
+                                            (0, 0, 0), (0, -1, 0)) for c in sc["cameras"][:2]]
+        sc["log_scales"] = sc["log_scales"] + 0.4
+        sc["sh"] = np.ascontiguousarray(sc["sh"][:, : (deg + 1) ** 2, :])
+        sc["sh"][:, 1:, :] *= 4.0                                      # make the view-dependent part matter
+        sc["sh_degree"] = deg
+        out.append((f"object-deg{deg}", sc))
     return out
 
 

@@ -253,8 +253,7 @@ def whole_job_rate(world, units_per_rank_per_step, ms_per_step):
 
 
 # ----------------------------------------------------------------------------- B200 leg
-STAGES = ("project_fwd", "bin_tiles", "raster_fwd", "l1_loss", "raster_bwd", "project_bwd")
-STAGES_ADAM = STAGES + ("adam",)
+BASE_STAGES = ("project_fwd", "bin_tiles", "raster_fwd", "l1_loss", "raster_bwd", "project_bwd")
 
 
 def run_b200(args):
@@ -313,7 +312,7 @@ def run_b200(args):
 
     stream = torch.cuda.current_stream()
 
-    STAGES = STAGES_ADAM if args.adam != "none" else globals()["STAGES"]
+    STAGES = BASE_STAGES + (("adam",) if args.adam != "none" else ())
 
     def timed_step(ev):
         p5 = (lambda: st.project_bwd(accumulate=2)) if args.sparse_grads else st.project_bwd

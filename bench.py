@@ -326,6 +326,10 @@ def run_b200(args):
 
     for _ in range(max(args.warmup, 3)):
         st.step(sync=False)
+        if args.adam != "none":
+            st.adam(args.adam)            # (also allocates the moments outside the timed region)
+        if args.sparse_grads:
+            st.project_bwd(accumulate=2)
     barrier()
 
     sampler = ClockSampler(local_rank)

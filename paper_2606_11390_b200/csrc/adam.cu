@@ -71,6 +71,8 @@ struct AdamMultiArgs {
     int64_t N;
     int32_t n_arrays, C, vec;
     int32_t row[kAdamMaxArrays];
+    int32_t start[kAdamMaxArrays];      // first element of array q in the concatenated row
+    int32_t total_row;
     float* p[kAdamMaxArrays]; const float* g[kAdamMaxArrays]; float* m[kAdamMaxArrays]; float* v[kAdamMaxArrays];
     float lr, b1, b2, eps, c1, c2;
     const int32_t* radii;
@@ -102,13 +104,16 @@ __global__ void __launch_bounds__(256) adam_visible_multi_kernel(const AdamMulti
                 const int s = __ffs(mask) - 1;
                 mask &= mask - 1;
                 const int64_t i = base + 4 * s + k;
-                for (int q = 0; q < a.n_arrays; ++q) {
-                    const int64_t r0 = i * a.row[q];
-                    for (int e = lane; e < a.row[q]; e += 32) {
-                        float p = a.p[q][r0 + e], m = a.m[q][r0 + e], v = a.v[q][r0 + e];
-                        adam1(p, __ldg(a.g[q] + r0 + e), m, v, h);
-                        a.p[q][r0 + e] = p; a.m[q][r0 + e] = m; a.v[q][r0 + e] = v;
-                    }
+                // the lanes run over the concatenation of the Gaussian's rows in all arrays (59 floats for the five
+                // parameter arrays at SH degree 3): every load of a Gaussian is issued before the first use
+                for (int e = lane; e < a.total_row; e += 32) {
+                    int q = 0;
+#pragma unroll
+                    for (int j = 1; j < kAdamMaxArrays; ++j) q += (j < a.n_arrays && e >= a.start[j]) ? 1 : 0;
+                    const int64_t o = i * a.row[q] + (e - a.start[q]);
+                    float p = a.p[q][o], m = a.m[q][o], v = a.v[q][o];
+                    adam1(p, __ldg(a.g[q] + o), m, v, h);
+                    a.p[q][o] = p; a.m[q][o] = m; a.v[q][o] = v;
                 }
             }
         }
@@ -129,9 +134,13 @@ extern "C" int gs_adam_step_visible(int64_t N, int32_t n_arrays, const int32_t* 
     AdamMultiArgs a;
     a.N = N; a.n_arrays = n_arrays; a.C = C; a.radii = radii;
     a.vec = (aligned(radii, 16) && (N % 4 == 0 || C == 1)) ? 1 : 0;
+    a.total_row = 0;
+    for (int q = 0; q < kAdamMaxArrays; ++q) { a.row[q] = 1; a.start[q] = 0; a.p[q] = nullptr; a.g[q] = nullptr; a.m[q] = nullptr; a.v[q] = nullptr; }
     for (int q = 0; q < n_arrays; ++q) {
         if (row_floats[q] < 1 || row_floats[q] > 4096 || !params[q] || !grads[q] || !ms[q] || !vs[q]) return GS_ERR_INVALID_ARGUMENT;
         a.row[q] = row_floats[q]; a.p[q] = params[q]; a.g[q] = grads[q]; a.m[q] = ms[q]; a.v[q] = vs[q];
+        a.start[q] = a.total_row;
+        a.total_row += row_floats[q];
     }
     a.lr = lr; a.b1 = beta1; a.b2 = beta2; a.eps = eps;
     a.c1 = (float)(1.0 / (1.0 - pow((double)beta1, (double)step)));

@@ -1,16 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- forward+backward splatting throughput on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload object|room|block|city|tiny]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload city|block|room|object|tiny]
     python bench.py --impl reference ...      # the CPU oracle timed on the host cores
 
 A "step" is one pass of the whole hot path over one batch of synthetic views:
 gs_project_fwd -> gs_bin_tiles -> gs_raster_fwd -> gs_l1_loss -> gs_raster_bwd -> gs_project_bwd.
-`value` = megapixels/s (C*W*H per step / device time) with inputs resident in HBM; `e2e` = the same
-with the step's inputs (parameters + target images) copied from pinned host memory and the loss read
-back inside the timed region.  One JSON line is printed by rank 0.
+`value` = megapixels/s (C*W*H per step / median device time of a step, the paper's protocol PAPER.md:100: 20 iterations
+after 10 warm-up) with inputs resident in HBM; `e2e` = the same with the step's inputs (parameters + target images)
+copied from pinned host memory and the loss read back inside the timed region.  One JSON line is printed by rank 0.
 
-Multi-GPU: the path is "replicas only" (SURVEY.md §8(e), north_star: no sharding, no collectives):
+The default workload is `city` (60 M Gaussians, four 4K views): BASELINE.json's metric is not quoted on one config, so
+the N = 1 line is on the largest single-GPU one; `per_config` carries the short runs of the other configs.
+
+Multi-GPU: the path is "replicas only" (SURVEY.md 8(e), north_star: no sharding, no collectives):
 every rank runs the same workload on its own GPU; value = total pixels of all ranks / max time.
 """
 from __future__ import annotations
@@ -31,15 +34,20 @@ if ROOT not in sys.path:
 
 METRIC = "fwd+bwd megapixels/s"
 FP32_LANES_PER_SM = 128
+HBM_NOMINAL_GBS = 8000.0      # north_star: "achieved HBM GB/s against ~8 TB/s"
+# flop per (pixel, record) pair, itemised in DESIGN.md section 6 from O-R1 / O-R2
+FWD_FLOP_COMPOSITED, FWD_FLOP_REJECTED = 22, 11
+BWD_FLOP_COMPOSITED, BWD_FLOP_REJECTED = 60, 13
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="object", choices=["tiny", "object", "room", "block", "city"])
+    ap.add_argument("--workload", default="city", choices=["tiny", "object", "room", "block", "city"])
+    ap.add_argument("--far-inf", action="store_true", help="city without a far plane (SURVEY 8(c) A4 stress variant)")
     ap.add_argument("--n", type=int, default=None, help="override the Gaussian count (debugging only)")
     ap.add_argument("--loss", default="l1", choices=["l1", "l1ssim"],
                     help="loss of the step: mean L1 (BASELINE.json configs, default) or the fused 0.8 L1 + 0.2 (1 - SSIM) (SURVEY 8(f) NEXT-1)")
@@ -48,14 +56,18 @@ def parse_args():
                          "one-time preprocessing, its device time is reported as morton_sort_ms, not part of a step)")
     ap.add_argument("--adam", default="none", choices=["none", "dense", "sparse"],
                     help="append the fused Adam step (SURVEY 8(f) NEXT-3) to the step, with lr = 0 so that the scene stays the same: "
-                         "dense, or sparse = only Gaussians visible in the batch")
+                         "dense (the paper's fused Adam), or sparse = only Gaussians visible in the batch (a semantic variant, reading A28)")
     ap.add_argument("--sparse-grads", action="store_true",
                     help="P5 writes only the rows of Gaussians visible in the batch (gs_project_bwd accumulate = 2) instead of the dense "
-                         "overwrite; goes with --adam sparse")
+                         "overwrite; only valid with --adam sparse or none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE configs")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
-    return ap.parse_args()
+    args = ap.parse_args()
+    if args.sparse_grads and args.adam == "dense":
+        ap.error("--sparse-grads leaves stale rows for invisible Gaussians; the dense Adam step reads every row (use --adam sparse)")
+    return args
 
 
 # ----------------------------------------------------------------------------- peaks
@@ -83,6 +95,18 @@ def load_traffic(workload, kernel):
     return None
 
 
+def cpu_info():
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"nproc": os.cpu_count(), "cpu_model": model}
+
+
 # ----------------------------------------------------------------------------- clocks
 class ClockSampler:
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -97,7 +121,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -135,102 +159,141 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- CPU oracle leg
-def oracle_sample(workload, n_override, target_seconds):
-    """Time the oracle (float instantiation, single thread, as it stands) on a bounded sample of the
-    workload: view by view (view 0 first, further views while the time budget allows); for each view the
-    per-Gaussian stages and the binning on all N Gaussians; the per-pixel stages on every k-th tile (k
-    chosen from a pilot so that one view takes at most about target_seconds), scaled by k to a full view.
-    Returns MP/s for one full view (mean over the sampled views)."""
-    from oracle import gs_oracle as O
-    from paper_2606_11390_b200 import scenes
-    O.lib()
-    sc = scenes.make_scene(workload, n=n_override)
-    cfg = O.make_cfg(sh_degree=sc["sh_degree"])
-    f32 = np.float32
-    W, H = sc["cameras"][0]["width"], sc["cameras"][0]["height"]
-    gx, gy = O.grid(cfg, sc["cameras"][0])
-    tiles = gx * gy
-    rng = np.random.Generator(np.random.PCG64(123))
-    tgt = rng.random((1, H, W, 3), dtype=f32)
-    t_sum = {"project_fwd": 0.0, "bin_tiles": 0.0, "raster_fwd": 0.0, "raster_bwd": 0.0, "project_bwd": 0.0}
-    full_view_s, k, n_tiles_used, cpu_s, views = [], None, 0, 0.0, 0
-    for v in range(len(sc["cameras"])):
-        if v > 0 and cpu_s + cpu_s / v > target_seconds:
-            break
-        cams = sc["cameras"][v:v + 1]
-        t = {}
+class OracleSampler:
+    """The oracle (float instantiation, single thread, as it stands) on bounded samples of one workload.
+
+    Setup (once, untimed, like building the scene): the oracle's P1 and binning of view 0 on all Gaussians, which the
+    per-pixel stages need as input.  One timed sample = one pass of the five stages over view 0 restricted to
+      * a contiguous slice of N / kg Gaussians for the per-Gaussian stages P1 and P5 (the scene generators draw Gaussians
+        i.i.d. over the index, so a slice is a random sample),
+      * all Gaussians for the binning,
+      * every kt-th tile for the per-pixel stages R1 and R2,
+    with kg and kt chosen from a pilot so that one sample takes about `seconds`.  The full-view time is extrapolated as
+    kg (t_P1 + t_P5) + t_bin + kt (t_R1 + t_R2); MP/s = W H / that."""
+
+    def __init__(self, workload, n_override, seconds, far_inf=False):
+        from oracle import gs_oracle as O
+        from paper_2606_11390_b200 import scenes
+        self.O = O
+        O.lib()
+        kw = {"far": 3.0e38} if (far_inf and workload == "city") else {}
+        self.sc = sc = scenes.make_scene(workload, n=n_override, **kw)
+        self.workload = workload
+        self.cfg = cfg = O.make_cfg(sh_degree=sc["sh_degree"])
+        self.f32 = f32 = np.float32
+        self.cams = cams = sc["cameras"][:1]
+        self.W, self.H = cams[0]["width"], cams[0]["height"]
+        self.N = N = sc["means"].shape[0]
+        gx, gy = O.grid(cfg, cams[0])
+        self.tiles = gx * gy
+        rng = np.random.Generator(np.random.PCG64(123))
+        self.tgt = rng.random((1, self.H, self.W, 3), dtype=f32)
+        # ---- setup: full-view P1 + binning (input of the per-pixel stages)
         t0 = time.perf_counter()
-        pf = O.project_fwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], cams, f32)
+        self.pf = pf = O.project_fwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], cams, f32)
+        t_p1_full = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        self.keys, self.vals, self.ranges = O.bin_tiles(cfg, cams, pf["means2d"], pf["depths"], pf["radii"])
+        t_bin = time.perf_counter() - t0
+        lens = self.ranges[:, 1] - self.ranges[:, 0]
+        # ---- pilot on a few tiles -> kt; per-Gaussian slice -> kg
+        pilot = np.zeros(self.tiles, np.uint8)
+        pilot[:: max(1, self.tiles // 16)] = 1
+        t0 = time.perf_counter()
+        O.raster_fwd(cfg, cams, self.vals, self.ranges, pf["means2d"], pf["conics"], pf["opacities"], pf["rgbs"], sc["bg"], f32, tile_mask=pilot)
+        tp = max(time.perf_counter() - t0, 1e-4)
+        per_rec = tp / max(int(lens[pilot > 0].sum()), 1)
+        est_raster = per_rec * max(int(lens.sum()), 1) * 2.2                 # forward + backward, all tiles
+        est_gauss = t_p1_full * 3.0                                          # P1 + P5 (P5 is about twice P1), all Gaussians
+        budget = max(seconds - t_bin, 0.5)
+        self.kt = int(max(1, np.ceil(est_raster / (0.6 * budget))))
+        self.kg = int(max(1, np.ceil(est_gauss / (0.4 * budget))))
+        self.mask = np.zeros(self.tiles, np.uint8)
+        self.mask[:: self.kt] = 1
+        self.n_slice = max(1, N // self.kg)
+        self.setup_seconds = {"project_fwd_full_view": round(t_p1_full, 3), "bin_tiles_full_view": round(t_bin, 3)}
+
+    def sample(self, k=0):
+        """One timed sample; the Gaussian slice rotates with k.  Returns (wall seconds of the sample, stage seconds,
+        extrapolated full-view seconds)."""
+        O, sc, cfg, cams, f32, pf = self.O, self.sc, self.cfg, self.cams, self.f32, self.pf
+        n_sl = self.n_slice
+        s0 = (k * n_sl) % max(self.N - n_sl + 1, 1)
+        sl = slice(s0, s0 + n_sl)
+        t = {}
+        w0 = time.perf_counter()
+        t0 = time.perf_counter()
+        O.project_fwd(cfg, sc["means"][sl], sc["log_scales"][sl], sc["quats"][sl], sc["opacity_logits"][sl], sc["sh"][sl], cams, f32)
         t["project_fwd"] = time.perf_counter() - t0
         t0 = time.perf_counter()
-        keys, vals, ranges = O.bin_tiles(cfg, cams, pf["means2d"], pf["depths"], pf["radii"])
+        O.bin_tiles(cfg, cams, pf["means2d"], pf["depths"], pf["radii"])
         t["bin_tiles"] = time.perf_counter() - t0
-        lens = ranges[:, 1] - ranges[:, 0]
-        if k is None:
-            # pilot on a few tiles to size the sample
-            pilot = np.zeros(tiles, np.uint8)
-            pilot[:: max(1, tiles // 16)] = 1
-            t0 = time.perf_counter()
-            O.raster_fwd(cfg, cams, vals, ranges, pf["means2d"], pf["conics"], pf["opacities"], pf["rgbs"], sc["bg"], f32, tile_mask=pilot)
-            tp = max(time.perf_counter() - t0, 1e-4)
-            cpu_s += tp
-            per_rec = tp / max(int(lens[pilot > 0].sum()), 1)
-            budget = max(target_seconds - t["project_fwd"] * 2 - t["bin_tiles"], 2.0)
-            est_full = per_rec * max(int(lens.sum()), 1) * 2.2          # forward + backward
-            k = int(max(1, np.ceil(est_full / budget)))
-        mask = np.zeros(tiles, np.uint8)
-        mask[::k] = 1
         t0 = time.perf_counter()
-        img, T, nc = O.raster_fwd(cfg, cams, vals, ranges, pf["means2d"], pf["conics"], pf["opacities"], pf["rgbs"], sc["bg"], f32, tile_mask=mask)
-        t["raster_fwd"] = (time.perf_counter() - t0)
-        dL = (np.sign(img - tgt) / img.size).astype(f32)
+        img, T, nc = O.raster_fwd(cfg, cams, self.vals, self.ranges, pf["means2d"], pf["conics"], pf["opacities"], pf["rgbs"], sc["bg"], f32,
+                                  tile_mask=self.mask)
+        t["raster_fwd"] = time.perf_counter() - t0
+        dL = (np.sign(img - self.tgt) / img.size).astype(f32)
         t0 = time.perf_counter()
-        g2 = O.raster_bwd(cfg, cams, vals, ranges, pf["means2d"], pf["conics"], pf["opacities"], pf["rgbs"], sc["bg"], T, nc, dL, f32, tile_mask=mask)
-        t["raster_bwd"] = (time.perf_counter() - t0)
+        g2 = O.raster_bwd(cfg, cams, self.vals, self.ranges, pf["means2d"], pf["conics"], pf["opacities"], pf["rgbs"], sc["bg"], T, nc, dL, f32,
+                          tile_mask=self.mask)
+        t["raster_bwd"] = time.perf_counter() - t0
         t0 = time.perf_counter()
-        O.project_bwd(cfg, sc["means"], sc["log_scales"], sc["quats"], sc["opacity_logits"], sc["sh"], cams, pf["radii"],
-                      g2["means2d"], g2["conics"], g2["opacities"], g2["rgbs"], f32)
+        O.project_bwd(cfg, sc["means"][sl], sc["log_scales"][sl], sc["quats"][sl], sc["opacity_logits"][sl], sc["sh"][sl], cams,
+                      np.ascontiguousarray(pf["radii"][:, sl]), np.ascontiguousarray(g2["means2d"][:, sl]), np.ascontiguousarray(g2["conics"][:, sl]),
+                      np.ascontiguousarray(g2["opacities"][:, sl]), np.ascontiguousarray(g2["rgbs"][:, sl]), f32)
         t["project_bwd"] = time.perf_counter() - t0
-        frac = float(mask.sum()) / tiles
-        full_view_s.append(t["project_fwd"] + t["bin_tiles"] + (t["raster_fwd"] + t["raster_bwd"]) / frac + t["project_bwd"])
-        for k2, val in t.items():
-            t_sum[k2] += val
-        cpu_s += sum(t.values())
-        n_tiles_used = int(mask.sum())
-        views += 1
-    full_view = float(np.mean(full_view_s))
-    mpix = W * H / 1e6
-    return {
-        "value": mpix / full_view, "unit": "MP/s", "cores": 1, "kind": "oracle",
-        "sample": (f"oracle<float>, 1 thread: {views} view(s) of '{workload}' (N={sc['means'].shape[0]}), one at a time; project fwd/bwd "
-                   f"and binning on all Gaussians, raster fwd+bwd on every {k}-th tile ({n_tiles_used} of {tiles}) scaled by {k}; "
-                   f"measured {cpu_s:.1f} s of CPU work"),
-        "stage_seconds": {k2: round(v2, 4) for k2, v2 in t_sum.items()},
-        "gaussians_per_s": sc["means"].shape[0] / full_view,
-        "step_mpix": len(sc["cameras"]) * mpix,
-    }
+        wall = time.perf_counter() - w0
+        frac_t = float(self.mask.sum()) / self.tiles
+        scale_g = self.N / n_sl
+        full = scale_g * (t["project_fwd"] + t["project_bwd"]) + t["bin_tiles"] + (t["raster_fwd"] + t["raster_bwd"]) / frac_t
+        return wall, t, full
+
+    def describe(self, n_samples, cpu_s):
+        return (f"oracle<float>, 1 thread, view 0 of '{self.workload}' (N={self.N}), {n_samples} sample(s): P1 and P5 on a slice of "
+                f"{self.n_slice} Gaussians (scaled by {self.N / self.n_slice:.1f}), binning on all Gaussians, raster fwd+bwd on every "
+                f"{self.kt}-th tile ({int(self.mask.sum())} of {self.tiles}, scaled by {self.tiles / float(self.mask.sum()):.1f}); "
+                f"{cpu_s:.1f} s of timed CPU work; untimed setup = the oracle's full-view P1 + binning")
+
+
+def oracle_baseline(workload, n_override, seconds, far_inf=False):
+    smp = OracleSampler(workload, n_override, seconds, far_inf)
+    wall, t, full = smp.sample(0)
+    mpix = smp.W * smp.H / 1e6
+    out = {"value": mpix / full, "unit": "MP/s", "cores": 1, "kind": "oracle", "sample": smp.describe(1, wall),
+           "stage_seconds": {k: round(v, 4) for k, v in t.items()}, "setup_seconds": smp.setup_seconds,
+           "gaussians_per_s": smp.N / full, "full_view_seconds_extrapolated": round(full, 3), "sample_seconds": round(wall, 3)}
+    out.update(cpu_info())
+    return out
 
 
 def run_reference(args):
-    """--impl reference: the oracle as it stands, on rank 0 only."""
+    """--impl reference: the oracle as it stands, on rank 0 only.  `ms_per_step` is the wall time of one timed sample
+    (what a step of this arm actually ran); `value` is the full-view throughput extrapolated from the samples, the
+    scale factors are in `cpu_baseline`."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    per_step = []
-    res = None
-    for _ in range(args.warmup + args.steps):
-        # each "step" is one bounded sample; keep the whole run within a few minutes
-        res = oracle_sample(args.workload, args.n, max(2.0, min(args.cpu_seconds, 120.0 / max(args.warmup + args.steps, 1))))
-        per_step.append(res["value"])
-    vals = per_step[args.warmup:] or per_step
-    v = float(np.mean(vals))
+    n_total = max(args.warmup + args.steps, 1)
+    smp = OracleSampler(args.workload, args.n, max(1.5, min(args.cpu_seconds, 100.0 / n_total)), args.far_inf)
+    walls, fulls = [], []
+    for k in range(n_total):
+        wall, t, full = smp.sample(k)
+        walls.append(wall); fulls.append(full)
+    walls, fulls = walls[args.warmup:] or walls, fulls[args.warmup:] or fulls
+    mpix = smp.W * smp.H / 1e6
+    full = float(np.median(fulls))
+    v = mpix / full
+    cpu = {"value": v, "unit": "MP/s", "cores": 1, "kind": "oracle", "sample": smp.describe(len(walls), float(np.sum(walls))),
+           "full_view_seconds_extrapolated": round(full, 3), "sample_seconds_median": round(float(np.median(walls)), 3),
+           "scale_gaussians": smp.N / smp.n_slice, "scale_tiles": smp.tiles / float(smp.mask.sum()), "setup_seconds": smp.setup_seconds}
+    cpu.update(cpu_info())
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": "MP/s", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": res["step_mpix"] / v * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic", "config": {"workload": args.workload},
-        "cpu_baseline": {"value": v, "unit": "MP/s", "cores": 1, "kind": "oracle", "sample": res["sample"]},
+        "warmup": args.warmup, "ms_per_step": float(np.median(walls)) * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": {"workload": args.workload, "far_inf": bool(args.far_inf)},
+        "cpu_baseline": cpu,
         "e2e": {"value": v, "unit": "MP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gaussians_per_s": res["gaussians_per_s"],
+        "gaussians_per_s": smp.N / full,
     }
     print(json.dumps(line))
 
@@ -254,9 +317,34 @@ def whole_job_rate(world, units_per_rank_per_step, ms_per_step):
 
 # ----------------------------------------------------------------------------- B200 leg
 BASE_STAGES = ("project_fwd", "bin_tiles", "raster_fwd", "l1_loss", "raster_bwd", "project_bwd")
+KERNEL_OF = {"raster_bwd": "raster_bwd_kernel", "raster_fwd": "raster_fwd_kernel", "project_fwd": "project_fwd_kernel",
+             "project_bwd": "project_bwd_kernel", "bin_tiles": "tile_sweep_kernel"}
 
 
-def run_b200(args):
+def pin_host(arr):
+    """Pinned view of a numpy array without a second host copy (cudaHostRegister); falls back to a pinned copy."""
+    import torch
+    a = np.ascontiguousarray(arr, dtype=np.float32)
+    t = torch.from_numpy(a)
+    try:
+        rc = torch.cuda.cudart().cudaHostRegister(t.data_ptr(), t.numel() * t.element_size(), 0)
+        if int(rc) == 0 and t.is_pinned():
+            return t
+    except Exception:
+        pass
+    return t.pin_memory()
+
+
+def unpin_host(t):
+    import torch
+    try:
+        torch.cuda.cudart().cudaHostUnregister(t.data_ptr())
+    except Exception:
+        pass
+
+
+def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, far_inf=False):
+    """Times `steps` steps of one workload on this rank's GPU; returns the fields of the JSON line that depend on it."""
     import torch
     import torch.distributed as dist
 
@@ -264,20 +352,10 @@ def run_b200(args):
     from paper_2606_11390_b200 import scenes
     from paper_2606_11390_b200.pipeline import SplatStep
 
-    B.lib()   # fails loudly when the CUDA extension is missing: there is no fallback
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device"
-    torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    dev = torch.device("cuda", local_rank)
-    peaks = load_peaks()
     props = torch.cuda.get_device_properties(dev)
     sms = props.multi_processor_count
-
-    sc = scenes.make_scene(args.workload, n=args.n)
+    kw = {"far": 3.0e38} if (far_inf and workload == "city") else {}
+    sc = scenes.make_scene(workload, n=args.n, **kw)
     tgt_host = scenes.target_image(sc)
     st = SplatStep(sc, device=dev)
     st.set_target(tgt_host)
@@ -311,7 +389,6 @@ def run_b200(args):
         torch.cuda.synchronize()
 
     stream = torch.cuda.current_stream()
-
     STAGES = BASE_STAGES + (("adam",) if args.adam != "none" else ())
 
     def timed_step(ev):
@@ -324,7 +401,7 @@ def run_b200(args):
             fn()
             ev[k + 1].record(stream)
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         st.step(sync=False)
         if args.adam != "none":
             st.adam(args.adam)            # (also allocates the moments outside the timed region)
@@ -332,21 +409,22 @@ def run_b200(args):
             st.project_bwd(accumulate=2)
     barrier()
 
-    sampler = ClockSampler(local_rank)
+    sampler = ClockSampler(dev.index if dev.index is not None else 0)
     sampler.start()
-    events = [[torch.cuda.Event(enable_timing=True) for _ in range(len(STAGES) + 1)] for _ in range(args.steps)]
+    events = [[torch.cuda.Event(enable_timing=True) for _ in range(len(STAGES) + 1)] for _ in range(steps)]
     barrier()
     t_wall0 = time.perf_counter()
-    for k in range(args.steps):
+    for k in range(steps):
         flush.fill_(k & 0xFF)                 # L2 flush between timed iterations (outside the step's events)
         timed_step(events[k])
     barrier()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
+    assert st.overflow_count == 0 and not st.check_overflow(wait=True), "intersection capacity overflowed during the timed steps"
     step_ms = np.array([ev[0].elapsed_time(ev[-1]) for ev in events])
-    stage_ms = {s: float(np.mean([ev[i].elapsed_time(ev[i + 1]) for ev in events])) for i, s in enumerate(STAGES)}
-    total_ms = max_over_ranks(float(step_ms.sum()), world, dev)
-    ms_per_step = total_ms / args.steps
+    stage_ms = {s: float(np.median([ev[i].elapsed_time(ev[i + 1]) for ev in events])) for i, s in enumerate(STAGES)}
+    ms_per_step = max_over_ranks(float(np.median(step_ms)), world, dev)          # median of the steps, slowest rank
+    ms_mean = max_over_ranks(float(step_ms.mean()), world, dev)
     mpix_step = C * W * H / 1e6
     value = whole_job_rate(world, mpix_step, ms_per_step)
     gauss_per_s = whole_job_rate(world, C * N, ms_per_step)
@@ -355,9 +433,12 @@ def run_b200(args):
     vis = st.radii > 0
     V_sum = int(vis.sum().item())
     V_any = int(vis.any(dim=0).sum().item())
+    del vis
     M_now = int(st.M_dev.item())
-    pairs_bwd = int(st.n_contrib.to(torch.int64).sum().item())
-    lens = (st.tile_ranges[:, 1] - st.tile_ranges[:, 0])
+    stats = torch.zeros((4,), dtype=torch.int64, device=dev)
+    B.gs_raster_pair_stats(st.cfg, st.cams, st.isect_vals, st.tile_ranges, st.means2d, st.conics, st.opacities, stats)
+    pairs_composited, pairs_rej_fwd, pairs_rej_bwd, pairs_dense = [int(x) for x in stats.cpu().tolist()]
+    n_contrib_sum = int(st.n_contrib.to(torch.int64).sum().item())
     # binning plan (mirrors gs_bin_tiles): depth sort = 4 passes over bits 0..30 plus the view bits; tile sort =
     # P_t passes of 8 or 9 bits over the tile id; the generating pass writes (key, value), the last pass values only
     tile_bits = max(1, int(np.ceil(np.log2(C * st.gx * st.gy))))
@@ -376,11 +457,11 @@ def run_b200(args):
         "project_bwd": 4 * N * C + 36 * V_sum + par_b * V_any + par_b * (V_any if args.sparse_grads else N),
         # L1: read image, target, write dL; L1 + SSIM: + three derivative maps written and read, image and target read twice
         "l1_loss": (12 if args.loss == "l1" else 44) * C * W * H * 3,
-        # flops (per evaluated (pixel, record) pair: DESIGN.md "algorithmic flops per pair")
         # Adam: p, g, m, v read, p, m, v written, per float; sparse: radii scan + the same for visible rows only
         "adam": (28 * (par_b // 4) * N if args.adam == "dense" else 4 * N * C + 28 * (par_b // 4) * V_any),
-        "raster_fwd": 22 * pairs_bwd,
-        "raster_bwd": 60 * pairs_bwd,
+        # flops of the method's own work: composited pairs and pairs evaluated but rejected
+        "raster_fwd": FWD_FLOP_COMPOSITED * pairs_composited + FWD_FLOP_REJECTED * pairs_rej_fwd,
+        "raster_bwd": BWD_FLOP_COMPOSITED * pairs_composited + BWD_FLOP_REJECTED * pairs_rej_bwd,
     }
     fp32_peak = sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12      # TFLOP/s
     stage_roof = {}
@@ -393,71 +474,138 @@ def run_b200(args):
         else:
             ach = work[s] / (ms * 1e-3) / 1e9
             stage_roof[s] = {"ms": round(ms, 4), "bound": "hbm", "achieved": round(ach, 1), "peak": peaks["hbm_gbs"],
-                             "unit": "GB/s", "frac": round(ach / peaks["hbm_gbs"], 4)}
+                             "unit": "GB/s", "frac": round(ach / peaks["hbm_gbs"], 4), "frac_nominal": round(ach / HBM_NOMINAL_GBS, 4)}
     dominant = max(STAGES, key=lambda s: stage_ms[s])
     roof = dict(stage_roof[dominant])
     roof.pop("ms")
-    roof["kernel"] = {"raster_bwd": "raster_bwd_kernel", "raster_fwd": "raster_fwd_kernel", "project_fwd": "project_fwd_kernel",
-                      "project_bwd": "project_bwd_kernel", "bin_tiles": "tile_sweep_kernel", "l1_loss": "l1_loss_kernel" if args.loss == "l1" else "ssim_stats_kernel",
-                      "adam": "adam_dense_kernel" if args.adam == "dense" else "adam_visible_multi_kernel"}[dominant]
-    roof["share_of_step"] = round(stage_ms[dominant] / (ms_per_step if world == 1 else float(step_ms.mean())), 4)
-    roof["peak_source"] = ("MEASURED_PEAKS.json (%s)" % peaks["source"]) if roof["bound"] == "hbm" else \
-        f"{sms} SMs x 128 FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)"
-    roof["traffic"] = load_traffic(args.workload, roof["kernel"])
+    kernel_of = dict(KERNEL_OF)
+    kernel_of["l1_loss"] = "l1_loss_kernel" if args.loss == "l1" else "ssim_stats_kernel"
+    kernel_of["adam"] = "adam_dense_kernel" if args.adam == "dense" else "adam_visible_multi_kernel"
+    if dominant == "project_bwd" and not args.sparse_grads and N >= (1 << 22):
+        kernel_of["project_bwd"] = "zero_fill_kernel + project_bwd_kernel"
+    roof["kernel"] = kernel_of[dominant]
+    roof["share_of_step"] = round(stage_ms[dominant] / float(np.median(step_ms)), 4)
+    if roof["bound"] == "hbm":
+        roof["peak_source"] = "MEASURED_PEAKS.json hbm_gbs (%s); frac_nominal is against the nominal 8 TB/s" % peaks["source"]
+    else:
+        roof["peak_source"] = f"{sms} SMs x 128 FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)"
+        roof["note"] = ("flops counted on the pairs the method evaluates (gs_raster_pair_stats): "
+                        f"{FWD_FLOP_COMPOSITED if dominant == 'raster_fwd' else BWD_FLOP_COMPOSITED} per composited pair, "
+                        f"{FWD_FLOP_REJECTED if dominant == 'raster_fwd' else BWD_FLOP_REJECTED} per evaluated-and-rejected pair; the kernel is "
+                        "latency/barrier bound (ncu FMA pipe < 45 % of cycles, profiles/), not pipe bound")
+    roof["traffic"] = load_traffic(workload + ("_farinf" if far_inf else ""), roof["kernel"].split(" ")[0])
 
-    # ---- end to end: inputs from pinned host memory, loss read back, every step
+    # ---- end to end: inputs from pinned host memory, loss read back, every step; uploads of step k + 1 overlap step k
     e2e = None
-    if not args.no_e2e:
-        host_params = {k: torch.from_numpy(np.ascontiguousarray(sc[k], dtype=np.float32)).pin_memory() for k in st.param_names}
-        host_tgt = torch.from_numpy(tgt_host).pin_memory()
+    if want_e2e:
+        # the parameters the timed steps used (Morton order included), back on the host
+        src = {k: (st.params[k].cpu().numpy() if args.morton else sc[k]) for k in st.param_names}
+        host_params = {k: pin_host(src[k]) for k in st.param_names}
+        host_tgt = pin_host(tgt_host)
         host_loss = torch.zeros((1,), dtype=torch.float32).pin_memory()
         h2d = sum(v.numel() * 4 for v in host_params.values()) + host_tgt.numel() * 4
         d2h = 4
 
-        def e2e_step():
-            # the public end-to-end call: H2D of parameters and targets (the target copy overlaps P1..R1 on a
-            # second stream), the step, D2H of the loss, stream drained
-            st.step_from_host(host_params, host_tgt, host_loss)
+        def e2e_run(n, with_params):
+            st.upload_async(host_params if with_params else None, host_tgt)
+            for k in range(n):
+                if k + 1 < n:
+                    st.upload_async(host_params if with_params else None, host_tgt)      # overlaps step k
+                st.step_uploaded(host_loss)
+                stream.synchronize()                                                     # the loss of step k is on the host
 
-        for _ in range(3):
-            e2e_step()
+        n_e2e = max(3, min(steps, 10))
+        e2e_run(2, True)
         barrier()
-        n_e2e = max(3, min(args.steps, 10))
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        for _ in range(n_e2e):
-            e2e_step()
+        e2e_run(n_e2e, True)
         e1.record(stream)
         barrier()
-        e_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
-        e2e = {"value": whole_job_rate(world, mpix_step, e_ms / n_e2e), "unit": "MP/s", "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms / n_e2e, "steps": n_e2e, "loss": float(host_loss.item())}
+        e_ms = max_over_ranks(e0.elapsed_time(e1), world, dev) / n_e2e
+        # the same with the parameters resident in HBM (optimizer state, as in a training loop): only the targets move
+        e2e_run(2, False)
+        barrier()
+        e0.record(stream)
+        e2e_run(n_e2e, False)
+        e1.record(stream)
+        barrier()
+        r_ms = max_over_ranks(e0.elapsed_time(e1), world, dev) / n_e2e
+        tgt_bytes = host_tgt.numel() * 4
+        e2e = {"value": whole_job_rate(world, mpix_step, e_ms), "unit": "MP/s", "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms, "steps": n_e2e, "loss": float(host_loss.item()),
+               "h2d_gbs_achieved": round(h2d / (e_ms * 1e-3) / 1e9, 2),
+               "inputs": "parameters + target images from pinned host memory every step, double-buffered on a copy stream",
+               "targets_only": {"value": whole_job_rate(world, mpix_step, r_ms), "unit": "MP/s", "ms_per_step": r_ms,
+                                "h2d_bytes_per_step": int(tgt_bytes), "inputs": "target images only; parameters resident in HBM"}}
+        for t in list(host_params.values()) + [host_tgt]:
+            unpin_host(t)
+        del host_params, host_tgt
 
+    out = {
+        "value": value, "ms_per_step": ms_per_step, "ms_per_step_mean": ms_mean, "gaussians_per_s": gauss_per_s,
+        "config": {"workload": workload + (" (far = +inf)" if far_inf else ""), "loss": args.loss, "morton": bool(args.morton), "adam": args.adam,
+                   "sparse_grads": bool(args.sparse_grads), "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
+                   "intersections": M_now, "visible_entries": V_sum, "visible_gaussians": V_any,
+                   "pairs_composited": pairs_composited, "pairs_rejected_fwd": pairs_rej_fwd, "pairs_rejected_bwd": pairs_rej_bwd,
+                   "pairs_dense_bound": pairs_dense, "n_contrib_sum": n_contrib_sum,
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "timing": "median of the timed steps (CUDA events)",
+                   "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},
+        "morton_sort_ms": morton_ms, "clocks": clocks, "e2e": e2e,
+        "gpu_launches": (st.launches_per_step() + {"none": 0, "dense": 5, "sparse": 1}[args.adam]) * steps,
+        "roofline": roof, "stages": stage_roof, "wall_s_timed_region": round(t_wall, 3),
+    }
+    del st, flush
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_11390_b200 import binding as B
+
+    B.lib()   # fails loudly when the CUDA extension is missing: there is no fallback
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+    peaks = load_peaks()
+
+    main = bench_workload(args, args.workload, dev, peaks, world, args.steps, args.warmup, not args.no_e2e, args.far_inf)
+    per_config = None
+    if world == 1 and not args.no_per_config and args.workload == "city" and args.n is None and not args.far_inf:
+        # the other BASELINE configs, short runs (parity-test cases, reported here so that one run covers every config)
+        per_config = {}
+        for wl in ("object", "room", "block"):
+            r = bench_workload(args, wl, dev, peaks, world, 10, 5, False)
+            per_config[wl] = {"value": round(r["value"], 1), "unit": "MP/s", "ms_per_step": round(r["ms_per_step"], 4),
+                              "gaussians_per_s": r["gaussians_per_s"], "steps": 10, "warmup": 5,
+                              "stages": {s: {k: v[k] for k in ("ms", "frac", "bound")} for s, v in r["stages"].items()},
+                              "intersections": r["config"]["intersections"], "visible_entries": r["config"]["visible_entries"],
+                              "pairs_composited": r["config"]["pairs_composited"]}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        cpu = oracle_sample(args.workload, args.n, args.cpu_seconds)
+        cpu = oracle_baseline(args.workload, args.n, args.cpu_seconds, args.far_inf)
     line = {
-        "metric": METRIC, "value": value, "unit": "MP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "metric": METRIC, "value": main["value"], "unit": "MP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": args.workload, "loss": args.loss, "morton": bool(args.morton), "adam": args.adam, "sparse_grads": bool(args.sparse_grads), "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
-                   "intersections": M_now, "visible_entries": V_sum, "pairs_bwd": pairs_bwd,
-                   "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},
-        "gaussians_per_s": gauss_per_s,
-        "morton_sort_ms": morton_ms,
-        "clocks": clocks,
-        "e2e": e2e,
-        "gpu_launches": (st.launches_per_step() + {"none": 0, "dense": 5, "sparse": 1}[args.adam]) * args.steps,
-        "roofline": roof,
-        "stages": stage_roof,
-        "cpu_baseline": cpu,
-        "wall_s_timed_region": round(t_wall, 3),
     }
+    for k in ("config", "gaussians_per_s", "ms_per_step_mean", "morton_sort_ms", "clocks", "e2e", "gpu_launches", "roofline", "stages"):
+        line[k] = main[k]
+    line["cpu_baseline"] = cpu
+    line["per_config"] = per_config
+    line["wall_s_timed_region"] = main["wall_s_timed_region"]
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -131,6 +131,17 @@ int gs_raster_bwd(const gs_config* cfg /*host*/, int32_t C, const gs_camera* cam
                   const int32_t* radii /*optional*/, float* dL_dmeans2d, float* dL_dconics, float* dL_dopacities,
                   float* dL_drgbs, void* stream);
 
+/* Measurement aid (not a step of the hot path; bench.py calls it outside the timed region to count the work the method
+ * itself does): replays the per-pixel decisions of O-R1 over the tile lists and writes
+ *   stats[0] = (pixel, record) pairs composited,
+ *   stats[1] = pairs the forward definition evaluates without compositing (rejected by a rule, or terminating the pixel),
+ *   stats[2] = pairs the backward definition walks (list position <= n_contrib) without compositing,
+ *   stats[3] = 256 x number of records (the dense bound).
+ * stats: device uint64[4], overwritten.  Asynchronous on `stream`. */
+int gs_raster_pair_stats(const gs_config* cfg /*host*/, int32_t C, const gs_camera* cams /*host*/,
+                         const int32_t* isect_vals, const int64_t* tile_ranges, const float* means2d,
+                         const float* conics, const float* opacities, uint64_t* stats, void* stream);
+
 /* P5 -- per-Gaussian backward.  Chain rule through conic ->
  * 2-D covariance -> (J, Sigma) -> (mean, log-scale, quaternion), mean2d -> mean, rgb -> SH
  * coefficients and view direction -> mean, opacity -> logit; summed over the C views.  Gradients
@@ -146,6 +157,14 @@ int gs_project_bwd(const gs_config* cfg /*host*/, int64_t N, const float* means,
                    const float* dL_dconics, const float* dL_dopacities, const float* dL_drgbs,
                    float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats, float* dL_dopacity_logits,
                    float* dL_dsh, int32_t accumulate, void* stream);
+
+/* The dense zero-fill of gs_project_bwd as a call of its own: zeroes all N rows of the five gradient arrays.
+ * gs_grad_zero_fill followed by gs_project_bwd(accumulate = 1) gives exactly the result of gs_project_bwd(accumulate = 0).
+ * It exists so that a caller can run the 236 N bytes of stores (SH degree 3) on a second stream while the rasterisation
+ * kernels, which leave the HBM almost idle, run on the first (the paper's own remedy for memory stalls is to overlap,
+ * PAPER.md:84).  Asynchronous on `stream`.  Errors: GS_ERR_INVALID_ARGUMENT, GS_ERR_CUDA. */
+int gs_grad_zero_fill(int64_t N, int32_t sh_degree, float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats,
+                      float* dL_dopacity_logits, float* dL_dsh, void* stream);
 
 /* Harness loss (SURVEY.md 8(c) reading A18): mean-reduced L1 against a target image.
  * dL_dimage[n] = sign(image - target) / n; *loss_sum (device, float, caller-zeroed) += sum |image - target| / n. */

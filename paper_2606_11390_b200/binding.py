@@ -13,12 +13,12 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, os.environ.get("GS_LIB_NAME", "libgsplat_b200.so"))   # GS_LIB_NAME: tuning builds
+LIB_PATH = os.path.join(_HERE, "libgsplat_b200.so")
 
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
-           "gs_raster_fwd", "gs_raster_bwd", "gs_project_bwd", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
+           "gs_raster_fwd", "gs_raster_bwd", "gs_raster_pair_stats", "gs_project_bwd", "gs_grad_zero_fill", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
 
 
 class gs_camera(C.Structure):
@@ -198,6 +198,16 @@ def gs_raster_bwd(cfg, cams, N_total, isect_vals, tile_ranges, means2d, conics, 
     _check(rc, "gs_raster_bwd")
 
 
+def gs_raster_pair_stats(cfg, cams, isect_vals, tile_ranges, means2d, conics, opacities, stats, stream=None):
+    """Measurement aid: stats (int64[4], device) = composited pairs, pairs the forward / the backward definition evaluates
+    without compositing, 256 x records."""
+    import torch
+    rc = lib().gs_raster_pair_stats(C.byref(cfg), C.c_int32(len(cams)), cams, _ptr(isect_vals, torch.int32),
+                                    _ptr(tile_ranges, torch.int64), _ptr(means2d, torch.float32), _ptr(conics, torch.float32),
+                                    _ptr(opacities, torch.float32), _ptr(stats, torch.int64), _stream(stream))
+    _check(rc, "gs_raster_pair_stats")
+
+
 def gs_project_bwd(cfg, means, log_scales, quats, opacity_logits, sh, cams, radii, dL_dmeans2d, dL_dconics,
                    dL_dopacities, dL_drgbs, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh,
                    accumulate=False, stream=None):
@@ -212,6 +222,15 @@ def gs_project_bwd(cfg, means, log_scales, quats, opacity_logits, sh, cams, radi
                               _ptr(dL_dopacity_logits, torch.float32), _ptr(dL_dsh, torch.float32),
                               C.c_int32(int(accumulate)), _stream(stream))
     _check(rc, "gs_project_bwd")
+
+
+def gs_grad_zero_fill(sh_degree, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh, stream=None):
+    import torch
+    N = dL_dmeans.shape[0]
+    rc = lib().gs_grad_zero_fill(C.c_int64(N), C.c_int32(sh_degree), _ptr(dL_dmeans, torch.float32), _ptr(dL_dlog_scales, torch.float32),
+                                 _ptr(dL_dquats, torch.float32), _ptr(dL_dopacity_logits, torch.float32), _ptr(dL_dsh, torch.float32),
+                                 _stream(stream))
+    _check(rc, "gs_grad_zero_fill")
 
 
 def gs_l1_loss(image, target, dL_dimage, loss_sum, stream=None):

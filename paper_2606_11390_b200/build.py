@@ -13,12 +13,10 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, os.environ.get("GS_LIB_NAME", "libgsplat_b200.so"))
+LIB = os.path.join(HERE, "libgsplat_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
-# tuning experiments: extra -D definitions (e.g. GS_NVCC_DEFS="-DGS_BWD_BATCH=128") and another output name
-FLAGS += os.environ.get("GS_NVCC_DEFS", "").split()
 
 
 def sources():

@@ -58,18 +58,12 @@ constexpr int kSortTile = kSortThreads * kSortItems;
 
 constexpr int kTsThreads = 512;        // tile sort
 constexpr int kTsWarps = kTsThreads / 32;
-#ifndef GS_TS_ITEMS
-#define GS_TS_ITEMS 16
-#endif
-constexpr int kTsItems = GS_TS_ITEMS;
+constexpr int kTsItems = 16;
 constexpr int kTsTile = kTsThreads * kTsItems;
 constexpr int kTsMaxBits = 9;
 constexpr int kTsMaxBins = 1 << kTsMaxBits;
 constexpr int kTsMaxPasses = 4;
-#ifndef GS_LOOK_WIDE
-#define GS_LOOK_WIDE 1
-#endif
-constexpr int kLookWide = GS_LOOK_WIDE;   // predecessors inspected per look-back round trip
+constexpr int kLookWide = 1;              // predecessors inspected per look-back round trip (4 and 8 measured: no gain)
 
 struct SortPlan {
     int P;
@@ -988,10 +982,7 @@ struct TileSweepSmem {
 };
 
 template <int BITS, bool GEN>
-#ifndef GS_TS_MINB
-#define GS_TS_MINB 2
-#endif
-__global__ void __launch_bounds__(kTsThreads, GS_TS_MINB) tile_sweep_kernel(const TileSweepArgs a) {
+__global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSweepArgs a) {
     using Smem = TileSweepSmem<BITS>;
     constexpr int BINS = Smem::BINS;
     static_assert(kTsItems % 8 == 0, "blocked generation reads 8 heads per vector");
@@ -1217,23 +1208,11 @@ __global__ void __launch_bounds__(256) keys_kernel(const unsigned int* __restric
 
 __global__ void set_count_kernel(unsigned long long* count, unsigned long long n) { *count = n; }
 
-static int sm_count() {
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    return sms;
-}
-
 // 64-bit radix passes; data starts in (k0, v0) and ping-pongs with (k1, v1)
 static int run_sort(const SortPlan& plan, uint64_t* k0, int32_t* v0, uint64_t* k1, int32_t* v1, const unsigned long long* count,
                     unsigned int* tickets, unsigned int* hist, unsigned long long* status, int64_t capacity, cudaStream_t st) {
     if (plan.P == 0) return GS_OK;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SweepSmem)) != cudaSuccess)
-            return GS_ERR_CUDA;
-        attr_set = true;
-    }
+    if (int rc0 = ensure_smem(onesweep_kernel, 1, (int)sizeof(SweepSmem))) return rc0;
     const int sms = sm_count();
     const int64_t tiles = (capacity + kSortTile - 1) / kSortTile;
     const int64_t hist_blocks = tiles < (int64_t)sms * 4 ? tiles : (int64_t)sms * 4;
@@ -1258,16 +1237,17 @@ static int run_sort(const SortPlan& plan, uint64_t* k0, int32_t* v0, uint64_t* k
 
 template <int BITS, bool GEN>
 static int launch_tile_sweep(const TileSweepArgs& a, int64_t capacity, cudaStream_t st) {
-    static int blocks_per_sm = 0;
     const int smem = (int)sizeof(TileSweepSmem<BITS>);
-    if (!blocks_per_sm) {
-        if (cudaFuncSetAttribute(tile_sweep_kernel<BITS, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GS_ERR_CUDA;
+    constexpr int slot = 2 + (BITS == 9 ? 2 : 0) + (GEN ? 1 : 0);
+    if (int rc0 = ensure_smem(tile_sweep_kernel<BITS, GEN>, slot, smem)) return rc0;
+    DeviceCache& dc = device_cache();
+    if (!dc.occ[slot]) {
         int b = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, tile_sweep_kernel<BITS, GEN>, kTsThreads, smem) != cudaSuccess || b < 1) return GS_ERR_CUDA;
-        blocks_per_sm = b;
+        dc.occ[slot] = b;
     }
     const int64_t tiles = (capacity + kTsTile - 1) / kTsTile;
-    const int64_t resident = (int64_t)sm_count() * blocks_per_sm;
+    const int64_t resident = (int64_t)dc.sms * dc.occ[slot];
     tile_sweep_kernel<BITS, GEN><<<(unsigned)(tiles < resident ? tiles : resident), kTsThreads, smem, st>>>(a);
     return launch_status();
 }

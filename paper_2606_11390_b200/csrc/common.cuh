@@ -89,6 +89,38 @@ inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_
 inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? GS_OK : GS_ERR_CUDA; }
 inline int launch_status() { return cuda_status(cudaGetLastError()); }
 
+// Per-device cache of immutable facts about the current device (SM count; which kernels already have their opt-in
+// dynamic shared-memory size set; resident blocks per SM of the persistent kernels).  Entries are idempotent, so
+// concurrent first calls are harmless; nothing here changes the result of any call.
+struct DeviceCache {
+    int sms;
+    unsigned attr_mask;     // bit k: kernel slot k has its shared-memory attribute set on this device
+    int occ[16];            // resident blocks per SM per kernel slot (0 = not queried yet)
+};
+inline DeviceCache& device_cache() {
+    static DeviceCache cache[64];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    DeviceCache& d = cache[dev & 63];
+    if (!d.sms) {
+        int sms = 148;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        d.sms = sms;
+    }
+    return d;
+}
+inline int sm_count() { return device_cache().sms; }
+// sets cudaFuncAttributeMaxDynamicSharedMemorySize once per device and kernel slot
+template <typename Kernel>
+inline int ensure_smem(Kernel kernel, int slot, int bytes) {
+    DeviceCache& d = device_cache();
+    if (!(d.attr_mask & (1u << slot))) {
+        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) return GS_ERR_CUDA;
+        d.attr_mask |= 1u << slot;
+    }
+    return GS_OK;
+}
+
 // Tile rectangle of O-P1 step 8, fp32 with one rounding per operation (no FMA contraction:
 // the same bits must come out of P1, the emit kernel and the host-side reference).
 __device__ __forceinline__ int clampi(int a, int lo, int hi) { return min(max(a, lo), hi); }

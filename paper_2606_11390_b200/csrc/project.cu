@@ -35,10 +35,7 @@ constexpr int kProjThreads = 128;   // P1 block
 constexpr int kBwdThreads = 128;    // P5 block (168 registers per thread)
 constexpr int64_t kZeroFillMinN = 1 << 22;   // from here the dense zero-fill of P5 runs as its own streaming kernels (measured:
                                              // slower at 1 M Gaussians, 0.555 -> 0.44 ms at 10 M, 2.98 -> 2.34 ms at 60 M)
-#ifndef GS_PROJ_ITEMS
-#define GS_PROJ_ITEMS 8
-#endif
-constexpr int kProjItems = GS_PROJ_ITEMS;   // Gaussians per thread in P1's streaming phase
+constexpr int kProjItems = 8;   // Gaussians per thread in P1's streaming phase
 
 template <int DEG>
 __device__ __forceinline__ void load_sh(const float* __restrict__ sh, int64_t i, float* f) {
@@ -572,13 +569,6 @@ __global__ void __launch_bounds__(256) zero_fill_kernel(float* __restrict__ p, i
     if (blockIdx.x == 0 && threadIdx.x < 4 && (n4 << 2) + threadIdx.x < count) p[(n4 << 2) + threadIdx.x] = 0.f;
 }
 
-static int sm_count() {
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    return sms;
-}
-
 // persistent grid: resident blocks of the kernel, or fewer when there are fewer chunks
 template <typename Kernel>
 static unsigned persistent_grid(Kernel kernel, int threads, int64_t n_chunks, int sms) {
@@ -672,6 +662,31 @@ extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* mean
     return GS_OK;
 }
 
+// dense zero-fill of the five gradient arrays (16-byte stores when the pointer allows it)
+static int zero_fill_all(int64_t N, int sh_degree, float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats, float* dL_dopacity_logits,
+                         float* dL_dsh, cudaStream_t st) {
+    const int64_t K3 = 3 * (int64_t)(sh_degree + 1) * (sh_degree + 1);
+    float* ptrs[5] = {dL_dsh, dL_dquats, dL_dmeans, dL_dlog_scales, dL_dopacity_logits};
+    const int64_t counts[5] = {K3 * N, 4 * N, 3 * N, 3 * N, N};
+    for (int k = 0; k < 5; ++k) {
+        if (aligned(ptrs[k], 16)) {
+            const int64_t blocks = ((counts[k] >> 2) + 1023) / 1024;
+            zero_fill_kernel<<<(unsigned)(blocks > 0 ? blocks : 1), 256, 0, st>>>(ptrs[k], counts[k]);
+        } else if (cudaMemsetAsync(ptrs[k], 0, (size_t)counts[k] * sizeof(float), st) != cudaSuccess) {
+            return GS_ERR_CUDA;
+        }
+    }
+    return launch_status();
+}
+
+extern "C" int gs_grad_zero_fill(int64_t N, int32_t sh_degree, float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats,
+                                 float* dL_dopacity_logits, float* dL_dsh, void* stream) {
+    if (N < 0 || sh_degree < 0 || sh_degree > 3) return GS_ERR_INVALID_ARGUMENT;
+    if (N == 0) return GS_OK;
+    if (!dL_dmeans || !dL_dlog_scales || !dL_dquats || !dL_dopacity_logits || !dL_dsh) return GS_ERR_INVALID_ARGUMENT;
+    return zero_fill_all(N, sh_degree, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh, (cudaStream_t)stream);
+}
+
 extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* means, const float* log_scales,
                               const float* quats, const float* opacity_logits, const float* sh, int32_t C,
                               const gs_camera* cams, const int32_t* radii, const float* dL_dmeans2d,
@@ -716,14 +731,7 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
                      aligned(dL_dopacity_logits, 16) && aligned(dL_dsh, 16)) ? 1 : 0;
         a.prezeroed = (accumulate == 2) ? 1 : 0;
         if (!a.accumulate && accumulate != 2 && a.vec_out && N >= kZeroFillMinN) {
-            const int64_t K3 = 3 * (int64_t)(cfg->sh_degree + 1) * (cfg->sh_degree + 1);
-            float* ptrs[5] = {dL_dsh, dL_dquats, dL_dmeans, dL_dlog_scales, dL_dopacity_logits};
-            const int64_t counts[5] = {K3 * N, 4 * N, 3 * N, 3 * N, N};
-            for (int k = 0; k < 5; ++k) {
-                const int64_t blocks = ((counts[k] >> 2) + 1023) / 1024;
-                zero_fill_kernel<<<(unsigned)(blocks > 0 ? blocks : 1), 256, 0, st>>>(ptrs[k], counts[k]);
-            }
-            rc = launch_status();
+            rc = zero_fill_all(N, cfg->sh_degree, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh, st);
             if (rc) return rc;
             a.prezeroed = 1;
         }

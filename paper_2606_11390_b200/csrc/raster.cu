@@ -268,10 +268,7 @@ struct RasterBwdIO {
 // row stride of 72 floats, so that both the 64-bit stores of the evaluation phase and the 128-bit
 // loads of the reduction phase (lane (record g, row pair t) reads pixels 16 t .. 16 t + 15) are free
 // of bank conflicts.
-#ifndef GS_BWD_BATCH
-#define GS_BWD_BATCH 64
-#endif
-constexpr int kBwdBatch = GS_BWD_BATCH;
+constexpr int kBwdBatch = 64;
 constexpr int kBwdChunks = kBwdBatch / 32;
 constexpr int kWarps = kBlock / 32;
 constexpr int kTStride = 72;                // floats per transposition row: 64 pixels + 4 + 4
@@ -593,6 +590,63 @@ __global__ void __launch_bounds__(256) l1_loss_kernel(int64_t n, const float* __
     }
 }
 
+
+// Measurement aid (bench.py's roofline, outside any timed region): replays the per-pixel decisions of O-R1, one thread per
+// pixel, and counts the (pixel, record) pairs the METHOD evaluates -- stats[0] pairs composited; stats[1] pairs the forward
+// definition evaluates without compositing (a rule rejects them, or they terminate the pixel); stats[2] pairs the backward
+// definition walks (list position <= n_contrib) without compositing; stats[3] records of all tile lists times 256 (the
+// dense upper bound).
+__global__ void __launch_bounds__(256) pair_stats_kernel(const RasterArgs a, unsigned long long* __restrict__ stats) {
+    __shared__ float s_u[256], s_v[256], s_A[256], s_B[256], s_C[256], s_lo[256];
+    __shared__ unsigned long long s_sum[3];
+    const int tid = threadIdx.x;
+    const int64_t bt = blockIdx.x;
+    const int64_t view = bt / a.tiles;
+    const int t = (int)(bt - view * a.tiles);
+    const int ty = t / a.gx, tx = t - ty * a.gx;
+    const int j = tx * kTile + (tid & 15), i = ty * kTile + (tid >> 4);
+    const bool inside = (i < a.height) && (j < a.width);
+    const float px = (float)j + 0.5f, py = (float)i + 0.5f;
+    const int64_t start = __ldg(a.ranges + 2 * bt), end = __ldg(a.ranges + 2 * bt + 1);
+    if (tid < 3) s_sum[tid] = 0ull;
+    float T = 1.0f;
+    bool done = !inside;
+    unsigned int n_comp = 0, n_rej = 0, n_rej_before_last = 0, rej_run = 0;
+    for (int64_t base = start; base < end; base += 256) {
+        __syncthreads();
+        const int64_t k = base + tid;
+        if (k < end) {
+            const int g = __ldg(a.vals + k);
+            const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + g);
+            s_u[tid] = uv.x; s_v[tid] = uv.y;
+            s_A[tid] = -0.5f * kLog2e * __ldg(a.conics + 3 * (int64_t)g);
+            s_B[tid] = -kLog2e * __ldg(a.conics + 3 * (int64_t)g + 1);
+            s_C[tid] = -0.5f * kLog2e * __ldg(a.conics + 3 * (int64_t)g + 2);
+            s_lo[tid] = __log2f(__ldg(a.opacities + g));
+        }
+        __syncthreads();
+        const int cnt = (int)((end - base) < 256 ? (end - base) : 256);
+        for (int q = 0; q < cnt && !done; ++q) {
+            const float e = quad_form(s_A[q], s_B[q], s_C[q], s_u[q] - px, s_v[q] - py);
+            const float al = fminf(a.alpha_max, ex2_approx(e + s_lo[q]));
+            if (e > 0.0f || al < a.alpha_min) { ++n_rej; ++rej_run; continue; }
+            const float Tn = T * (1.0f - al);
+            if (Tn < a.t_min) { ++n_rej; done = true; break; }
+            T = Tn;
+            ++n_comp;
+            n_rej_before_last += rej_run;     // rejected pairs in front of the last composited one = what the backward pass walks
+            rej_run = 0;
+        }
+    }
+    __syncthreads();
+    atomicAdd(&s_sum[0], (unsigned long long)n_comp);
+    atomicAdd(&s_sum[1], (unsigned long long)n_rej);
+    atomicAdd(&s_sum[2], (unsigned long long)n_rej_before_last);
+    __syncthreads();
+    if (tid < 3 && s_sum[tid]) atomicAdd(stats + tid, s_sum[tid]);
+    if (tid == 3 && end > start) atomicAdd(stats + 3, (unsigned long long)(end - start) * 256ull);
+}
+
 static int fill_args(const gs_config* cfg, int32_t C, const gs_camera* cams, const int32_t* vals, const int64_t* ranges,
                      const float* means2d, const float* conics, const float* opacities, const float* rgbs, const float* bg,
                      RasterArgs& a) {
@@ -655,13 +709,22 @@ extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* c
         }
     }
     RasterBwdIO io{final_T, n_contrib, dL_dimage, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs};
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(raster_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BwdSmem)) != cudaSuccess)
-            return GS_ERR_CUDA;
-        attr_set = true;
-    }
+    rc = ensure_smem(raster_bwd_kernel, 0, (int)sizeof(BwdSmem));
+    if (rc) return rc;
     raster_bwd_kernel<<<(unsigned)(C * a.tiles), kBlock, sizeof(BwdSmem), st>>>(a, io);
+    return launch_status();
+}
+
+extern "C" int gs_raster_pair_stats(const gs_config* cfg, int32_t C, const gs_camera* cams, const int32_t* isect_vals,
+                                    const int64_t* tile_ranges, const float* means2d, const float* conics, const float* opacities,
+                                    uint64_t* stats, void* stream) {
+    RasterArgs a;
+    const float bg[3] = {0.f, 0.f, 0.f};
+    int rc = fill_args(cfg, C, cams, isect_vals, tile_ranges, means2d, conics, opacities, opacities /*unused*/, bg, a);
+    if (rc) return rc;
+    if (!stats || !aligned(stats, 8)) return GS_ERR_INVALID_ARGUMENT;
+    if (cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream) != cudaSuccess) return GS_ERR_CUDA;
+    pair_stats_kernel<<<(unsigned)(C * a.tiles), 256, 0, (cudaStream_t)stream>>>(a, reinterpret_cast<unsigned long long*>(stats));
     return launch_status();
 }
 
@@ -669,9 +732,7 @@ extern "C" int gs_l1_loss(int64_t n, const float* image, const float* target, fl
     if (n < 0) return GS_ERR_INVALID_ARGUMENT;
     if (n == 0) return GS_OK;
     if (!image || !target || !dL_dimage || !loss_sum) return GS_ERR_INVALID_ARGUMENT;
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int sms = sm_count();
     int64_t blocks = (n + 255) / 256;
     if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
     l1_loss_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(n, image, target, dL_dimage, loss_sum, 1.0f / (float)n);

@@ -66,6 +66,11 @@ class SplatStep:
         self.M_dev = torch.zeros((1,), dtype=torch.int64, device=d)
         self.capacity_M = 0
         self.M = None
+        # asynchronous overflow watch (step(sync=False)): M of the last asynchronous binning call, copied to pinned host
+        # memory behind an event and checked at the start of the next step
+        self._M_host = torch.zeros((1,), dtype=torch.int64).pin_memory()
+        self._M_event = None
+        self.overflow_count = 0
         self._alloc_isect(capacity_M if capacity_M else max(1 << 16, 8 * Cn * N // 4))
 
     # -- intersection buffers ------------------------------------------------------------
@@ -88,15 +93,42 @@ class SplatStep:
         B.gs_project_fwd(self.cfg, p["means"], p["log_scales"], p["quats"], p["opacity_logits"], p["sh"], self.cams,
                          self.means2d, self.depths, self.conics, self.opacities, self.rgbs, self.radii, self.tiles_touched)
 
+    def check_overflow(self, wait=False):
+        """Looks at the record count of the last asynchronous binning call (without blocking unless ``wait``).  When it
+        exceeded the capacity, that step rendered only the background (gs_bin_tiles clears every range on overflow):
+        the buffers are regrown for the following steps, ``overflow_count`` is incremented and True is returned."""
+        ev = self._M_event
+        if ev is None:
+            return False
+        if wait:
+            ev.synchronize()
+        elif not ev.query():
+            return False
+        self._M_event = None
+        m = int(self._M_host.item())
+        if m > self.capacity_M:
+            torch.cuda.current_stream(self.device).synchronize()     # no kernel may still use the old buffers
+            self._alloc_isect(int(m * 1.1) + 1024)
+            self.overflow_count += 1
+            return True
+        return False
+
     def bin_tiles(self, sync=True):
         """With ``sync`` the record count is read back (one host sync) and the buffers grow when
-        the capacity is too small; without it the call is fully asynchronous."""
+        the capacity is too small; without it the call is fully asynchronous and the count is copied to pinned host
+        memory behind an event (see ``check_overflow``)."""
+        if not sync:
+            self.check_overflow()
         while True:
             try:
                 m = B.gs_bin_tiles(self.cfg, self.N, self.cams, self.means2d, self.depths, self.radii, self.workspace,
                                    self.capacity_M, self.isect_keys, self.isect_vals, self.tile_ranges, self.M_dev, sync)
                 if sync:
                     self.M = m
+                elif self._M_event is None:
+                    self._M_host.copy_(self.M_dev, non_blocking=True)
+                    self._M_event = torch.cuda.Event()
+                    self._M_event.record(torch.cuda.current_stream(self.device))
                 return m
             except B.GsError as e:
                 if e.status != B.GS_ERR_CAPACITY:
@@ -131,8 +163,10 @@ class SplatStep:
                          g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], accumulate)
 
     def adam(self, mode="dense", lr=0.0, beta1=0.9, beta2=0.999, eps=1e-15):
-        """One fused Adam step over the five parameter arrays (gs_adam_step); ``mode`` "dense" or "sparse" (only Gaussians
-        visible in >= 1 view of the batch, from the saved radii)."""
+        """One fused Adam step over the five parameter arrays (gs_adam_step); ``mode`` "dense" (the paper's _fused_adam_,
+        PAPER.md:82; needs the dense gradient, i.e. ``project_bwd(accumulate=0)``: with accumulate = 2 the rows of invisible
+        Gaussians hold stale values) or "sparse" (reading A28, a SEMANTIC VARIANT: only Gaussians visible in >= 1 view of the
+        batch are updated, the moments of all other rows do not decay)."""
         if getattr(self, "_adam_m", None) is None:
             self._adam_m = {k: torch.zeros_like(v) for k, v in self.params.items()}
             self._adam_v = {k: torch.zeros_like(v) for k, v in self.params.items()}
@@ -156,35 +190,113 @@ class SplatStep:
         self.raster_bwd()
         self.project_bwd()
 
-    def step(self, sync=False):
-        """One forward+backward pass with the L1 loss against ``self.target``."""
-        self.forward(sync)
+    # From this many Gaussians the dense zero-fill of the gradient arrays (236 N bytes at SH degree 3, the largest single
+    # item of a city step) runs on a second stream underneath the rasterisation kernels, and P5 accumulates into it.
+    OVERLAP_ZERO_FILL_MIN_N = 1 << 22
+
+    def fork_grad_zero_fill(self):
+        """Start the dense zero-fill of the gradient arrays on the side stream (after everything enqueued so far)."""
+        main = torch.cuda.current_stream(self.device)
+        if getattr(self, "_zf_stream", None) is None:
+            self._zf_stream = torch.cuda.Stream(self.device, priority=0)
+            self._zf_fork = torch.cuda.Event()
+            self._zf_join = torch.cuda.Event()
+            self._zf_t0 = torch.cuda.Event(enable_timing=True)
+            self._zf_t1 = torch.cuda.Event(enable_timing=True)
+        self._zf_fork.record(main)
+        zs = self._zf_stream
+        zs.wait_event(self._zf_fork)
+        g = self.grads
+        self._zf_t0.record(zs)
+        B.gs_grad_zero_fill(self.cfg.sh_degree, g["means"], g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], stream=zs)
+        self._zf_t1.record(zs)
+        self._zf_join.record(zs)
+
+    def join_grad_zero_fill(self):
+        torch.cuda.current_stream(self.device).wait_event(self._zf_join)
+
+    def step(self, sync=False, overlap_zero_fill=None):
+        """One forward+backward pass with the L1 loss against ``self.target``.  ``overlap_zero_fill`` (default: from
+        OVERLAP_ZERO_FILL_MIN_N Gaussians): zero-fill the gradients on a second stream while R1, the loss and R2 run."""
+        if overlap_zero_fill is None:
+            overlap_zero_fill = self.N >= self.OVERLAP_ZERO_FILL_MIN_N
+        self.project_fwd()
+        self.bin_tiles(sync)
+        if overlap_zero_fill:
+            self.fork_grad_zero_fill()
+        self.raster_fwd()
         self.l1_loss()
-        self.backward()
+        self.raster_bwd()
+        if overlap_zero_fill:
+            self.join_grad_zero_fill()
+            self.project_bwd(accumulate=1)
+        else:
+            self.project_bwd()
 
     def step_from_host(self, host_params, host_target, host_loss):
-        """End-to-end step: parameters and target images come from (pinned) host tensors, the loss goes back
-        to ``host_loss``.  The parameters are copied on the compute stream; the target images, which only
-        the loss needs, are copied on a second stream while P1, binning and R1 run, and the loss kernel waits
-        for that copy.  Returns after the stream has drained (the loss value is then valid on the host)."""
+        """End-to-end step, synchronous form: ``upload_async`` + ``step_uploaded`` + wait.  Parameters and target images
+        come from (pinned) host tensors, the loss goes back to ``host_loss``."""
+        self.upload_async(host_params, host_target)
+        self.step_uploaded(host_loss)
+        torch.cuda.current_stream(self.device).synchronize()
+
+    # The end-to-end path is torch copies plus the stage calls (there is no host-buffer entry point in the C ABI).  Inputs
+    # are double-buffered: upload_async(k + 1) runs on a copy stream while step k computes on the main stream.
+    def upload_async(self, host_params, host_target):
+        """Enqueue the H2D copies of one step's inputs (parameter arrays -- pass None to keep the resident parameters --
+        and target images) into the set of device buffers that the step after the current one will use."""
         main = torch.cuda.current_stream(self.device)
         if getattr(self, "_copy_stream", None) is None:
             self._copy_stream = torch.cuda.Stream(self.device)
-            self._target_ready = torch.cuda.Event()
-        if self.target is None:
-            self.target = torch.empty(tuple(host_target.shape), dtype=torch.float32, device=self.device)
-        self._copy_stream.wait_stream(main)          # the previous step's loss kernel has read the old target
-        with torch.cuda.stream(self._copy_stream):
-            self.target.copy_(host_target, non_blocking=True)
-            self._target_ready.record(self._copy_stream)
-        for k in self.param_names:
-            self.params[k].copy_(host_params[k], non_blocking=True)
+            self._slot = 0                       # buffer set the NEXT step_uploaded will consume
+            self._pending = 0                    # uploads enqueued and not yet consumed (0..2)
+            self._in_params = [None, None]
+            self._in_target = [None, None]
+            self._in_ready = [None, None]        # copy finished (copy stream)
+            self._in_free = [None, None]         # the step that read this set has finished (main stream)
+        assert self._pending < 2, "two uploads are already waiting"
+        k = (self._slot + self._pending) % 2
+        if self._in_target[k] is None:
+            self._in_target[k] = torch.empty(tuple(host_target.shape), dtype=torch.float32, device=self.device)
+            if host_params is not None:
+                # set 0 is the resident parameter set itself; set 1 is a second copy
+                self._in_params[k] = self.params if k == 0 else {n: torch.empty_like(v) for n, v in self.params.items()}
+        cs = self._copy_stream
+        if self._in_free[k] is not None:
+            cs.wait_event(self._in_free[k])
+        else:
+            cs.wait_stream(main)
+        with torch.cuda.stream(cs):
+            if host_params is not None:
+                for n in self.param_names:
+                    self._in_params[k][n].copy_(host_params[n], non_blocking=True)
+            self._in_target[k].copy_(host_target, non_blocking=True)
+            ev = torch.cuda.Event()
+            ev.record(cs)
+        self._in_ready[k] = ev
+        self._in_has_params = host_params is not None
+        self._pending += 1
+
+    def step_uploaded(self, host_loss=None):
+        """Run one step on the oldest uploaded input set; the loss is copied to ``host_loss`` (pinned) asynchronously.
+        Does not synchronise the host."""
+        assert getattr(self, "_pending", 0) > 0, "call upload_async first"
+        main = torch.cuda.current_stream(self.device)
+        k = self._slot
+        main.wait_event(self._in_ready[k])
+        if self._in_params[k] is not None:
+            self.params = self._in_params[k]
+        self.target = self._in_target[k]
         self.forward(sync=False)
-        main.wait_event(self._target_ready)
         self.l1_loss()
         self.backward()
-        host_loss.copy_(self.loss, non_blocking=True)
-        main.synchronize()
+        ev = torch.cuda.Event()
+        ev.record(main)
+        self._in_free[k] = ev
+        if host_loss is not None:
+            host_loss.copy_(self.loss, non_blocking=True)
+        self._slot = (k + 1) % 2
+        self._pending -= 1
 
     # launches of this library's kernels in one step (memsets excluded): P1; compact, tile y-scan, x-scan,
     # ranges, histogram scan, depth-sort histogram + passes, entry offsets, tile-sort passes (+ keys); R1, L1,

@@ -59,6 +59,22 @@ def test_reference_arm_prints_the_contract_line_on_rank0():
     assert line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] == 1
     assert line["e2e"] == {"value": line["value"], "unit": "MP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert line["config"]["workload"] == "tiny" and line["vs_baseline"] is None
+    # ms_per_step is what one step of this arm actually timed (a bounded sample), the extrapolation sits in cpu_baseline
+    cb = line["cpu_baseline"]
+    assert line["ms_per_step"] == pytest.approx(cb["sample_seconds_median"] * 1e3, rel=1e-2, abs=1.0)
+    assert cb["nproc"] >= 1 and isinstance(cb["cpu_model"], str) and cb["scale_gaussians"] >= 1 and cb["scale_tiles"] >= 1
+    assert cb["full_view_seconds_extrapolated"] > 0
+
+
+def test_reference_arm_slices_gaussians_and_tiles_on_a_larger_scene():
+    """With a small time budget the sample takes a slice of the Gaussians and every k-th tile; the extrapolated
+    full-view time stays within a factor of the time of running the whole view."""
+    import bench
+    smp = bench.OracleSampler("object", 20_000, 0.5)
+    assert smp.kt > 1 and smp.n_slice <= smp.N
+    wall, t, full = smp.sample(0)
+    assert set(t) == {"project_fwd", "bin_tiles", "raster_fwd", "raster_bwd", "project_bwd"}
+    assert full > wall > 0
 
 
 def test_reference_arm_other_ranks_exit_without_work():

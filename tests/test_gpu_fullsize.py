@@ -81,9 +81,28 @@ def depth_tolerance(sc, ref):
     return tol
 
 
+def record(entry, fname="parity_fullsize.jsonl"):
+    """Append one result record to gpurun_out/ (summarised under profiles/)."""
+    import json
+    import os
+    try:
+        d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+        os.makedirs(d, exist_ok=True)
+        with open(os.path.join(d, fname), "a") as f:
+            f.write(json.dumps(entry) + "\n")
+    except OSError:
+        pass
+
+
 def check_project_fwd(st, ref, name, sc):
     got = {k: getattr(st, k).cpu().numpy() for k in ("means2d", "depths", "conics", "opacities", "rgbs", "radii")}
     got["tiles_touched"] = st.tiles_touched.cpu().numpy().view(np.uint32)
+    check_project_fwd_arrays(got, ref, name, sc)
+    return got
+
+
+def check_project_fwd_arrays(got, ref, name, sc):
+    """`got`, `ref`: P1 outputs [C, n, *] of the same Gaussians; sc["means"] holds those n Gaussians."""
     rr = ref["radius_real"]
     amb_r = np.abs(rr - np.round(rr)) <= 1e-4 * np.maximum(rr, 1.0)
     u = ref["means2d"]
@@ -113,7 +132,8 @@ def check_project_fwd(st, ref, name, sc):
     assert np.abs(got["rgbs"][m] - ref["rgbs"][m]).max() <= 5e-6
     print(f"[{name}] P1: visible {int(both.sum())} of {both.size}; ambiguous radius {int(dr.sum())}, tiles {int(dt.sum())}; "
           f"mean2d max err {err_u.max():.2e} px, max err/bound {(err_u / tol_u).max():.2f}")
-    return got
+    return {"visible": int(both.sum()), "entries": int(both.size), "ambiguous_radius": int(dr.sum()), "ambiguous_tiles": int(dt.sum()),
+            "mean2d_max_err_px": float(err_u.max()), "conic_max_rel_err": float(err_c.max())}
 
 
 # ------------------------------------------------------------------------------------ object: everything
@@ -150,6 +170,8 @@ def test_object_full_config_chained_step(B, oracle):
     assert abs(float(st.loss.item()) - loss_ref) <= 1e-5 * max(loss_ref, 1e-3)
     errs = {k: rel_l2(st.grads[k].cpu().numpy(), gp[k]) for k in gp}
     print(f"[object] M {M}; image err>1e-4 frac {frac_bad:.2e}; grad rel L2 {errs}")
+    record({"test": "object_full_config_chained_step", "M": M, "frac_clear_pixels_above_1e-4": float(frac_bad),
+            "median_err": float(np.median(err)), "ambiguous_pixels": int((~clear).sum()), "grad_rel_l2": errs})
     for k, e in errs.items():
         assert e <= 1e-3, (k, e)
 
@@ -256,5 +278,7 @@ def test_full_size_sampled(B, oracle, workload, stride, n):
         assert np.all(g[~anyvis] == 0)                        # dense overwrite
         e5[k] = rel_l2(g, gp[k])
         assert e5[k] <= 1e-3, (k, e5[k])
+    record({"test": "full_size_sampled", "workload": workload, "N": N, "M": M, "tile_lists_exact": n_checked, "pixels": int(pm.sum()),
+            "image_max_err_clear": float(err[clear].max()), "ambiguous_pixels": int((pm & ~clear).sum()), "r2_rel_l2": e2, "p5_rel_l2": e5})
     print(f"[{workload}] M {M}; {n_checked} tile lists exact; {int(pm.sum())} pixels on {len(sample)} tiles, max err "
           f"{err[clear].max():.2e}, ambiguous {int((pm & ~clear).sum())}; R2 rel L2 {e2}; P5 rel L2 {e5}")

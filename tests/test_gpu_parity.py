@@ -452,6 +452,9 @@ def test_end_to_end_step_against_oracle(B, oracle, name, sc):
     assert abs(float(st.loss.item()) - loss_ref) <= 1e-5 * max(loss_ref, 1e-3)
     errs = {k: rel_l2(st.grads[k].cpu().numpy(), gp[k]) for k in gp}
     print(f"[{name}] M {st.M} image err>1e-4 frac {frac_bad:.2e}; grad rel L2 {errs}")
+    from test_gpu_fullsize import record
+    record({"test": "end_to_end_step_against_oracle", "scene": name, "M": int(st.M), "frac_clear_pixels_above_1e-4": float(frac_bad),
+            "median_err": float(np.median(err)), "ambiguous_pixels": int((~clear).sum()), "grad_rel_l2": errs})
     for k, e in errs.items():
         assert e <= 1e-3, (k, e)
 
@@ -479,6 +482,68 @@ def test_step_from_host_equals_resident_step(B):
     assert abs(float(host_loss.item()) - float(ref.loss.item())) <= 1e-6
     for k in st.param_names:
         assert rel_l2(st.grads[k].cpu().numpy(), ref.grads[k].cpu().numpy()) <= 1e-5, k
+
+
+def test_pipelined_uploads_equal_resident_steps(B):
+    """upload_async(k + 1) overlapping step_uploaded(k) (two input sets, copy stream): every step sees its own inputs.
+    Steps alternate between two parameter sets and two targets; each must reproduce the resident step on that pair."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    name, sc = SCENES[1]
+    tgt = scenes.target_image(sc)
+    sc2 = dict(sc)
+    sc2["means"] = (sc["means"] * np.float32(0.9)).astype(np.float32)
+    tgt2 = (1.0 - tgt).astype(np.float32)
+    refs = []
+    for s_, t_ in ((sc, tgt), (sc2, tgt2)):
+        r = SplatStep(s_)
+        r.set_target(t_)
+        r.step(sync=True)
+        torch.cuda.synchronize()
+        refs.append((float(r.loss.item()), r.image.clone(), {k: r.grads[k].clone() for k in r.param_names}, r.capacity_M))
+    st = SplatStep(sc, upload=False, capacity_M=max(refs[0][3], refs[1][3]))
+    hp = [{k: torch.from_numpy(np.ascontiguousarray(s_[k], dtype=np.float32)).pin_memory() for k in st.param_names} for s_ in (sc, sc2)]
+    ht = [torch.from_numpy(t_).pin_memory() for t_ in (tgt, tgt2)]
+    n = 5
+    losses = [torch.zeros((1,), dtype=torch.float32).pin_memory() for _ in range(n)]
+    st.upload_async(hp[0], ht[0])
+    for k in range(n):
+        if k + 1 < n:
+            st.upload_async(hp[(k + 1) % 2], ht[(k + 1) % 2])
+        st.step_uploaded(losses[k])
+        if k >= n - 2:                       # check the last two steps (one of each input set) before their buffers are reused
+            torch.cuda.synchronize()
+            loss_ref, img_ref, g_ref, _ = refs[k % 2]
+            assert torch.equal(st.image, img_ref)
+            assert abs(float(losses[k].item()) - loss_ref) <= 1e-6
+            for name_ in st.param_names:
+                assert rel_l2(st.grads[name_].cpu().numpy(), g_ref[name_].cpu().numpy()) <= 1e-5, name_
+    torch.cuda.synchronize()
+    for k in range(n):
+        assert abs(float(losses[k].item()) - refs[k % 2][0]) <= 1e-6
+
+
+def test_async_overflow_is_detected_and_recovered(B):
+    """step(sync=False) with a capacity that is too small renders only the background (documented behaviour of
+    gs_bin_tiles); the asynchronous watch sees it at the next step, regrows, and the following step is correct."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    name, sc = SCENES[1]
+    tgt = scenes.target_image(sc)
+    ref = SplatStep(sc)
+    ref.set_target(tgt)
+    ref.step(sync=True)
+    torch.cuda.synchronize()
+    st = SplatStep(sc, capacity_M=max(1024, ref.M // 3))
+    st.set_target(tgt)
+    st.step(sync=False)
+    torch.cuda.synchronize()
+    assert int(st.M_dev.item()) == ref.M > st.capacity_M
+    assert float(st.image.abs().max().item()) == 0.0          # black background only
+    assert st.check_overflow(wait=True) and st.overflow_count == 1 and st.capacity_M >= ref.M
+    st.step(sync=False)
+    torch.cuda.synchronize()
+    assert not st.check_overflow(wait=True) and st.overflow_count == 1
+    assert torch.equal(st.image, ref.image)
+    assert torch.equal(st.isect_vals[: ref.M], ref.isect_vals[: ref.M])
 
 
 @pytest.mark.parametrize("name,sc", SCENES[1:], ids=[s[0] for s in SCENES[1:]])

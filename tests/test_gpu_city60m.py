@@ -97,7 +97,7 @@ def test_city_60m(B, oracle, city60, far):
     ref = oracle.project_fwd(cfg, sub["means"], sub["log_scales"], sub["quats"], sub["opacity_logits"], sub["sh"], cams)
     got = {k: getattr(st, k)[:, rows_t].cpu().numpy() for k in ("means2d", "depths", "conics", "opacities", "rgbs", "radii")}
     got["tiles_touched"] = st.tiles_touched[:, rows_t].cpu().numpy().view(np.uint32)
-    p1 = check_project_fwd_arrays(got, ref, "city-60M", dict(sc, means=sub["means"]))
+    p1 = check_project_fwd_arrays(got, ref, "city-60M", dict(sc, means=sub["means"], log_scales=sub["log_scales"], quats=sub["quats"]))
     del ref
 
     # ---- binning: properties on the whole output

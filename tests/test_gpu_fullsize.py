@@ -81,6 +81,60 @@ def depth_tolerance(sc, ref):
     return tol
 
 
+def conic_tolerance(sc, ref):
+    """First-order fp32 error estimate of the conic, relative to its largest entry (eps = 2^-24).  O-P1 steps 2-4 form
+    Sigma' = T Sigma T^T from Sigma = M M^T, so a Gaussian that is thin along the viewing direction gets its small
+    projected variance as a difference of large terms, and the 2 x 2 inversion amplifies by the cancellation in
+    det = a c - b^2.  Terms: rounding of the products 8 eps |T| (|M| |M|^T) |T|^T; error of T (from t = W p + tau, relative
+    size d = eps max_k S_k / t_z, S as in mean2d_tolerance) 4 d |T_r| |Sigma T_c^T|; det: a dc + c da + 2 |b| db.  The
+    constants are calibrated, not worst-case: oracle<float> against oracle<double> stays below 0.45 (object), 0.3 (room),
+    0.1 (city, 60 M) of this estimate.  The bar is max(2e-4, estimate): 2e-4 for all but the
+    ill-conditioned entries (2e-5 of the object entries, 0.2 % of room, 13 % of city with its 2 km coordinates)."""
+    eps = 2.0 ** -24
+    p = sc["means"].astype(np.float64)
+    s = np.exp(sc["log_scales"].astype(np.float64))
+    q = sc["quats"].astype(np.float64)
+    q = q / np.linalg.norm(q, axis=-1, keepdims=True)
+    w, x, y, z = q[:, 0], q[:, 1], q[:, 2], q[:, 3]
+    R = np.stack([1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y),
+                  2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x),
+                  2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)], axis=-1).reshape(-1, 3, 3)
+    Mm = R * s[:, None, :]
+    Sig = Mm @ Mm.transpose(0, 2, 1)
+    Sabs = np.abs(Mm) @ np.abs(Mm).transpose(0, 2, 1)
+    tol = np.zeros(ref["depths"].shape)
+    for ci, cam in enumerate(sc["cameras"]):
+        vm = np.asarray(cam["viewmat"], np.float64).reshape(3, 4)
+        W, tau = vm[:, :3], vm[:, 3]
+        t = p @ W.T + tau
+        Smax = (np.abs(p) @ np.abs(W).T + np.abs(tau)).max(axis=-1)
+        tz = np.where(t[:, 2] > 1e-6, t[:, 2], 1.0)
+        d = eps * Smax / tz
+        fx, fy = cam["fx"], cam["fy"]
+        limx, limy = 1.3 * cam["width"] / (2 * fx), 1.3 * cam["height"] / (2 * fy)
+        xt = np.clip(t[:, 0] / tz, -limx, limx); yt = np.clip(t[:, 1] / tz, -limy, limy)
+        J = np.zeros((len(p), 2, 3))
+        J[:, 0, 0] = fx / tz; J[:, 0, 2] = -fx * xt / tz
+        J[:, 1, 1] = fy / tz; J[:, 1, 2] = -fy * yt / tz
+        T = J @ W
+        Tabs = np.abs(J) @ np.abs(W)
+        ST = Sig @ T.transpose(0, 2, 1)
+        nT = np.linalg.norm(Tabs, axis=-1)
+        nST = np.linalg.norm(ST, axis=1)
+        E = 8 * eps * (Tabs @ Sabs @ Tabs.transpose(0, 2, 1))
+        E[:, 0, 0] += 4 * d * nT[:, 0] * nST[:, 0]
+        E[:, 1, 1] += 4 * d * nT[:, 1] * nST[:, 1]
+        E[:, 0, 1] += 2 * d * (nT[:, 0] * nST[:, 1] + nT[:, 1] * nST[:, 0])
+        Sp = T @ ST
+        a, b, c = Sp[:, 0, 0] + 0.3, Sp[:, 0, 1], Sp[:, 1, 1] + 0.3
+        det = a * c - b * b
+        ddet = a * E[:, 1, 1] + c * E[:, 0, 0] + 2 * np.abs(b) * E[:, 0, 1] + 4 * eps * (a * c + b * b)
+        mx = np.maximum(a, c)
+        with np.errstate(all="ignore"):
+            tol[ci] = (np.maximum(np.maximum(E[:, 0, 0], E[:, 1, 1]), E[:, 0, 1]) + 4 * eps * mx) / mx + ddet / np.abs(det)
+    return np.maximum(2e-4, np.nan_to_num(tol, nan=np.inf))
+
+
 def record(entry, fname="parity_fullsize.jsonl"):
     """Append one result record to gpurun_out/ (summarised under profiles/)."""
     import json
@@ -102,7 +156,7 @@ def check_project_fwd(st, ref, name, sc):
 
 
 def check_project_fwd_arrays(got, ref, name, sc):
-    """`got`, `ref`: P1 outputs [C, n, *] of the same Gaussians; sc["means"] holds those n Gaussians."""
+    """`got`, `ref`: P1 outputs [C, n, *] of the same Gaussians; sc["means"], sc["log_scales"], sc["quats"] hold those n Gaussians."""
     rr = ref["radius_real"]
     amb_r = np.abs(rr - np.round(rr)) <= 1e-4 * np.maximum(rr, 1.0)
     u = ref["means2d"]
@@ -127,13 +181,19 @@ def check_project_fwd_arrays(got, ref, name, sc):
     assert np.all(err_d <= depth_tolerance(sc, ref)[m]), err_d.max()
     cn = np.abs(ref["conics"][m]).max(axis=-1, keepdims=True)
     err_c = (np.abs(got["conics"][m] - ref["conics"][m]) / cn).max(axis=-1)
-    assert err_c.max() <= 2e-4, (err_c.max(), ref["depths"][m][err_c.argmax()])
+    rows = np.nonzero(m.any(axis=0))[0]                 # the estimate only for Gaussians visible somewhere (memory)
+    tol_full = np.full(m.shape, 2e-4)
+    tol_full[:, rows] = conic_tolerance(dict(sc, means=sc["means"][rows], log_scales=sc["log_scales"][rows], quats=sc["quats"][rows]),
+                                        {"depths": ref["depths"][:, rows]})
+    tol_c = tol_full[m]
+    assert np.all(err_c <= tol_c), (err_c.max(), (err_c / tol_c).max(), ref["depths"][m][(err_c / tol_c).argmax()])
     np.testing.assert_allclose(got["opacities"][m], ref["opacities"][m], rtol=2e-6)
     assert np.abs(got["rgbs"][m] - ref["rgbs"][m]).max() <= 5e-6
     print(f"[{name}] P1: visible {int(both.sum())} of {both.size}; ambiguous radius {int(dr.sum())}, tiles {int(dt.sum())}; "
           f"mean2d max err {err_u.max():.2e} px, max err/bound {(err_u / tol_u).max():.2f}")
     return {"visible": int(both.sum()), "entries": int(both.size), "ambiguous_radius": int(dr.sum()), "ambiguous_tiles": int(dt.sum()),
-            "mean2d_max_err_px": float(err_u.max()), "conic_max_rel_err": float(err_c.max())}
+            "mean2d_max_err_px": float(err_u.max()), "conic_max_rel_err": float(err_c.max()),
+            "conic_max_err_over_bar": float((err_c / tol_c).max()), "conic_entries_with_bar_above_2e-4": int((tol_c > 2e-4).sum())}
 
 
 # ------------------------------------------------------------------------------------ object: everything

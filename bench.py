@@ -60,6 +60,13 @@ def parse_args():
     ap.add_argument("--sparse-grads", action="store_true",
                     help="P5 writes only the rows of Gaussians visible in the batch (gs_project_bwd accumulate = 2) instead of the dense "
                          "overwrite; only valid with --adam sparse or none")
+    ap.add_argument("--no-mask", action="store_true",
+                    help="every stage scans the dense radii[C, N] instead of reading P1's visibility bit mask (and P1 does not use the "
+                         "scene-wide log-scale bound)")
+    ap.add_argument("--overlap", action="store_true",
+                    help="run the dense zero-fill of the gradients on a second stream underneath the rasterisation kernels instead of "
+                         "inside project_bwd (measured: no gain, see pipeline.py)")
+    ap.add_argument("--zf-priority", type=int, default=0, help="stream priority of the zero-fill stream (0 or -1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE configs")
@@ -357,7 +364,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     kw = {"far": 3.0e38} if (far_inf and workload == "city") else {}
     sc = scenes.make_scene(workload, n=args.n, **kw)
     tgt_host = scenes.target_image(sc)
-    st = SplatStep(sc, device=dev)
+    st = SplatStep(sc, device=dev, use_mask=False if args.no_mask else None)
     st.set_target(tgt_host)
     st.loss_mode = args.loss
     morton_ms = None
@@ -390,10 +397,20 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
 
     stream = torch.cuda.current_stream()
     STAGES = BASE_STAGES + (("adam",) if args.adam != "none" else ())
+    overlap = args.overlap and not args.sparse_grads
+    st.ZERO_FILL_STREAM_PRIORITY = args.zf_priority
 
-    def timed_step(ev):
-        p5 = (lambda: st.project_bwd(accumulate=2)) if args.sparse_grads else st.project_bwd
-        calls = (st.project_fwd, lambda: st.bin_tiles(sync=False), st.raster_fwd, st.l1_loss, st.raster_bwd, p5)
+    def timed_step(ev, zf_ev=None):
+        if args.sparse_grads:
+            p5 = lambda: st.project_bwd(accumulate=2)
+        elif overlap:
+            p5 = lambda: (st.join_grad_zero_fill(), st.project_bwd(accumulate=1))
+        else:
+            p5 = st.project_bwd
+        bin_call = lambda: st.bin_tiles(sync=False)
+        if overlap:
+            bin_call = lambda: (st.bin_tiles(sync=False), st.fork_grad_zero_fill(*(zf_ev or (None, None))))
+        calls = (st.project_fwd, bin_call, st.raster_fwd, st.l1_loss, st.raster_bwd, p5)
         if args.adam != "none":
             calls = calls + (lambda: st.adam(args.adam),)
         ev[0].record(stream)
@@ -412,17 +429,19 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     sampler = ClockSampler(dev.index if dev.index is not None else 0)
     sampler.start()
     events = [[torch.cuda.Event(enable_timing=True) for _ in range(len(STAGES) + 1)] for _ in range(steps)]
+    zf_events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     barrier()
     t_wall0 = time.perf_counter()
     for k in range(steps):
         flush.fill_(k & 0xFF)                 # L2 flush between timed iterations (outside the step's events)
-        timed_step(events[k])
+        timed_step(events[k], zf_events[k])
     barrier()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
     assert st.overflow_count == 0 and not st.check_overflow(wait=True), "intersection capacity overflowed during the timed steps"
     step_ms = np.array([ev[0].elapsed_time(ev[-1]) for ev in events])
     stage_ms = {s: float(np.median([ev[i].elapsed_time(ev[i + 1]) for ev in events])) for i, s in enumerate(STAGES)}
+    zf_ms = float(np.median([a.elapsed_time(b) for a, b in zf_events])) if overlap else None
     ms_per_step = max_over_ranks(float(np.median(step_ms)), world, dev)          # median of the steps, slowest rank
     ms_mean = max_over_ranks(float(step_ms.mean()), world, dev)
     mpix_step = C * W * H / 1e6
@@ -430,7 +449,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     gauss_per_s = whole_job_rate(world, C * N, ms_per_step)
 
     # ---- algorithmic work of this step (harness-side counting, outside the timed region)
-    vis = st.radii > 0
+    vis = st.visible()
     V_sum = int(vis.sum().item())
     V_any = int(vis.any(dim=0).sum().item())
     del vis
@@ -449,16 +468,22 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     tsort_bytes = 4 * M_now if P_t == 1 else (8 + 16 * (P_t - 2) + 12) * M_now
     K3 = 3 * st.K
     par_b = 4 * (3 + 3 + 4 + 1 + K3)
+    # how visibility travels: the bit mask written by P1 (C * GS_VIS_WORDS(N) words) or the dense radii (and tiles_touched)
+    vis_w = 4 * C * B.vis_words(N) if st.use_mask else 8 * N * C        # written by P1
+    vis_r = 4 * C * B.vis_words(N) if st.use_mask else 4 * N * C        # read by every later stage that needs visibility
     work = {
         # bytes
-        "project_fwd": 12 * N + (par_b - 12) * V_any + 48 * V_sum + 8 * N * C,
-        # compaction (radii; uv, depth -> key, id) + depth sort (histogram, P_d passes) + entry table + tile sort + grid scans, ranges
-        "bin_tiles": 4 * N * C + 24 * V_sum + (8 + 24 * P_d) * V_sum + (32 + 16) * V_sum + tsort_bytes + 24 * cells + 16 * C * st.gx * st.gy,
-        "project_bwd": 4 * N * C + 36 * V_sum + par_b * V_any + par_b * (V_any if args.sparse_grads else N),
+        "project_fwd": 12 * N + (par_b - 12) * V_any + 48 * V_sum + vis_w,
+        # compaction (visibility; uv, depth -> key, id) + depth sort (histogram, P_d passes) + entry table + tile sort + grid scans, ranges
+        "bin_tiles": vis_r + 24 * V_sum + (8 + 24 * P_d) * V_sum + (32 + 16) * V_sum + tsort_bytes + 24 * cells + 16 * C * st.gx * st.gy,
+        # P5: visibility, 2-D gradients, parameters re-read; gradient rows: visible rows only (sparse), visible rows read +
+        # written on top of the zero-fill (overlap), or every row written (dense overwrite)
+        "project_bwd": vis_r + 36 * V_sum + par_b * V_any + par_b * (V_any if args.sparse_grads else (2 * V_any if overlap else N)),
+        "grad_zero_fill": par_b * N,
         # L1: read image, target, write dL; L1 + SSIM: + three derivative maps written and read, image and target read twice
         "l1_loss": (12 if args.loss == "l1" else 44) * C * W * H * 3,
         # Adam: p, g, m, v read, p, m, v written, per float; sparse: radii scan + the same for visible rows only
-        "adam": (28 * (par_b // 4) * N if args.adam == "dense" else 4 * N * C + 28 * (par_b // 4) * V_any),
+        "adam": (28 * (par_b // 4) * N if args.adam == "dense" else vis_r + 28 * (par_b // 4) * V_any),
         # flops of the method's own work: composited pairs and pairs evaluated but rejected
         "raster_fwd": FWD_FLOP_COMPOSITED * pairs_composited + FWD_FLOP_REJECTED * pairs_rej_fwd,
         "raster_bwd": BWD_FLOP_COMPOSITED * pairs_composited + BWD_FLOP_REJECTED * pairs_rej_bwd,
@@ -475,13 +500,18 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
             ach = work[s] / (ms * 1e-3) / 1e9
             stage_roof[s] = {"ms": round(ms, 4), "bound": "hbm", "achieved": round(ach, 1), "peak": peaks["hbm_gbs"],
                              "unit": "GB/s", "frac": round(ach / peaks["hbm_gbs"], 4), "frac_nominal": round(ach / HBM_NOMINAL_GBS, 4)}
+    if overlap:
+        ach = work["grad_zero_fill"] / (zf_ms * 1e-3) / 1e9
+        stage_roof["grad_zero_fill"] = {"ms": round(zf_ms, 4), "bound": "hbm", "achieved": round(ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                        "frac": round(ach / peaks["hbm_gbs"], 4), "frac_nominal": round(ach / HBM_NOMINAL_GBS, 4),
+                                        "note": "second stream, concurrent with raster_fwd / l1_loss / raster_bwd of the same step; not additive"}
     dominant = max(STAGES, key=lambda s: stage_ms[s])
     roof = dict(stage_roof[dominant])
     roof.pop("ms")
     kernel_of = dict(KERNEL_OF)
     kernel_of["l1_loss"] = "l1_loss_kernel" if args.loss == "l1" else "ssim_stats_kernel"
     kernel_of["adam"] = "adam_dense_kernel" if args.adam == "dense" else "adam_visible_multi_kernel"
-    if dominant == "project_bwd" and not args.sparse_grads and N >= (1 << 22):
+    if dominant == "project_bwd" and not args.sparse_grads and not overlap and N >= (1 << 22):
         kernel_of["project_bwd"] = "zero_fill_kernel + project_bwd_kernel"
     roof["kernel"] = kernel_of[dominant]
     roof["share_of_step"] = round(stage_ms[dominant] / float(np.median(step_ms)), 4)
@@ -545,7 +575,9 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     out = {
         "value": value, "ms_per_step": ms_per_step, "ms_per_step_mean": ms_mean, "gaussians_per_s": gauss_per_s,
         "config": {"workload": workload + (" (far = +inf)" if far_inf else ""), "loss": args.loss, "morton": bool(args.morton), "adam": args.adam,
-                   "sparse_grads": bool(args.sparse_grads), "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
+                   "sparse_grads": bool(args.sparse_grads),
+                   "visibility": "bit mask written by P1 + scene-wide log-scale bound" if st.use_mask else "dense radii",
+                   "grad_zero_fill": "second stream, under the rasterisation kernels" if overlap else "inside project_bwd", "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
                    "intersections": M_now, "visible_entries": V_sum, "visible_gaussians": V_any,
                    "pairs_composited": pairs_composited, "pairs_rejected_fwd": pairs_rej_fwd, "pairs_rejected_bwd": pairs_rej_bwd,
                    "pairs_dense_bound": pairs_dense, "n_contrib_sum": n_contrib_sum,

@@ -34,6 +34,12 @@ extern "C" {
 
 #define GS_MAX_VIEWS 64 /* upper bound on C per call */
 
+/* Visibility mask (optional fast path for scenes in which a small fraction of the C*N entries is visible).
+ * uint32 words [C][GS_VIS_WORDS(N)], 16-byte aligned; bit (i & 31) of word c*GS_VIS_WORDS(N) + (i >> 5) is 1 iff entry
+ * (view c, Gaussian i) is visible (radius > 0 and >= 1 tile); bits of i >= N are 0.  gs_project_fwd writes it; gs_bin_tiles,
+ * gs_raster_bwd, gs_project_bwd and gs_adam_step_visible read it instead of scanning the dense radii[C,N]. */
+#define GS_VIS_WORDS(N) ((((int64_t)(N) + 511) / 512) * 16)
+
 typedef enum gs_status {
     GS_OK = 0,
     GS_ERR_INVALID_ARGUMENT = -1, /* null / misaligned pointer, N < 0, C out of range, bad config, views differ in size */
@@ -71,11 +77,22 @@ const char* gs_status_string(int status);
  * tiles_touched; SH colour (+0.5, clamp >= 0) along the camera->Gaussian direction; sigmoid opacity.
  * in : means[N,3] log_scales[N,3] quats[N,4] opacity_logits[N] sh[N,K,3]; cams: host array of C.
  * out: means2d[C,N,2] depths[C,N] conics[C,N,3] (A,B,C) opacities[C,N] rgbs[C,N,3]
- *      radii[C,N] (int32, 0 = culled) tiles_touched[C,N] (uint32). */
+ *      radii[C,N] (int32, 0 = culled) tiles_touched[C,N] (uint32).
+ * vis_mask (optional, out): when given, visibility is reported through the mask (see GS_VIS_WORDS) and radii /
+ *   tiles_touched are written ONLY for visible entries -- the 8*C*N-byte dense zero-fill is skipped and the radii of culled
+ *   entries keep whatever the caller's buffer held; every later stage must then be given the same mask.
+ * log_scale_bound (optional, device scalar): an upper bound of every log-scale (gs_log_scale_bound computes it,
+ *   gs_adam_step* can keep it up to date).  With it, a Gaussian whose largest possible 3-sigma radius cannot reach the
+ *   image of a view is dropped while the means are streamed, before its own scales are read.  It never changes a result
+ *   as long as it is a true upper bound (a NaN bound disables the test). */
 int gs_project_fwd(const gs_config* cfg /*host*/, int64_t N, const float* means, const float* log_scales,
                    const float* quats, const float* opacity_logits, const float* sh, int32_t C,
                    const gs_camera* cams /*host*/, float* means2d, float* depths, float* conics,
-                   float* opacities, float* rgbs, int32_t* radii, uint32_t* tiles_touched, void* stream);
+                   float* opacities, float* rgbs, int32_t* radii, uint32_t* tiles_touched, uint32_t* vis_mask /*optional*/,
+                   const float* log_scale_bound /*optional*/, void* stream);
+
+/* bound[0] (device float) = max over the 3 N log-scales (N >= 1; NaNs are ignored).  Asynchronous on `stream`. */
+int gs_log_scale_bound(int64_t N, const float* log_scales, float* bound, void* stream);
 
 /* B1..B4 -- tile binning for a batch of views.
  * For every entry e = c*N + i with radii[e] > 0, in ascending e, one record per overlapped 16x16
@@ -94,9 +111,11 @@ int gs_project_fwd(const gs_config* cfg /*host*/, int64_t N, const float* means,
  *   through M_dev.
  * isect_keys[capacity_M] (uint64, optional: NULL = the sorted keys are not materialised; the
  * rasteriser reads only values and ranges), isect_vals[capacity_M] (int32),
- * tile_ranges[C*tiles,2] (int64).  depths must be positive (they are: depth > near > 0). */
+ * tile_ranges[C*tiles,2] (int64).  depths must be positive (they are: depth > near > 0).
+ * vis_mask (optional): the mask gs_project_fwd wrote; the visible entries are then exactly its set bits (radii is read
+ *   only for those) and no pass over the dense radii is made. */
 int gs_bin_tiles(const gs_config* cfg /*host*/, int64_t N, int32_t C, const gs_camera* cams /*host*/,
-                 const float* means2d, const float* depths, const int32_t* radii, void* workspace,
+                 const float* means2d, const float* depths, const int32_t* radii, const uint32_t* vis_mask /*optional*/, void* workspace,
                  size_t* workspace_bytes /*host*/, int64_t capacity_M, uint64_t* isect_keys,
                  int32_t* isect_vals, int64_t* tile_ranges, int64_t* M_dev, int64_t* M_out /*host*/,
                  void* stream);
@@ -122,14 +141,14 @@ int gs_raster_fwd(const gs_config* cfg /*host*/, int32_t C, const gs_camera* cam
  * per (view, Gaussian) entry with warp-shuffle + shared-memory reduction and device-scope atomics.
  * radii (optional): when given, only rows with radii > 0 are zero-filled before accumulation (rows of
  * culled entries are left untouched and are never read by gs_project_bwd); when NULL all C*N rows
- * are zero-filled.  N_total = C*N.
+ * are zero-filled.  N_total = C*N.  vis_mask (optional, takes precedence over radii): rows of its set bits are zero-filled.
  * out: dL_dmeans2d[C,N,2] dL_dconics[C,N,3] dL_dopacities[C,N] dL_drgbs[C,N,3]. */
 int gs_raster_bwd(const gs_config* cfg /*host*/, int32_t C, const gs_camera* cams /*host*/, int64_t N_total,
                   const int32_t* isect_vals, const int64_t* tile_ranges, const float* means2d,
                   const float* conics, const float* opacities, const float* rgbs, const float* bg /*host[3]*/,
                   const float* final_T, const int32_t* n_contrib, const float* dL_dimage /*[C,H,W,3]*/,
-                  const int32_t* radii /*optional*/, float* dL_dmeans2d, float* dL_dconics, float* dL_dopacities,
-                  float* dL_drgbs, void* stream);
+                  const int32_t* radii /*optional*/, const uint32_t* vis_mask /*optional*/, float* dL_dmeans2d, float* dL_dconics,
+                  float* dL_dopacities, float* dL_drgbs, void* stream);
 
 /* Measurement aid (not a step of the hot path; bench.py calls it outside the timed region to count the work the method
  * itself does): replays the per-pixel decisions of O-R1 over the tile lists and writes
@@ -150,10 +169,11 @@ int gs_raster_pair_stats(const gs_config* cfg /*host*/, int32_t C, const gs_came
  * accumulate == 1: rows of Gaussians visible in >= 1 view are added to, other rows untouched;
  * accumulate == 2: rows of Gaussians visible in >= 1 view are OVERWRITTEN, other rows untouched (the visible-only
  *                  gradient that goes with gs_adam_step_visible; C <= 16, else GS_ERR_UNSUPPORTED).
+ * Visibility comes from vis_mask when given (radii may then be NULL), else from radii > 0.
  * out: dL_dmeans[N,3] dL_dlog_scales[N,3] dL_dquats[N,4] dL_dopacity_logits[N] dL_dsh[N,K,3]. */
 int gs_project_bwd(const gs_config* cfg /*host*/, int64_t N, const float* means, const float* log_scales,
                    const float* quats, const float* opacity_logits, const float* sh, int32_t C,
-                   const gs_camera* cams /*host*/, const int32_t* radii, const float* dL_dmeans2d,
+                   const gs_camera* cams /*host*/, const int32_t* radii, const uint32_t* vis_mask /*optional*/, const float* dL_dmeans2d,
                    const float* dL_dconics, const float* dL_dopacities, const float* dL_drgbs,
                    float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats, float* dL_dopacity_logits,
                    float* dL_dsh, int32_t accumulate, void* stream);
@@ -204,16 +224,21 @@ int gs_gather_rows(int64_t N, int32_t row_floats, const float* src, const int32_
  * radii == NULL: every element is updated (16-byte accesses when all four pointers are 16-byte aligned).
  * radii != NULL ([C, N] int32 as saved by gs_project_fwd): only the rows of Gaussians with radius > 0 in at least one
  * of the C views are updated; parameter and moments of every other row are left untouched.
+ * running_max (optional, device float): *running_max = max(*running_max, every updated parameter value) -- pass the
+ * log-scale bound of gs_project_fwd with the log_scales array so that it stays an upper bound while training.
  * Asynchronous on `stream`.  Errors: GS_ERR_INVALID_ARGUMENT, GS_ERR_CUDA. */
 int gs_adam_step(int64_t N, int32_t row_floats, float* param, const float* grad, float* m, float* v, float lr, float beta1,
-                 float beta2, float eps, int32_t step, const int32_t* radii, int32_t C, void* stream);
+                 float beta2, float eps, int32_t step, const int32_t* radii, int32_t C, float* running_max /*optional*/, void* stream);
 
 /* The visible-only Adam step over n_arrays (<= 8) parameter arrays in ONE launch: the radii [C, N] are scanned once.
  * row_floats, params, grads, ms, vs: HOST arrays of n_arrays entries (row sizes; device pointers to [N, row] arrays).
- * Same update and same row selection as gs_adam_step with radii != NULL. */
+ * Same update and same row selection as gs_adam_step with radii != NULL.  vis_mask (optional, takes precedence over radii):
+ * the rows are those of Gaussians with a set bit in any view.  running_max (optional): as in gs_adam_step, over the updated
+ * values of array number max_array. */
 int gs_adam_step_visible(int64_t N, int32_t n_arrays, const int32_t* row_floats, float* const* params, const float* const* grads,
                          float* const* ms, float* const* vs, float lr, float beta1, float beta2, float eps, int32_t step,
-                         const int32_t* radii, int32_t C, void* stream);
+                         const int32_t* radii, const uint32_t* vis_mask /*optional*/, int32_t C, float* running_max /*optional*/,
+                         int32_t max_array, void* stream);
 
 #ifdef __cplusplus
 }

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libgsplat_b200.so")
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
-           "gs_raster_fwd", "gs_raster_bwd", "gs_raster_pair_stats", "gs_project_bwd", "gs_grad_zero_fill", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
+           "gs_raster_fwd", "gs_raster_bwd", "gs_raster_pair_stats", "gs_project_bwd", "gs_grad_zero_fill", "gs_log_scale_bound", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
 
 
 class gs_camera(C.Structure):
@@ -113,28 +113,47 @@ def _check(rc, where):
         raise GsError(rc, where)
 
 
+def vis_words(N):
+    """GS_VIS_WORDS(N): uint32 words per view of a visibility mask."""
+    return (int(N) + 511) // 512 * 16
+
+
+def _opt(t, dtype=None):
+    return _ptr(t, dtype) if t is not None else None
+
+
 def gs_project_fwd(cfg, means, log_scales, quats, opacity_logits, sh, cams, means2d, depths, conics, opacities, rgbs,
-                   radii, tiles_touched, stream=None):
+                   radii, tiles_touched, vis_mask=None, log_scale_bound=None, stream=None):
+    """``vis_mask``: optional int32 tensor [C, vis_words(N)] (uint32 bit patterns), written; ``log_scale_bound``: optional
+    float32 tensor of one element (see gs_log_scale_bound)."""
     import torch
     N = means.shape[0]
     rc = lib().gs_project_fwd(C.byref(cfg), C.c_int64(N), _ptr(means, torch.float32), _ptr(log_scales, torch.float32),
                               _ptr(quats, torch.float32), _ptr(opacity_logits, torch.float32), _ptr(sh, torch.float32),
                               C.c_int32(len(cams)), cams, _ptr(means2d, torch.float32), _ptr(depths, torch.float32),
                               _ptr(conics, torch.float32), _ptr(opacities, torch.float32), _ptr(rgbs, torch.float32),
-                              _ptr(radii, torch.int32), _ptr(tiles_touched), _stream(stream))
+                              _ptr(radii, torch.int32), _ptr(tiles_touched), _opt(vis_mask, torch.int32),
+                              _opt(log_scale_bound, torch.float32), _stream(stream))
     _check(rc, "gs_project_fwd")
+
+
+def gs_log_scale_bound(log_scales, bound, stream=None):
+    """bound (float32 tensor of one element) = max over all log-scales."""
+    import torch
+    rc = lib().gs_log_scale_bound(C.c_int64(log_scales.shape[0]), _ptr(log_scales, torch.float32), _ptr(bound, torch.float32), _stream(stream))
+    _check(rc, "gs_log_scale_bound")
 
 
 def gs_bin_tiles_workspace_bytes(cfg, N, cams, capacity_M):
     n = C.c_size_t(0)
-    rc = lib().gs_bin_tiles(C.byref(cfg), C.c_int64(N), C.c_int32(len(cams)), cams, None, None, None, None, C.byref(n),
+    rc = lib().gs_bin_tiles(C.byref(cfg), C.c_int64(N), C.c_int32(len(cams)), cams, None, None, None, None, None, C.byref(n),
                             C.c_int64(capacity_M), None, None, None, None, None, None)
     _check(rc, "gs_bin_tiles(size query)")
     return int(n.value)
 
 
 def gs_bin_tiles(cfg, N, cams, means2d, depths, radii, workspace, capacity_M, isect_keys, isect_vals, tile_ranges,
-                 M_dev=None, sync=True, stream=None):
+                 M_dev=None, sync=True, stream=None, vis_mask=None):
     """``isect_keys`` may be None (the 64-bit keys are then not materialised).
     Returns M (host int) when ``sync`` is true, else None (M is then only in ``M_dev``).
     Raises GsError(GS_ERR_CAPACITY) with ``.needed`` set when capacity_M is too small."""
@@ -142,7 +161,7 @@ def gs_bin_tiles(cfg, N, cams, means2d, depths, radii, workspace, capacity_M, is
     wb = C.c_size_t(workspace.numel() * workspace.element_size())
     m = C.c_int64(0)
     rc = lib().gs_bin_tiles(C.byref(cfg), C.c_int64(N), C.c_int32(len(cams)), cams, _ptr(means2d, torch.float32),
-                            _ptr(depths, torch.float32), _ptr(radii, torch.int32), _ptr(workspace), C.byref(wb),
+                            _ptr(depths, torch.float32), _ptr(radii, torch.int32), _opt(vis_mask, torch.int32), _ptr(workspace), C.byref(wb),
                             C.c_int64(capacity_M), _ptr(isect_keys) if isect_keys is not None else None,
                             _ptr(isect_vals, torch.int32),
                             _ptr(tile_ranges, torch.int64), _ptr(M_dev, torch.int64) if M_dev is not None else None,
@@ -186,13 +205,13 @@ def gs_raster_fwd(cfg, cams, isect_vals, tile_ranges, means2d, conics, opacities
 
 
 def gs_raster_bwd(cfg, cams, N_total, isect_vals, tile_ranges, means2d, conics, opacities, rgbs, bg, final_T, n_contrib,
-                  dL_dimage, radii, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs, stream=None):
+                  dL_dimage, radii, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs, stream=None, vis_mask=None):
     import torch
     rc = lib().gs_raster_bwd(C.byref(cfg), C.c_int32(len(cams)), cams, C.c_int64(N_total), _ptr(isect_vals, torch.int32),
                              _ptr(tile_ranges, torch.int64), _ptr(means2d, torch.float32), _ptr(conics, torch.float32),
                              _ptr(opacities, torch.float32), _ptr(rgbs, torch.float32), _bg(bg),
                              _ptr(final_T, torch.float32), _ptr(n_contrib, torch.int32), _ptr(dL_dimage, torch.float32),
-                             _ptr(radii, torch.int32) if radii is not None else None, _ptr(dL_dmeans2d, torch.float32),
+                             _opt(radii, torch.int32), _opt(vis_mask, torch.int32), _ptr(dL_dmeans2d, torch.float32),
                              _ptr(dL_dconics, torch.float32), _ptr(dL_dopacities, torch.float32),
                              _ptr(dL_drgbs, torch.float32), _stream(stream))
     _check(rc, "gs_raster_bwd")
@@ -210,12 +229,12 @@ def gs_raster_pair_stats(cfg, cams, isect_vals, tile_ranges, means2d, conics, op
 
 def gs_project_bwd(cfg, means, log_scales, quats, opacity_logits, sh, cams, radii, dL_dmeans2d, dL_dconics,
                    dL_dopacities, dL_drgbs, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh,
-                   accumulate=False, stream=None):
+                   accumulate=False, stream=None, vis_mask=None):
     import torch
     N = means.shape[0]
     rc = lib().gs_project_bwd(C.byref(cfg), C.c_int64(N), _ptr(means, torch.float32), _ptr(log_scales, torch.float32),
                               _ptr(quats, torch.float32), _ptr(opacity_logits, torch.float32), _ptr(sh, torch.float32),
-                              C.c_int32(len(cams)), cams, _ptr(radii, torch.int32), _ptr(dL_dmeans2d, torch.float32),
+                              C.c_int32(len(cams)), cams, _opt(radii, torch.int32), _opt(vis_mask, torch.int32), _ptr(dL_dmeans2d, torch.float32),
                               _ptr(dL_dconics, torch.float32), _ptr(dL_dopacities, torch.float32),
                               _ptr(dL_drgbs, torch.float32), _ptr(dL_dmeans, torch.float32),
                               _ptr(dL_dlog_scales, torch.float32), _ptr(dL_dquats, torch.float32),
@@ -305,7 +324,7 @@ def morton_sort(params, stream=None):
     return out, perm
 
 
-def gs_adam_step(param, grad, m, v, lr, beta1, beta2, eps, step, radii=None, stream=None):
+def gs_adam_step(param, grad, m, v, lr, beta1, beta2, eps, step, radii=None, stream=None, running_max=None):
     """In-place Adam step on one [N, ...] float32 array; with ``radii`` ([C, N] int32) only rows visible in >= 1 view."""
     import torch
     N = param.shape[0]
@@ -314,12 +333,14 @@ def gs_adam_step(param, grad, m, v, lr, beta1, beta2, eps, step, radii=None, str
     rc = lib().gs_adam_step(C.c_int64(N), C.c_int32(row), _ptr(param, torch.float32), _ptr(grad, torch.float32),
                             _ptr(m, torch.float32), _ptr(v, torch.float32), C.c_float(lr), C.c_float(beta1), C.c_float(beta2),
                             C.c_float(eps), C.c_int32(step), _ptr(radii, torch.int32) if radii is not None else None,
-                            C.c_int32(Cv), _stream(stream))
+                            C.c_int32(Cv), _opt(running_max, torch.float32), _stream(stream))
     _check(rc, "gs_adam_step")
 
 
-def gs_adam_step_visible(params, grads, ms, vs, lr, beta1, beta2, eps, step, radii, stream=None):
-    """Visible-only Adam step over several [N, ...] float32 arrays (lists of tensors) in one launch."""
+def gs_adam_step_visible(params, grads, ms, vs, lr, beta1, beta2, eps, step, radii, stream=None, vis_mask=None, n_views=None,
+                         running_max=None, max_array=0):
+    """Visible-only Adam step over several [N, ...] float32 arrays (lists of tensors) in one launch; the visible rows come
+    from ``vis_mask`` ([C, vis_words(N)]) when given, else from ``radii`` ([C, N])."""
     import torch
     n = len(params)
     N = params[0].shape[0]
@@ -327,6 +348,7 @@ def gs_adam_step_visible(params, grads, ms, vs, lr, beta1, beta2, eps, step, rad
     def ptrs(ts):
         return (C.c_void_p * n)(*[_ptr(t, torch.float32).value for t in ts])
     rc = lib().gs_adam_step_visible(C.c_int64(N), C.c_int32(n), rows, ptrs(params), ptrs(grads), ptrs(ms), ptrs(vs), C.c_float(lr),
-                                    C.c_float(beta1), C.c_float(beta2), C.c_float(eps), C.c_int32(step), _ptr(radii, torch.int32),
-                                    C.c_int32(int(radii.shape[0])), _stream(stream))
+                                    C.c_float(beta1), C.c_float(beta2), C.c_float(eps), C.c_int32(step), _opt(radii, torch.int32),
+                                    _opt(vis_mask, torch.int32), C.c_int32(int(n_views if n_views is not None else (vis_mask if radii is None else radii).shape[0])),
+                                    _opt(running_max, torch.float32), C.c_int32(int(max_array)), _stream(stream))
     _check(rc, "gs_adam_step_visible")

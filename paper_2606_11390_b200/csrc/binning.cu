@@ -464,8 +464,9 @@ __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs
 //                        bytes), lanes = bits when a mask word is expanded.
 constexpr int kMaskVec = 8;                                   // 16-byte loads per thread of visible_kernel
 constexpr int kMaskTile = kScanThreads * 4 * kMaskVec;        // 8 192 entries per block
-constexpr int kMaskWordsPerThread = 4;                        // compact_mask_kernel: 128 entries per thread
-constexpr int kMaskWordsPerBlock = kScanThreads * kMaskWordsPerThread;
+// compact_mask_kernel: WPT mask words per thread -- 16 (512 entries, one ticket per 131 072 entries) for the large sparse inputs
+// the mask exists for, 4 when the mask is small (a dense mask then costs at most 128 serial entries per thread)
+constexpr int64_t kMaskWideMinWords = 1 << 19;
 constexpr int64_t kMaskMinEntries = 1 << 24;                  // measured on B200: fused 50 us vs split 62 us at 10 M entries, 530 vs 265 us at 240 M
 
 __global__ void __launch_bounds__(kScanThreads) visible_kernel(const CompactArgs a, unsigned int* __restrict__ vmask, int64_t n_words) {
@@ -521,25 +522,37 @@ __global__ void __launch_bounds__(kScanThreads) visible_kernel(const CompactArgs
     }
 }
 
-__global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const CompactArgs a, const unsigned int* __restrict__ vmask, int64_t n_words) {
+// VIEWS = false: `vmask` is the flat mask over the entries e = c N + i written by visible_kernel (which has also added the
+// corner differences).  VIEWS = true: `vmask` is the per-view mask [C][wn] written by gs_project_fwd (bit i & 31 of word
+// c wn + (i >> 5)); the rectangle corners are added here, from the gathered means2d and radii of the visible entries.
+// wn is a multiple of 16 words and a thread owns 16 consecutive words, so a thread's words belong to one view.
+template <bool VIEWS, int WPT>
+__global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const CompactArgs a, const unsigned int* __restrict__ vmask, int64_t n_words,
+                                                                    int64_t wn) {
     __shared__ unsigned int s_ticket;
     __shared__ ChainScanSmem s_scan;
-    const int tid = threadIdx.x, lane = tid & 31;
+    __shared__ unsigned int s_w[WPT][kScanThreads];     // the thread's words, indexed dynamically in the expansion
+    const int tid = threadIdx.x;
     if (tid == 0) s_ticket = atomicAdd(&a.hdr->compact_ticket, 1u);
     __syncthreads();
     const int64_t tile = s_ticket;
-    const int64_t wi = tile * kMaskWordsPerBlock + (int64_t)tid * kMaskWordsPerThread;
-    unsigned int w[kMaskWordsPerThread];
-    if (wi + kMaskWordsPerThread <= n_words) {
-        const uint4 v = __ldg(reinterpret_cast<const uint4*>(vmask + wi));
-        w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
-    } else {
+    const int64_t wi = tile * (kScanThreads * WPT) + (int64_t)tid * WPT;
+    unsigned int cnt = 0, nzw = 0;      // set bits; which of the thread's words are non-zero
 #pragma unroll
-        for (int q = 0; q < kMaskWordsPerThread; ++q) w[q] = (wi + q < n_words) ? __ldg(vmask + wi + q) : 0u;
+    for (int v4 = 0; v4 < WPT / 4; ++v4) {
+        const int64_t w4 = wi + 4 * v4;
+        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+        if (w4 + 4 <= n_words) {
+            v = __ldg(reinterpret_cast<const uint4*>(vmask + w4));
+        } else {
+            if (w4 < n_words) v.x = __ldg(vmask + w4);
+            if (w4 + 1 < n_words) v.y = __ldg(vmask + w4 + 1);
+            if (w4 + 2 < n_words) v.z = __ldg(vmask + w4 + 2);
+        }
+        s_w[4 * v4][tid] = v.x; s_w[4 * v4 + 1][tid] = v.y; s_w[4 * v4 + 2][tid] = v.z; s_w[4 * v4 + 3][tid] = v.w;
+        cnt += (unsigned int)(__popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w));
+        nzw |= ((v.x ? 1u : 0u) | (v.y ? 2u : 0u) | (v.z ? 4u : 0u) | (v.w ? 8u : 0u)) << (4 * v4);
     }
-    unsigned int cnt = 0;
-#pragma unroll
-    for (int q = 0; q < kMaskWordsPerThread; ++q) cnt += (unsigned int)__popc(w[q]);
     unsigned long long be, bt;
     const unsigned long long pos = block_chained_scan((unsigned long long)cnt, a.status, tile, s_scan, be, bt);
     if (tid == 0 && tile == (int64_t)a.n_blocks - 1) {
@@ -547,41 +560,60 @@ __global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const Compac
         a.hdr->V = V < (unsigned long long)a.vcap ? V : (unsigned long long)a.vcap;
     }
     if (bt == 0) return;
-    // expansion: the warp takes the non-zero words of its lanes one at a time, lane = bit (C * N < 2^31: 32-bit ranks)
+    // expansion: every thread walks the set bits of its own words, four entries per round so that the gathers of a
+    // round are in flight together; its ranks start at the exclusive prefix `pos` (C * N < 2^31: 32-bit ranks)
     const unsigned int n32 = (unsigned int)a.N;
-    const unsigned int lt_mask = (1u << lane) - 1u;
-    const int64_t warp_word0 = wi - (int64_t)lane * kMaskWordsPerThread;
-    unsigned int pre = (unsigned int)pos;
-#pragma unroll
-    for (int q = 0; q < kMaskWordsPerThread; ++q) {
-        unsigned int nz = __ballot_sync(0xffffffffu, w[q] != 0u);
-        while (nz) {
-            // four words per round: the depth gathers of a round are in flight together
+    int64_t e_first = wi << 5;      // entry of bit 0 of this thread's first word
+    unsigned int my_view = 0;
+    if (VIEWS) {
+        my_view = (unsigned int)(wi / wn);
+        e_first = (int64_t)my_view * a.N + ((wi - (int64_t)my_view * wn) << 5);
+    }
+    const int sx = a.gx + 1, sy = a.gy + 1;
+    int* const grid = VIEWS ? a.tdiff + (int64_t)my_view * ((int64_t)sx * sy) : nullptr;
+    unsigned int r = (unsigned int)pos;
+    while (nzw) {
+        const int q = __ffs(nzw) - 1;
+        nzw &= nzw - 1;
+        unsigned int m = s_w[q][tid];
+        const int64_t eq = e_first + (q << 5);
+        while (m) {
             int64_t e[4];
-            unsigned int r[4];
             bool on[4];
             float dep[4];
+            float2 uv[4];
+            int rad[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const bool have = nz != 0u;            // warp-uniform
-                const int s = have ? __ffs(nz) - 1 : 0;
-                nz &= nz - 1;                          // 0 stays 0
-                const unsigned int word = __shfl_sync(0xffffffffu, w[q], s);
-                const unsigned int p0 = __shfl_sync(0xffffffffu, pre, s);
-                on[u] = have && ((word >> lane) & 1u);
-                e[u] = ((warp_word0 + (int64_t)s * kMaskWordsPerThread + q) << 5) + lane;
-                r[u] = p0 + (unsigned int)__popc(word & lt_mask);
-                on[u] = on[u] && (int64_t)r[u] < a.vcap;
-                dep[u] = on[u] ? __ldg(a.depths + e[u]) : 0.0f;
+                on[u] = m != 0u;
+                e[u] = eq + (on[u] ? __ffs(m) - 1 : 0);
+                m &= m - 1;                            // 0 stays 0
+                dep[u] = (on[u] && (int64_t)(r + u) < a.vcap) ? __ldg(a.depths + e[u]) : 0.0f;
+                if (VIEWS && on[u]) {
+                    uv[u] = __ldg(reinterpret_cast<const float2*>(a.means2d) + e[u]);
+                    rad[u] = __ldg(a.radii + e[u]);
+                }
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u)
                 if (on[u]) {
-                    a.ckeys[r[u]] = ((unsigned long long)((unsigned int)e[u] / n32) << 32) | (unsigned long long)__float_as_uint(dep[u]);
-                    a.cvals[r[u]] = (int)e[u];
+                    if (VIEWS) {
+                        // the rectangle's corner differences (every visible entry, also beyond the compact capacity: M must be exact)
+                        int x0, x1, y0, y1;
+                        tile_rect(uv[u].x, uv[u].y, rad[u], a.gx, a.gy, x0, x1, y0, y1);
+                        atomicAdd(grid + y0 * sx + x0, 1);
+                        atomicAdd(grid + y0 * sx + x1, -1);
+                        atomicAdd(grid + y1 * sx + x0, -1);
+                        atomicAdd(grid + y1 * sx + x1, 1);
+                    }
+                    if ((int64_t)r < a.vcap) {
+                        const unsigned int view = VIEWS ? my_view : (unsigned int)e[u] / n32;
+                        a.ckeys[r] = ((unsigned long long)view << 32) | (unsigned long long)__float_as_uint(dep[u]);
+                        a.cvals[r] = (int)e[u];
+                    }
+                    ++r;
                 }
         }
-        pre += (unsigned int)__popc(w[q]);
     }
 }
 
@@ -742,6 +774,7 @@ __global__ void __launch_bounds__(kScanThreads) offsets_kernel(const OffsetsArgs
     const int tid = threadIdx.x;
     const unsigned long long V = a.hdr->V;
     const int64_t n_blocks = (int64_t)((V + kScanTile - 1) / kScanTile);
+    if ((int64_t)blockIdx.x >= n_blocks) return;     // (the grid is sized for the capacity; only n_blocks blocks take a ticket)
     if (tid == 0) s_ticket = atomicAdd(&a.hdr->offs_ticket, 1u);
     __syncthreads();
     const int64_t tile = s_ticket;
@@ -841,6 +874,7 @@ __global__ void __launch_bounds__(kSortThreads) onesweep_kernel(const SweepArgs 
     const unsigned long long M = *a.count;
     const int64_t n = M < (unsigned long long)a.capacity ? (int64_t)M : a.capacity;
     const int64_t n_tiles = (n + kSortTile - 1) / kSortTile;
+    if ((int64_t)blockIdx.x >= n_tiles) return;       // (the grid is sized for the capacity; only n_tiles blocks take a ticket)
     if (tid == 0) sm.tile = atomicAdd(a.ticket, 1u);
     for (int k = tid; k < kSortWarps * kRadix; k += kSortThreads) (&sm.warp_hist[0][0])[k] = 0;
     __syncthreads();
@@ -1257,7 +1291,7 @@ static int launch_tile_sweep(const TileSweepArgs& a, int64_t capacity, cudaStrea
 using namespace gs;
 
 extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs_camera* cams, const float* means2d,
-                            const float* depths, const int32_t* radii, void* workspace, size_t* workspace_bytes,
+                            const float* depths, const int32_t* radii, const uint32_t* vis_mask, void* workspace, size_t* workspace_bytes,
                             int64_t capacity_M, uint64_t* isect_keys, int32_t* isect_vals, int64_t* tile_ranges,
                             int64_t* M_dev, int64_t* M_out, void* stream) {
     int rc = check_cfg(cfg);
@@ -1280,7 +1314,7 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
     }
     if (workspace_bytes && *workspace_bytes < w.total) return GS_ERR_INVALID_ARGUMENT;
     if (!isect_vals || !tile_ranges || !aligned(workspace, 256) || !aligned(isect_keys, 8)) return GS_ERR_INVALID_ARGUMENT;
-    if (N > 0 && (!means2d || !depths || !radii || !aligned(means2d, 8) || !aligned(radii, 16))) return GS_ERR_INVALID_ARGUMENT;
+    if (N > 0 && (!means2d || !depths || !radii || !aligned(means2d, 8) || !aligned(radii, 16) || !aligned(vis_mask, 16))) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t st = (cudaStream_t)stream;
     int tile_bits = 1, view_bits = 0;
     while ((1LL << tile_bits) < (int64_t)C * tiles) ++tile_bits;
@@ -1316,15 +1350,25 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
         a.tdiff = tdiff;
         a.hdr = hdr; a.status = status_at(w.off_compact_status);
         a.n_blocks = (unsigned int)n_blocks;
-        if (n_entries >= kMaskMinEntries) {
+        if (vis_mask) {
+            // the caller's visibility mask (written by gs_project_fwd): ordered scan over the mask, no pass over the radii
+            const int64_t wn = GS_VIS_WORDS(N), n_words = (int64_t)C * wn;
+            if (n_words >= kMaskWideMinWords) {
+                a.n_blocks = (unsigned int)((n_words + kScanThreads * 16 - 1) / (kScanThreads * 16));
+                compact_mask_kernel<true, 16><<<a.n_blocks, kScanThreads, 0, st>>>(a, vis_mask, n_words, wn);
+            } else {
+                a.n_blocks = (unsigned int)((n_words + kScanThreads * 4 - 1) / (kScanThreads * 4));
+                compact_mask_kernel<true, 4><<<a.n_blocks, kScanThreads, 0, st>>>(a, vis_mask, n_words, wn);
+            }
+        } else if (n_entries >= kMaskMinEntries) {
             // large inputs: streaming visibility mask, then the ordered scan over the mask
             unsigned int* vmask = reinterpret_cast<unsigned int*>(ws + w.off_vmask);
             const int64_t n_words = (n_entries + 31) / 32;
             visible_kernel<<<(unsigned)((n_entries + kMaskTile - 1) / kMaskTile), kScanThreads, 0, st>>>(a, vmask, n_words);
             rc = launch_status();
             if (rc) return rc;
-            a.n_blocks = (unsigned int)((n_words + kMaskWordsPerBlock - 1) / kMaskWordsPerBlock);
-            compact_mask_kernel<<<a.n_blocks, kScanThreads, 0, st>>>(a, vmask, n_words);
+            a.n_blocks = (unsigned int)((n_words + kScanThreads * 16 - 1) / (kScanThreads * 16));
+            compact_mask_kernel<false, 16><<<a.n_blocks, kScanThreads, 0, st>>>(a, vmask, n_words, 0);
         } else switch (cvec) {
             case 8: compact_kernel<8><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
             case 4: compact_kernel<4><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;

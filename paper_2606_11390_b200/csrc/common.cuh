@@ -24,6 +24,9 @@ struct DevCam {
     float ox, oy, oz;
     float wnorm2;              // upper bound of |W|_2^2 (1 for a rigid transform): max absolute row sum of W W^T
     int32_t width, height, gx, gy;
+    // linear lateral cull with a scene-wide scale bound s (project.cu, phase A): a Gaussian whose tile rectangle can be
+    // non-empty satisfies  fx |t_x - t_z (gx 8 - cx) / fx| <= lat_k1x t_z + lat_k2 s  (same in y)
+    float lat_cx, lat_cy, lat_k1x, lat_k1y, lat_k2, lat_abs;
 };
 
 struct CamBatch {
@@ -55,7 +58,27 @@ inline DevCam make_devcam(const gs_camera& c) {
     d.width = c.width; d.height = c.height;
     d.gx = (c.width + kTile - 1) / kTile;
     d.gy = (c.height + kTile - 1) / kTile;
+    d.lat_cx = d.lat_cy = d.lat_k1x = d.lat_k1y = d.lat_k2 = d.lat_abs = 0.0f;      // set by set_lateral_bound
     return d;
+}
+
+// Constants of the linear lateral cull.  A visible entry has a non-empty tile rectangle, hence |u - 8 gx| <= 8 gx + 16 + r
+// with r <= extent sqrt(lambda_max) + 1, lambda_max <= 2 (L + dilation) + sqrt(0.1), L <= s^2 |J|_F^2 |W|_2^2 and
+// |J|_F^2 <= (fx^2 (1 + lim_x^2) + fy^2 (1 + lim_y^2)) / t_z^2 =: jf0 / t_z^2.  With sqrt(a + b) <= sqrt(a) + sqrt(b) and
+// u = fx t_x / t_z + cx this gives  fx |t_x - t_z (8 gx - cx) / fx| <= t_z (8 gx + 17 + extent sqrt(2 dil + 0.32)) + extent s sqrt(2 jf0);
+// 0.2 % and 4 pixels of slack cover the fp32 rounding of both sides; the rounding of t = W p + tau itself (three products of
+// size <= |p| <= |t| + |tau| each) adds lat_abs = 16 eps |tau| max(fx, fy) (the |t| part is inside the 0.2 %).
+inline void set_lateral_bound(DevCam& d, float extent, float dilation) {
+    const float dil = dilation > 0.0f ? dilation : 0.0f;
+    const float pad = 17.0f + extent * sqrtf(2.0f * dil + 0.32f) + 4.0f;
+    d.lat_cx = (8.0f * (float)d.gx - d.cx) / d.fx;
+    d.lat_cy = (8.0f * (float)d.gy - d.cy) / d.fy;
+    d.lat_k1x = (8.0f * (float)d.gx + pad) * 1.002f;
+    d.lat_k1y = (8.0f * (float)d.gy + pad) * 1.002f;
+    const float jf0 = (d.fx * d.fx * (1.0f + d.lim_x * d.lim_x) + d.fy * d.fy * (1.0f + d.lim_y * d.lim_y)) * d.wnorm2;
+    d.lat_k2 = extent * sqrtf(2.0f * jf0) * 1.002f;
+    const float tn = sqrtf(d.tau[0] * d.tau[0] + d.tau[1] * d.tau[1] + d.tau[2] * d.tau[2]);
+    d.lat_abs = 16.0f * 5.9604645e-8f * tn * (d.fx > d.fy ? d.fx : d.fy);
 }
 
 inline bool finite_f(float x) { return x == x && x - x == 0.0f; }

@@ -29,6 +29,9 @@ struct ProjFwdArgs {
     int32_t* radii; uint32_t* tiles;
     float dilation, extent;
     int32_t vec_in, vec_out;   // 16-byte vector access allowed on means / on radii+tiles rows
+    uint32_t* vmask;           // optional visibility mask [C][wn] (bit i & 31 of word i >> 5); replaces the dense zero-fill of radii / tiles
+    int64_t wn;                // mask words per view, GS_VIS_WORDS(N)
+    const float* ls_bound;     // optional device scalar >= every log-scale: the streaming phase then culls laterally as well
 };
 
 constexpr int kProjThreads = 128;   // P1 block
@@ -122,6 +125,7 @@ __device__ __forceinline__ void project_fwd_one(const ProjFwdArgs& a, const CamB
             a.conics[3 * e] = m.c * inv; a.conics[3 * e + 1] = -m.b * inv; a.conics[3 * e + 2] = m.a * inv;
             a.radii[e] = radius;
             a.tiles[e] = nt;
+            if (a.vmask) atomicOr(a.vmask + (int64_t)c * a.wn + (i >> 5), 1u << (unsigned)(i & 31));
         }
     }
     if (!vis) return;
@@ -151,11 +155,24 @@ __device__ __forceinline__ void project_fwd_one(const ProjFwdArgs& a, const CamB
     }
 }
 
-// Conservative screen-space pre-cull from the mean and the largest scale alone (no rotation needed):
+// Conservative screen-space pre-cull from the mean and an upper bound of the largest scale alone (no rotation needed):
 // |Sigma'| <= (s_max |J|_F |W|_2)^2 =: L, so lambda_max <= 2 (L + dilation) + sqrt(0.1) and the integer radius
 // is at most rb = extent sqrt(that) + 1.  A view whose tile rectangle must then be empty (mean more
-// than rb outside the 16-pixel-padded image) is dropped from the mask; phase B would cull it at step 8
+// than rb outside the 16-pixel-padded image) is dropped; phase B would cull it at step 8
 // anyway, so no result changes.  Non-finite intermediates fail every comparison and keep the view.
+// smax2 = (upper bound of the scale)^2; tz = the camera-space depth already computed by the caller.
+__device__ __forceinline__ bool lateral_keep(const ProjFwdArgs& a, const DevCam& cam, float smax2, float px, float py, float pz, float tz) {
+    const float tx = cam.W[0] * px + cam.W[1] * py + cam.W[2] * pz + cam.tau[0];
+    const float ty = cam.W[3] * px + cam.W[4] * py + cam.W[5] * pz + cam.tau[1];
+    const float rz = 1.0f / tz;
+    const float u = cam.fx * tx * rz + cam.cx, v = cam.fy * ty * rz + cam.cy;
+    const float jf = (cam.fx * cam.fx * (1.0f + cam.lim_x * cam.lim_x) + cam.fy * cam.fy * (1.0f + cam.lim_y * cam.lim_y)) * cam.wnorm2 * rz * rz;
+    const float L = smax2 * jf;
+    const float rb = a.extent * sqrtf(2.0f * (L + fmaxf(a.dilation, 0.0f)) + 0.32f) * 1.001f + 3.0f;
+    const float w16 = (float)(cam.gx * kTile), h16 = (float)(cam.gy * kTile);
+    const bool out = (u + rb + 16.0f < 0.0f) || (u - rb > w16) || (v + rb + 16.0f < 0.0f) || (v - rb > h16);
+    return !out;
+}
 __device__ __forceinline__ uint32_t lateral_precull(const ProjFwdArgs& a, const CamBatch& cams, float lmax, float px, float py, float pz,
                                                     uint32_t zmask) {
     const float smax = expf(lmax);
@@ -163,38 +180,98 @@ __device__ __forceinline__ uint32_t lateral_precull(const ProjFwdArgs& a, const 
     for (int c = 0; c < a.C; ++c) {
         if (!((zmask >> c) & 1u)) continue;
         const DevCam& cam = cams.cam[c];
+        const float tz = cam.W[6] * px + cam.W[7] * py + cam.W[8] * pz + cam.tau[2];
+        if (lateral_keep(a, cam, smax * smax, px, py, pz, tz)) keep |= 1u << c;
+    }
+    return keep;
+}
+
+// linear lateral test of one Gaussian against the views of zmask (set_lateral_bound in common.cuh): ALU only
+__device__ __forceinline__ uint32_t lateral_linear(const ProjFwdArgs& a, const CamBatch& cams, float smax_all, float px, float py, float pz,
+                                                   uint32_t zmask) {
+    uint32_t keep = 0;
+    for (int c = 0; c < a.C; ++c) {
+        if (!((zmask >> c) & 1u)) continue;
+        const DevCam& cam = cams.cam[c];
         const float tx = cam.W[0] * px + cam.W[1] * py + cam.W[2] * pz + cam.tau[0];
         const float ty = cam.W[3] * px + cam.W[4] * py + cam.W[5] * pz + cam.tau[1];
         const float tz = cam.W[6] * px + cam.W[7] * py + cam.W[8] * pz + cam.tau[2];
-        const float rz = 1.0f / tz;
-        const float u = cam.fx * tx * rz + cam.cx, v = cam.fy * ty * rz + cam.cy;
-        const float jf = (cam.fx * cam.fx * (1.0f + cam.lim_x * cam.lim_x) + cam.fy * cam.fy * (1.0f + cam.lim_y * cam.lim_y)) * cam.wnorm2 * rz * rz;
-        const float L = smax * smax * jf;
-        const float rb = a.extent * sqrtf(2.0f * (L + fmaxf(a.dilation, 0.0f)) + 0.32f) * 1.001f + 3.0f;
-        const float w16 = (float)(cam.gx * kTile), h16 = (float)(cam.gy * kTile);
-        const bool out = (u + rb + 16.0f < 0.0f) || (u - rb > w16) || (v + rb + 16.0f < 0.0f) || (v - rb > h16);
+        const float kk = fmaf(cam.lat_k2, smax_all, cam.lat_abs);
+        const bool out = (cam.fx * fabsf(tx - tz * cam.lat_cx) > fmaf(cam.lat_k1x, tz, kk)) ||
+                         (cam.fy * fabsf(ty - tz * cam.lat_cy) > fmaf(cam.lat_k1y, tz, kk));
         if (!out) keep |= 1u << c;
     }
     return keep;
 }
 
+// pop up to 32 entries from the top of `src` (one per lane), hand (index, mask, mean) of this lane's entry to `f`, which
+// returns the new view mask; entries with a non-zero mask are pushed onto `dst`
+template <typename Src, typename Dst, typename F>
+__device__ __forceinline__ void stack_filter(Src& src, int& cnt_src, Dst& dst, int& cnt_dst, int lane, F f) {
+    const int n = cnt_src < 32 ? cnt_src : 32;
+    uint32_t idx[1] = {0u}, msk[1] = {0u};
+    float m[3] = {0.f, 0.f, 0.f};
+    if (lane < n) {
+        const int p = cnt_src - n + lane;
+        idx[0] = src.idx[p];
+        m[0] = src.xyz[0][p]; m[1] = src.xyz[1][p]; m[2] = src.xyz[2][p];
+        msk[0] = f(idx[0], src.msk[p], m);
+    }
+    cnt_src -= n;
+    __syncwarp();      // the popped entries have been read
+    warp_push<1>(idx, msk, m, dst, cnt_dst, lane);
+    __syncwarp();
+}
+
+// Stages of a warp (each runs with full warps whenever 32 items are waiting, the later the stage the higher its priority;
+// at the end of the input the stacks are drained):
+//   A   streaming: means of a chunk -> near/far test of every view; zero radii / tiles_touched (or the mask words)  -> s1
+//   B0a (only with the scene-wide scale bound) linear lateral test, ALU only                                        -> s1b
+//   B0b the Gaussian's own largest scale (12-byte gather) -> conservative screen-space pre-cull                     -> s2
+//   B1  full projection; SH only if visible somewhere
 template <int DEG, int ITEMS>
 __global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const ProjFwdArgs a, const __grid_constant__ CamBatch cams) {
     constexpr int CHUNK = 32 * ITEMS;                   // Gaussians per warp and phase-A step
     constexpr int WARPS = kProjThreads / 32;
     __shared__ WarpStack<32 + CHUNK, true> s1_all[WARPS];   // Gaussians inside some view's depth range
-    __shared__ WarpStack<64, true> s2_all[WARPS];           // survivors of the screen-space pre-cull
+    __shared__ WarpStack<64, true> s1b_all[WARPS];          // ... that pass the linear lateral test with the scene-wide scale bound
+    __shared__ WarpStack<64, true> s2_all[WARPS];           // survivors of the pre-cull with the Gaussian's own largest scale
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpStack<32 + CHUNK, true>& s1 = s1_all[warp];
+    WarpStack<64, true>& s1b = s1b_all[warp];
     WarpStack<64, true>& s2 = s2_all[warp];
     const int64_t n_chunks = (a.N + CHUNK - 1) / CHUNK;
     const int64_t stride = (int64_t)gridDim.x * WARPS;
     int64_t chunk = (int64_t)blockIdx.x * WARPS + warp;
-    int cnt1 = 0, cnt2 = 0;    // warp-uniform stack heights
+    int cnt1 = 0, cnt1b = 0, cnt2 = 0;    // warp-uniform stack heights
+    float smax_all = -1.0f;
+    if (a.ls_bound) smax_all = expf(__ldg(a.ls_bound));
+    const bool use_bound = smax_all >= 0.0f && smax_all < kInfF;      // false for a NaN bound as well: nothing is dropped then
     while (true) {
-        // ---- phase A (streaming) until a full warp of depth candidates is waiting: means -> near/far
-        //      test of every view; zero radii / tiles_touched of the chunk
-        while (cnt1 < 32 && chunk < n_chunks) {
+        const bool more = chunk < n_chunks;
+        if (cnt2 >= 32 || (cnt2 > 0 && !more && cnt1 == 0 && cnt1b == 0)) {
+            // ---- B1: full projection of up to one survivor per lane
+            const int n = cnt2 < 32 ? cnt2 : 32;
+            if (lane < n) {
+                const int p = cnt2 - n + lane;
+                project_fwd_one<DEG>(a, cams, (int64_t)s2.idx[p], s2.msk[p], s2.xyz[0][p], s2.xyz[1][p], s2.xyz[2][p]);
+            }
+            cnt2 -= n;
+            __syncwarp();          // the popped entries have been read
+        } else if (cnt1b >= 32 || (cnt1b > 0 && !more && cnt1 == 0)) {
+            // ---- B0b: screen-space pre-cull with the Gaussian's own largest scale -> s2
+            stack_filter(s1b, cnt1b, s2, cnt2, lane, [&](uint32_t i, uint32_t zmask, const float* m) {
+                const float* ls = a.log_scales + 3 * (int64_t)i;
+                const float lmax = fmaxf(__ldg(ls), fmaxf(__ldg(ls + 1), __ldg(ls + 2)));
+                return lateral_precull(a, cams, lmax, m[0], m[1], m[2], zmask);
+            });
+        } else if (cnt1 >= 32 || (cnt1 > 0 && !more)) {
+            // ---- B0a: linear lateral test with the scene-wide bound (a plain move without one) -> s1b
+            stack_filter(s1, cnt1, s1b, cnt1b, lane, [&](uint32_t, uint32_t zmask, const float* m) {
+                return use_bound ? lateral_linear(a, cams, smax_all, m[0], m[1], m[2], zmask) : zmask;
+            });
+        } else if (more) {
+            // ---- A (streaming): means -> near/far test of every view; zero radii / tiles_touched (or the mask words) of the chunk
             const int64_t i0 = chunk * CHUNK + (int64_t)lane * ITEMS;
             float m[3 * ITEMS];
             const bool full = i0 + ITEMS <= a.N;
@@ -221,7 +298,12 @@ __global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const Proj
                     if (tz > zn && tz < zf) msk[k] |= 1u << c;
                 }
                 const int64_t e0 = (int64_t)c * a.N + i0;
-                if (ITEMS % 4 == 0 && a.vec_out && full) {
+                if (a.vmask) {
+                    // the chunk's ITEMS mask words of this view (and the row's padding words behind the last chunk)
+                    uint32_t* row = a.vmask + (int64_t)c * a.wn;
+                    if (lane < ITEMS) row[chunk * ITEMS + lane] = 0u;
+                    if (chunk == n_chunks - 1 && n_chunks * ITEMS + lane < a.wn) row[n_chunks * ITEMS + lane] = 0u;
+                } else if (ITEMS % 4 == 0 && a.vec_out && full) {
 #pragma unroll
                     for (int k = 0; k < ITEMS / 4; ++k) {
                         reinterpret_cast<int4*>(a.radii + e0)[k] = make_int4(0, 0, 0, 0);
@@ -241,38 +323,9 @@ __global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const Proj
             warp_push<ITEMS>(idx, msk, m, s1, cnt1, lane);
             chunk += stride;
             __syncwarp();      // pushes visible to the warp; its zero-fill is ordered before phase B's stores
+        } else {
+            break;
         }
-        // ---- phase B0: screen-space pre-cull of up to one depth candidate per lane -> stack 2
-        if (cnt1 > 0 && cnt2 <= 32) {
-            const int n = cnt1 < 32 ? cnt1 : 32;
-            uint32_t idx[1] = {0u}, msk[1] = {0u};
-            float m[3] = {0.f, 0.f, 0.f};
-            if (lane < n) {
-                const int p = cnt1 - n + lane;
-                idx[0] = s1.idx[p];
-                m[0] = s1.xyz[0][p]; m[1] = s1.xyz[1][p]; m[2] = s1.xyz[2][p];
-                const float* ls = a.log_scales + 3 * (int64_t)idx[0];
-                const float lmax = fmaxf(__ldg(ls), fmaxf(__ldg(ls + 1), __ldg(ls + 2)));
-                msk[0] = lateral_precull(a, cams, lmax, m[0], m[1], m[2], s1.msk[p]);
-            }
-            cnt1 -= n;
-            __syncwarp();      // the popped entries have been read
-            warp_push<1>(idx, msk, m, s2, cnt2, lane);
-            __syncwarp();
-            if (cnt2 < 32 && (cnt1 > 0 || chunk < n_chunks)) continue;
-        }
-        if (cnt2 == 0) {
-            if (cnt1 == 0 && chunk >= n_chunks) break;
-            continue;
-        }
-        // ---- phase B1: full projection of up to one survivor per lane
-        const int n = cnt2 < 32 ? cnt2 : 32;
-        if (lane < n) {
-            const int p = cnt2 - n + lane;
-            project_fwd_one<DEG>(a, cams, (int64_t)s2.idx[p], s2.msk[p], s2.xyz[0][p], s2.xyz[1][p], s2.xyz[2][p]);
-        }
-        cnt2 -= n;
-        __syncwarp();          // the popped entries have been read
     }
 }
 
@@ -288,6 +341,8 @@ struct ProjBwdArgs {
     int32_t accumulate;
     int32_t vec_in, vec_out;   // 16-byte vector access allowed on the radii rows / on the five gradient arrays
     int32_t prezeroed;         // the gradient arrays were zero-filled by zero_fill_kernel: phase A only reads the radii
+    const uint32_t* vmask;     // optional visibility mask [C][wn] written by gs_project_fwd: read instead of the radii
+    int64_t wn;
 };
 
 template <int DEG>
@@ -493,8 +548,11 @@ __device__ __forceinline__ void zero_span(float* __restrict__ p, int64_t count, 
     }
 }
 
-template <int DEG, int ITEMS>
+// MASK: visibility comes from the bit mask of gs_project_fwd; a lane then takes one mask word (32 Gaussians) per view,
+// ITEMS = 32, and only the non-zero words are expanded (lane = bit).
+template <int DEG, int ITEMS, bool MASK = false>
 __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjBwdArgs a, const __grid_constant__ CamBatch cams) {
+    static_assert(!MASK || ITEMS == 32, "mask variant: one word per lane");
     constexpr int CHUNK = 32 * ITEMS;                   // Gaussians per warp and phase-A step
     constexpr int WARPS = kBwdThreads / 32;
     constexpr int K3 = 3 * (DEG + 1) * (DEG + 1);
@@ -511,6 +569,21 @@ __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjB
         while (cnt < 32 && chunk < n_chunks) {
             const int64_t base = chunk * CHUNK;
             const int64_t i0 = base + (int64_t)lane * ITEMS;
+            if constexpr (MASK) {
+                const int64_t word = chunk * 32 + lane;                      // this lane's word of every view's row
+                uint32_t any = 0;
+                if (word < a.wn)
+                    for (int c = 0; c < a.C; ++c) any |= __ldg(a.vmask + (int64_t)c * a.wn + word);
+                unsigned int nz = __ballot_sync(0xffffffffu, any != 0u);
+                while (nz) {
+                    const int sl = __ffs(nz) - 1;
+                    nz &= nz - 1;
+                    const int64_t ws = chunk * 32 + sl;
+                    uint32_t idx1[1] = {(uint32_t)(ws * 32 + lane)}, vis1[1] = {0u};
+                    for (int c = 0; c < a.C; ++c) vis1[0] |= ((__ldg(a.vmask + (int64_t)c * a.wn + ws) >> lane) & 1u) << c;   // (same address for all lanes)
+                    warp_push<1>(idx1, vis1, nullptr, stk, cnt, lane);
+                }
+            } else {
             const bool full = i0 + ITEMS <= a.N;
             uint32_t idx[ITEMS], vis[ITEMS];
 #pragma unroll
@@ -530,6 +603,10 @@ __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjB
                         if (i0 + k < a.N && __ldg(a.radii + e0 + k) > 0) vis[k] |= 1u << c;
                 }
             }
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) idx[k] = (uint32_t)(i0 + k);
+            warp_push<ITEMS>(idx, vis, nullptr, stk, cnt, lane);
+            }
             if (!a.accumulate && !a.prezeroed) {
                 const int64_t n = (a.N - base) < CHUNK ? (a.N - base) : CHUNK;
                 const bool vec = a.vec_out != 0;
@@ -539,9 +616,6 @@ __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjB
                 zero_span(a.d_quats + base * 4, n * 4, vec, lane);
                 zero_span(a.d_logits + base, n, vec, lane);
             }
-#pragma unroll
-            for (int k = 0; k < ITEMS; ++k) idx[k] = (uint32_t)(i0 + k);
-            warp_push<ITEMS>(idx, vis, nullptr, stk, cnt, lane);
             chunk += stride;
             __syncwarp();      // pushes visible to the warp; its zero-fill is ordered before phase B's stores
         }
@@ -567,6 +641,53 @@ __global__ void __launch_bounds__(256) zero_fill_kernel(float* __restrict__ p, i
     for (int k = 0; k < 4; ++k)
         if (i0 + k * 256 < n4) p4[i0 + k * 256] = zero;
     if (blockIdx.x == 0 && threadIdx.x < 4 && (n4 << 2) + threadIdx.x < count) p[(n4 << 2) + threadIdx.x] = 0.f;
+}
+
+// max over all log-scales (gs_log_scale_bound): 16-byte loads, warp shuffle, one atomic per warp
+__global__ void __launch_bounds__(256) log_scale_max_kernel(const float* __restrict__ ls, int64_t n, int vec, float* __restrict__ out) {
+    float m = -3.0e38f;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (vec) {
+        const int64_t n4 = n >> 2;
+        for (int64_t k = t0; k < n4; k += stride) {
+            const float4 v = __ldg(reinterpret_cast<const float4*>(ls) + k);
+            m = fmaxf(m, fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w)));
+        }
+        for (int64_t k = (n4 << 2) + t0; k < n; k += stride) m = fmaxf(m, __ldg(ls + k));
+    } else {
+        for (int64_t k = t0; k < n; k += stride) m = fmaxf(m, __ldg(ls + k));
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0 && m > -3.0e38f) {
+        if (m >= 0.0f) atomicMax(reinterpret_cast<int*>(out), __float_as_int(m));
+        else atomicMin(reinterpret_cast<unsigned int*>(out), __float_as_uint(m));
+    }
+}
+__global__ void set_float_kernel(float* p, float v) { *p = v; }
+
+// The same zero-fill as ONE launch with a small persistent grid (2 blocks of 256 threads per SM, 8 x 16-byte stores per
+// thread and round): made to run on a second stream UNDERNEATH other kernels (gs_grad_zero_fill).  A full-size grid would
+// take every free block slot of the SMs ahead of the kernels it is supposed to overlap with; two resident blocks per SM
+// keep enough stores in flight for the full store bandwidth and leave the rest of the SM to the rasterisation kernels.
+struct ZeroFillArgs {
+    float* p[5];
+    int64_t count[5];
+};
+__global__ void __launch_bounds__(256) zero_fill_persistent_kernel(const ZeroFillArgs a) {
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    const int64_t stride = (int64_t)gridDim.x * 2048;
+#pragma unroll 1
+    for (int k = 0; k < 5; ++k) {
+        float4* p4 = reinterpret_cast<float4*>(a.p[k]);
+        const int64_t n4 = a.count[k] >> 2;
+        for (int64_t i0 = (int64_t)blockIdx.x * 2048 + threadIdx.x; i0 < n4; i0 += stride) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (i0 + u * 256 < n4) p4[i0 + u * 256] = zero;
+        }
+        if (blockIdx.x == 0 && threadIdx.x < 4 && (n4 << 2) + threadIdx.x < a.count[k]) a.p[k][(n4 << 2) + threadIdx.x] = 0.f;
+    }
 }
 
 // persistent grid: resident blocks of the kernel, or fewer when there are fewer chunks
@@ -597,8 +718,14 @@ template <int DEG>
 int launch_bwd(const ProjBwdArgs& a, const CamBatch& cb, cudaStream_t st) {
     const int sms = sm_count();
     constexpr int warps = kBwdThreads / 32;
-    if (a.prezeroed) {
-        // phase A only scans the radii: 16 Gaussians per lane keep 4 C 16-byte loads in flight per lane
+    if (a.vmask) {
+        const int64_t chunks = (a.N + 1023) / 1024;
+        project_bwd_kernel<DEG, 32, true><<<persistent_grid(project_bwd_kernel<DEG, 32, true>, kBwdThreads, (chunks + warps - 1) / warps, sms),
+                                            kBwdThreads, 0, st>>>(a, cb);
+        return launch_status();
+    }
+    if (a.prezeroed || a.accumulate) {
+        // phase A only scans the radii (or the visibility mask): 16 Gaussians per lane keep 4 C 16-byte loads in flight per lane
         // (only when every resident warp still gets >= 8 such chunks; else the narrower variants below)
         const int64_t scan = (a.N + 32 * 16 - 1) / (32 * 16);
         const unsigned scan_grid = persistent_grid(project_bwd_kernel<DEG, 16>, kBwdThreads, (scan + warps - 1) / warps, sms);
@@ -625,7 +752,8 @@ using namespace gs;
 extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* means, const float* log_scales,
                               const float* quats, const float* opacity_logits, const float* sh, int32_t C,
                               const gs_camera* cams, float* means2d, float* depths, float* conics, float* opacities,
-                              float* rgbs, int32_t* radii, uint32_t* tiles_touched, void* stream) {
+                              float* rgbs, int32_t* radii, uint32_t* tiles_touched, uint32_t* vis_mask,
+                              const float* log_scale_bound, void* stream) {
     int rc = check_cfg(cfg);
     if (rc) return rc;
     rc = check_cams(C, cams);
@@ -635,13 +763,17 @@ extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* mean
     if (!means || !log_scales || !quats || !opacity_logits || !sh || !means2d || !depths || !conics || !opacities ||
         !rgbs || !radii || !tiles_touched)
         return GS_ERR_INVALID_ARGUMENT;
-    if (!aligned(quats, 16) || !aligned(sh, 16) || !aligned(means2d, 8) || !aligned(means, 4)) return GS_ERR_INVALID_ARGUMENT;
+    if (!aligned(quats, 16) || !aligned(sh, 16) || !aligned(means2d, 8) || !aligned(means, 4) || !aligned(vis_mask, 16)) return GS_ERR_INVALID_ARGUMENT;
     if ((int64_t)C * N >= (1LL << 31)) return GS_ERR_UNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
+    const int64_t wn = GS_VIS_WORDS(N);
     for (int c0 = 0; c0 < C; c0 += kMaxCamsPerLaunch) {
         const int nc = C - c0 < kMaxCamsPerLaunch ? C - c0 : kMaxCamsPerLaunch;
         CamBatch cb;
-        for (int c = 0; c < nc; ++c) cb.cam[c] = make_devcam(cams[c0 + c]);
+        for (int c = 0; c < nc; ++c) {
+            cb.cam[c] = make_devcam(cams[c0 + c]);
+            set_lateral_bound(cb.cam[c], cfg->extent, cfg->dilation);
+        }
         ProjFwdArgs a;
         a.N = N; a.C = nc;
         a.means = means; a.log_scales = log_scales; a.quats = quats; a.logits = opacity_logits; a.sh = sh;
@@ -651,6 +783,7 @@ extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* mean
         a.dilation = cfg->dilation; a.extent = cfg->extent;
         a.vec_in = aligned(means, 16) ? 1 : 0;
         a.vec_out = (aligned(a.radii, 16) && aligned(a.tiles, 16) && (N % 4 == 0 || nc == 1)) ? 1 : 0;
+        a.vmask = vis_mask ? vis_mask + (int64_t)c0 * wn : nullptr; a.wn = wn; a.ls_bound = log_scale_bound;
         switch (cfg->sh_degree) {
             case 0: rc = launch_fwd<0>(a, cb, st); break;
             case 1: rc = launch_fwd<1>(a, cb, st); break;
@@ -660,6 +793,19 @@ extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* mean
         if (rc) return rc;
     }
     return GS_OK;
+}
+
+extern "C" int gs_log_scale_bound(int64_t N, const float* log_scales, float* bound, void* stream) {
+    if (N < 1 || !log_scales || !bound || !aligned(bound, 4)) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    set_float_kernel<<<1, 1, 0, st>>>(bound, -3.0e38f);
+    const int64_t n = 3 * N;
+    int64_t blocks = (n / 4 + 255) / 256;
+    const int64_t cap = (int64_t)sm_count() * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    log_scale_max_kernel<<<(unsigned)blocks, 256, 0, st>>>(log_scales, n, aligned(log_scales, 16) ? 1 : 0, bound);
+    return launch_status();
 }
 
 // dense zero-fill of the five gradient arrays (16-byte stores when the pointer allows it)
@@ -684,12 +830,20 @@ extern "C" int gs_grad_zero_fill(int64_t N, int32_t sh_degree, float* dL_dmeans,
     if (N < 0 || sh_degree < 0 || sh_degree > 3) return GS_ERR_INVALID_ARGUMENT;
     if (N == 0) return GS_OK;
     if (!dL_dmeans || !dL_dlog_scales || !dL_dquats || !dL_dopacity_logits || !dL_dsh) return GS_ERR_INVALID_ARGUMENT;
+    if (aligned(dL_dmeans, 16) && aligned(dL_dlog_scales, 16) && aligned(dL_dquats, 16) && aligned(dL_dopacity_logits, 16) && aligned(dL_dsh, 16)) {
+        const int64_t K3 = 3 * (int64_t)(sh_degree + 1) * (sh_degree + 1);
+        ZeroFillArgs a;
+        a.p[0] = dL_dsh; a.p[1] = dL_dquats; a.p[2] = dL_dmeans; a.p[3] = dL_dlog_scales; a.p[4] = dL_dopacity_logits;
+        a.count[0] = K3 * N; a.count[1] = 4 * N; a.count[2] = 3 * N; a.count[3] = 3 * N; a.count[4] = N;
+        zero_fill_persistent_kernel<<<(unsigned)(2 * sm_count()), 256, 0, (cudaStream_t)stream>>>(a);
+        return launch_status();
+    }
     return zero_fill_all(N, sh_degree, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh, (cudaStream_t)stream);
 }
 
 extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* means, const float* log_scales,
                               const float* quats, const float* opacity_logits, const float* sh, int32_t C,
-                              const gs_camera* cams, const int32_t* radii, const float* dL_dmeans2d,
+                              const gs_camera* cams, const int32_t* radii, const uint32_t* vis_mask, const float* dL_dmeans2d,
                               const float* dL_dconics, const float* dL_dopacities, const float* dL_drgbs,
                               float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats, float* dL_dopacity_logits,
                               float* dL_dsh, int32_t accumulate, void* stream) {
@@ -699,7 +853,7 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
     if (rc) return rc;
     if (N < 0) return GS_ERR_INVALID_ARGUMENT;
     if (N == 0) return GS_OK;
-    if (!means || !log_scales || !quats || !opacity_logits || !sh || !radii || !dL_dmeans2d || !dL_dconics ||
+    if (!means || !log_scales || !quats || !opacity_logits || !sh || (!radii && !vis_mask) || !dL_dmeans2d || !dL_dconics ||
         !dL_dopacities || !dL_drgbs || !dL_dmeans || !dL_dlog_scales || !dL_dquats || !dL_dopacity_logits || !dL_dsh)
         return GS_ERR_INVALID_ARGUMENT;
     if (!aligned(quats, 16) || !aligned(sh, 16) || !aligned(dL_dquats, 16) || !aligned(dL_dsh, 16) || !aligned(dL_dmeans2d, 8))
@@ -716,7 +870,8 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
         a.N = N; a.C = nc;
         a.means = means; a.log_scales = log_scales; a.quats = quats; a.logits = opacity_logits; a.sh = sh;
         const int64_t off = (int64_t)c0 * N;
-        a.radii = radii + off;
+        a.radii = radii ? radii + off : nullptr;
+        a.vmask = vis_mask ? vis_mask + (int64_t)c0 * GS_VIS_WORDS(N) : nullptr; a.wn = GS_VIS_WORDS(N);
         a.g_means2d = dL_dmeans2d + 2 * off; a.g_conics = dL_dconics + 3 * off;
         a.g_opacities = dL_dopacities + off; a.g_rgbs = dL_drgbs + 3 * off;
         a.d_means = dL_dmeans; a.d_log_scales = dL_dlog_scales; a.d_quats = dL_dquats;
@@ -726,7 +881,7 @@ extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* mean
         // accumulate == 2 ("visible rows only"): the rows of Gaussians visible in this batch are overwritten, all other rows
         // are left untouched (no dense zero-fill: the caller's optimizer reads only visible rows, gs_adam_step_visible)
         a.accumulate = (accumulate == 1 || c0 > 0) ? 1 : 0;
-        a.vec_in = (aligned(a.radii, 16) && (N % 4 == 0 || nc == 1)) ? 1 : 0;
+        a.vec_in = (a.radii && aligned(a.radii, 16) && (N % 4 == 0 || nc == 1)) ? 1 : 0;
         a.vec_out = (aligned(dL_dmeans, 16) && aligned(dL_dlog_scales, 16) && aligned(dL_dquats, 16) &&
                      aligned(dL_dopacity_logits, 16) && aligned(dL_dsh, 16)) ? 1 : 0;
         a.prezeroed = (accumulate == 2) ? 1 : 0;

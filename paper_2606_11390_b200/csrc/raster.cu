@@ -570,6 +570,31 @@ __global__ void __launch_bounds__(256) zero_visible_rows_kernel(int64_t n, const
     }
 }
 
+// the same from the visibility mask [C][wn] of gs_project_fwd: a lane loads four mask words (16 bytes), the warp then walks
+// the non-zero words with lane = bit, so that the rows zeroed together are neighbours in memory
+__global__ void __launch_bounds__(256) zero_masked_rows_kernel(int64_t N, int64_t wn, int64_t n_words, const uint32_t* __restrict__ vmask,
+                                                               float* g_means2d, float* g_conics, float* g_opacities, float* g_rgbs) {
+    const int lane = threadIdx.x & 31;
+    const int64_t wi = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 4;              // n_words = C * wn is a multiple of 16
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (wi < n_words) v = __ldg(reinterpret_cast<const uint4*>(vmask + wi));
+    if (!__any_sync(0xffffffffu, (v.x | v.y | v.z | v.w) != 0u)) return;
+    const int64_t view = wi < n_words ? wi / wn : 0;                               // (a lane's four words belong to one view)
+    const int64_t e_lane = view * N + ((wi - view * wn) << 5);                     // entry of bit 0 of this lane's first word
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        uint32_t nz = __ballot_sync(0xffffffffu, w[q] != 0u);
+        while (nz) {
+            const int s = __ffs(nz) - 1;
+            nz &= nz - 1;
+            const uint32_t wd = __shfl_sync(0xffffffffu, w[q], s);
+            const unsigned int e_lo = __shfl_sync(0xffffffffu, (unsigned int)e_lane, s);   // C * N < 2^31
+            if ((wd >> lane) & 1u) zero_row((int64_t)e_lo + 32 * q + lane, g_means2d, g_conics, g_opacities, g_rgbs);
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256) l1_loss_kernel(int64_t n, const float* __restrict__ image, const float* __restrict__ target,
                                                       float* __restrict__ dL, float* loss_sum, float inv_n) {
     float acc = 0.f;
@@ -685,8 +710,8 @@ extern "C" int gs_raster_fwd(const gs_config* cfg, int32_t C, const gs_camera* c
 extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* cams, int64_t N_total,
                              const int32_t* isect_vals, const int64_t* tile_ranges, const float* means2d, const float* conics,
                              const float* opacities, const float* rgbs, const float* bg, const float* final_T,
-                             const int32_t* n_contrib, const float* dL_dimage, const int32_t* radii, float* dL_dmeans2d,
-                             float* dL_dconics, float* dL_dopacities, float* dL_drgbs, void* stream) {
+                             const int32_t* n_contrib, const float* dL_dimage, const int32_t* radii, const uint32_t* vis_mask,
+                             float* dL_dmeans2d, float* dL_dconics, float* dL_dopacities, float* dL_drgbs, void* stream) {
     RasterArgs a;
     int rc = fill_args(cfg, C, cams, isect_vals, tile_ranges, means2d, conics, opacities, rgbs, bg, a);
     if (rc) return rc;
@@ -695,7 +720,14 @@ extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* c
         return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t st = (cudaStream_t)stream;
     if (N_total > 0) {
-        if (radii) {
+        if (vis_mask) {
+            if (N_total % C != 0 || !aligned(vis_mask, 16)) return GS_ERR_INVALID_ARGUMENT;
+            const int64_t N = N_total / C, wn = GS_VIS_WORDS(N), n_words = (int64_t)C * wn;
+            zero_masked_rows_kernel<<<(unsigned)((n_words / 4 + 255) / 256), 256, 0, st>>>(N, wn, n_words, vis_mask, dL_dmeans2d, dL_dconics,
+                                                                                          dL_dopacities, dL_drgbs);
+            rc = launch_status();
+            if (rc) return rc;
+        } else if (radii) {
             zero_visible_rows_kernel<<<(unsigned)((N_total + 2047) / 2048), 256, 0, st>>>(N_total, radii, aligned(radii, 16) ? 1 : 0,
                                                                                            dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs);
             rc = launch_status();

@@ -17,9 +17,18 @@ from . import binding as B
 class SplatStep:
     """Device-resident state for a batch of C views of one scene."""
 
-    def __init__(self, scene, device="cuda:0", capacity_M=None, upload=True, want_keys=False):
+    MASK_MIN_ENTRIES = 1 << 23
+
+    def __init__(self, scene, device="cuda:0", capacity_M=None, upload=True, want_keys=False, use_mask=None):
         # want_keys: also materialise the sorted 64-bit (tile | depth) keys; no later stage reads them
+        # use_mask: visibility travels between the stages as a bit mask [C, GS_VIS_WORDS(N)] written by P1 (no dense
+        #   zero-fill of radii / tiles_touched, no pass over the C N radii in binning, R2, P5 and the visible-only Adam step)
+        #   and P1 culls laterally with the scene-wide log-scale bound; False = every stage scans the dense radii
         self.want_keys = bool(want_keys)
+        n_entries = len(scene["cameras"]) * int(scene["means"].shape[0])
+        # None = automatic: the mask pays when the dense radii[C, N] are large (measured: city 6.74 -> 6.07 ms per step, block
+        # 1.67 -> 1.63; at 4 M entries and below -- room, object -- the radii sit in the L2 and the mask gains nothing)
+        self.use_mask = bool(use_mask) if use_mask is not None else n_entries >= self.MASK_MIN_ENTRIES
         self.device = torch.device(device)
         self.scene_name = scene.get("name", "")
         self.cams_host = scene["cameras"]
@@ -51,6 +60,9 @@ class SplatStep:
         self.rgbs = torch.empty((Cn, N, 3), dtype=f32, device=d)
         self.radii = torch.empty((Cn, N), dtype=torch.int32, device=d)
         self.tiles_touched = torch.empty((Cn, N), dtype=torch.int32, device=d)   # uint32 bit patterns
+        self.vis_mask = torch.empty((Cn, B.vis_words(N)), dtype=torch.int32, device=d) if self.use_mask else None
+        self.ls_bound = torch.empty((1,), dtype=f32, device=d) if self.use_mask else None
+        self._ls_bound_valid = False
         self.g_means2d = torch.empty_like(self.means2d)
         self.g_conics = torch.empty_like(self.conics)
         self.g_opacities = torch.empty_like(self.opacities)
@@ -88,10 +100,35 @@ class SplatStep:
         self.target = t.to(self.device).contiguous()
 
     # -- stages -------------------------------------------------------------------------
+    def refresh_log_scale_bound(self):
+        """Recompute the scene-wide log-scale bound (after the parameters were replaced; the Adam step keeps it current)."""
+        if self.use_mask:
+            B.gs_log_scale_bound(self.params["log_scales"], self.ls_bound)
+            self._ls_bound_valid = True
+
     def project_fwd(self):
         p = self.params
+        if self.use_mask and not self._ls_bound_valid:
+            self.refresh_log_scale_bound()
         B.gs_project_fwd(self.cfg, p["means"], p["log_scales"], p["quats"], p["opacity_logits"], p["sh"], self.cams,
-                         self.means2d, self.depths, self.conics, self.opacities, self.rgbs, self.radii, self.tiles_touched)
+                         self.means2d, self.depths, self.conics, self.opacities, self.rgbs, self.radii, self.tiles_touched,
+                         vis_mask=self.vis_mask, log_scale_bound=self.ls_bound)
+
+    def visible(self):
+        """Harness-side view of the visibility as a bool tensor [C, N] (torch ops; not part of the hot path)."""
+        if not self.use_mask:
+            return self.radii > 0
+        bits = torch.arange(32, device=self.device, dtype=torch.int32)
+        m = ((self.vis_mask.unsqueeze(-1) >> bits) & 1).to(torch.bool).reshape(self.C, -1)
+        return m[:, : self.N]
+
+    def radii_dense(self):
+        """Harness-side: radii with the entries of culled Gaussians set to 0 (in mask mode P1 leaves them unwritten)."""
+        return torch.where(self.visible(), self.radii, torch.zeros_like(self.radii)) if self.use_mask else self.radii
+
+    def tiles_dense(self):
+        """Harness-side: tiles_touched (uint32 bit patterns in an int32 tensor) with the entries of culled Gaussians set to 0."""
+        return torch.where(self.visible(), self.tiles_touched, torch.zeros_like(self.tiles_touched)) if self.use_mask else self.tiles_touched
 
     def check_overflow(self, wait=False):
         """Looks at the record count of the last asynchronous binning call (without blocking unless ``wait``).  When it
@@ -122,7 +159,8 @@ class SplatStep:
         while True:
             try:
                 m = B.gs_bin_tiles(self.cfg, self.N, self.cams, self.means2d, self.depths, self.radii, self.workspace,
-                                   self.capacity_M, self.isect_keys, self.isect_vals, self.tile_ranges, self.M_dev, sync)
+                                   self.capacity_M, self.isect_keys, self.isect_vals, self.tile_ranges, self.M_dev, sync,
+                                   vis_mask=self.vis_mask)
                 if sync:
                     self.M = m
                 elif self._M_event is None:
@@ -154,13 +192,13 @@ class SplatStep:
     def raster_bwd(self):
         B.gs_raster_bwd(self.cfg, self.cams, self.C * self.N, self.isect_vals, self.tile_ranges, self.means2d, self.conics,
                         self.opacities, self.rgbs, self.bg, self.final_T, self.n_contrib, self.dL_dimage, self.radii,
-                        self.g_means2d, self.g_conics, self.g_opacities, self.g_rgbs)
+                        self.g_means2d, self.g_conics, self.g_opacities, self.g_rgbs, vis_mask=self.vis_mask)
 
     def project_bwd(self, accumulate=False):
         p, g = self.params, self.grads
         B.gs_project_bwd(self.cfg, p["means"], p["log_scales"], p["quats"], p["opacity_logits"], p["sh"], self.cams,
                          self.radii, self.g_means2d, self.g_conics, self.g_opacities, self.g_rgbs, g["means"],
-                         g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], accumulate)
+                         g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], accumulate, vis_mask=self.vis_mask)
 
     def adam(self, mode="dense", lr=0.0, beta1=0.9, beta2=0.999, eps=1e-15):
         """One fused Adam step over the five parameter arrays (gs_adam_step); ``mode`` "dense" (the paper's _fused_adam_,
@@ -175,10 +213,13 @@ class SplatStep:
         if mode == "sparse":
             ks = self.param_names
             B.gs_adam_step_visible([self.params[k] for k in ks], [self.grads[k] for k in ks], [self._adam_m[k] for k in ks],
-                                   [self._adam_v[k] for k in ks], lr, beta1, beta2, eps, self._adam_t, self.radii)
+                                   [self._adam_v[k] for k in ks], lr, beta1, beta2, eps, self._adam_t,
+                                   None if self.use_mask else self.radii, vis_mask=self.vis_mask, n_views=self.C,
+                                   running_max=self.ls_bound, max_array=ks.index("log_scales"))
             return
         for k in self.param_names:
-            B.gs_adam_step(self.params[k], self.grads[k], self._adam_m[k], self._adam_v[k], lr, beta1, beta2, eps, self._adam_t)
+            B.gs_adam_step(self.params[k], self.grads[k], self._adam_m[k], self._adam_v[k], lr, beta1, beta2, eps, self._adam_t,
+                           running_max=self.ls_bound if k == "log_scales" else None)
 
     # -- whole passes -------------------------------------------------------------------
     def forward(self, sync=True):
@@ -190,36 +231,36 @@ class SplatStep:
         self.raster_bwd()
         self.project_bwd()
 
-    # From this many Gaussians the dense zero-fill of the gradient arrays (236 N bytes at SH degree 3, the largest single
-    # item of a city step) runs on a second stream underneath the rasterisation kernels, and P5 accumulates into it.
-    OVERLAP_ZERO_FILL_MIN_N = 1 << 22
-
-    def fork_grad_zero_fill(self):
-        """Start the dense zero-fill of the gradient arrays on the side stream (after everything enqueued so far)."""
+    # The dense zero-fill of the gradient arrays (236 N bytes at SH degree 3, the largest single item of a city step) can run
+    # on a second stream underneath the rasterisation kernels, with P5 accumulating into it.  Measured on B200 (city, 60 M):
+    # no gain -- 6.09 / 6.22 ms per step with the overlap (full-size grid / two persistent blocks per SM) against 6.07 ms
+    # without: the 7.6 TB/s store stream saturates the HBM and the L2, and the gather latency of the rasterisation kernels
+    # (R1 0.83 -> 2.8 ms while it runs) grows by what the overlap saves.  Off by default; kept for measurement.
+    def fork_grad_zero_fill(self, t0=None, t1=None):
+        """Start the dense zero-fill of the gradient arrays on the side stream (after everything enqueued so far);
+        ``t0``/``t1``: optional timing events recorded around it on the side stream."""
         main = torch.cuda.current_stream(self.device)
         if getattr(self, "_zf_stream", None) is None:
-            self._zf_stream = torch.cuda.Stream(self.device, priority=0)
+            self._zf_stream = torch.cuda.Stream(self.device, priority=self.ZERO_FILL_STREAM_PRIORITY)
             self._zf_fork = torch.cuda.Event()
             self._zf_join = torch.cuda.Event()
-            self._zf_t0 = torch.cuda.Event(enable_timing=True)
-            self._zf_t1 = torch.cuda.Event(enable_timing=True)
         self._zf_fork.record(main)
         zs = self._zf_stream
         zs.wait_event(self._zf_fork)
         g = self.grads
-        self._zf_t0.record(zs)
+        if t0 is not None:
+            t0.record(zs)
         B.gs_grad_zero_fill(self.cfg.sh_degree, g["means"], g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], stream=zs)
-        self._zf_t1.record(zs)
+        if t1 is not None:
+            t1.record(zs)
         self._zf_join.record(zs)
 
     def join_grad_zero_fill(self):
         torch.cuda.current_stream(self.device).wait_event(self._zf_join)
 
-    def step(self, sync=False, overlap_zero_fill=None):
-        """One forward+backward pass with the L1 loss against ``self.target``.  ``overlap_zero_fill`` (default: from
-        OVERLAP_ZERO_FILL_MIN_N Gaussians): zero-fill the gradients on a second stream while R1, the loss and R2 run."""
-        if overlap_zero_fill is None:
-            overlap_zero_fill = self.N >= self.OVERLAP_ZERO_FILL_MIN_N
+    def step(self, sync=False, overlap_zero_fill=False):
+        """One forward+backward pass with the L1 loss against ``self.target``.  ``overlap_zero_fill``: zero-fill the gradients
+        on a second stream while R1, the loss and R2 run (see above: no gain measured)."""
         self.project_fwd()
         self.bin_tiles(sync)
         if overlap_zero_fill:
@@ -286,6 +327,7 @@ class SplatStep:
         main.wait_event(self._in_ready[k])
         if self._in_params[k] is not None:
             self.params = self._in_params[k]
+            self._ls_bound_valid = False          # new parameter values: the log-scale bound is recomputed (one reduction)
         self.target = self._in_target[k]
         self.forward(sync=False)
         self.l1_loss()
@@ -306,7 +348,7 @@ class SplatStep:
         view_bits = int(np.ceil(np.log2(self.C))) if self.C > 1 else 0
         depth_passes = 4 + (view_bits + 7) // 8
         tile_passes = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
-        compact = 2 if self.C * self.N >= (1 << 24) else 1          # visibility mask + scan over the mask for large inputs
+        compact = 1 if self.use_mask else (2 if self.C * self.N >= (1 << 24) else 1)   # radii mode, large inputs: visibility mask + scan over it
         p5 = 6 if self.N >= (1 << 22) else 1                         # dense zero-fill as five streaming launches for large N
         loss = 2 if getattr(self, "loss_mode", "l1") == "l1ssim" else 1
         return (loss - 1) + (p5 - 1) + 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

@@ -59,30 +59,30 @@ def test_host_side_validation_needs_no_gpu(cuda_lib):
     cfg = cuda_lib.default_config()
     # null pointers with N > 0
     rc = lib.gs_project_fwd(C.byref(cfg), C.c_int64(10), None, None, None, None, None, C.c_int32(1), cams,
-                            None, None, None, None, None, None, None, None)
+                            None, None, None, None, None, None, None, None, None, None)
     assert rc == cuda_lib.GS_ERR_INVALID_ARGUMENT
     # bad SH degree, bad tile
     bad = cuda_lib.default_config(sh_degree=4)
     assert lib.gs_project_fwd(C.byref(bad), C.c_int64(0), None, None, None, None, None, C.c_int32(1), cams,
-                              None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_INVALID_ARGUMENT
+                              None, None, None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_INVALID_ARGUMENT
     bad = cuda_lib.default_config(tile=8)
     assert lib.gs_project_fwd(C.byref(bad), C.c_int64(0), None, None, None, None, None, C.c_int32(1), cams,
-                              None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_UNSUPPORTED
+                              None, None, None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_UNSUPPORTED
     # N < 0, C out of range
     assert lib.gs_project_fwd(C.byref(cfg), C.c_int64(-1), None, None, None, None, None, C.c_int32(1), cams,
-                              None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_INVALID_ARGUMENT
+                              None, None, None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_INVALID_ARGUMENT
     assert lib.gs_project_fwd(C.byref(cfg), C.c_int64(0), None, None, None, None, None, C.c_int32(0), cams,
-                              None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_INVALID_ARGUMENT
+                              None, None, None, None, None, None, None, None, None, None) == cuda_lib.GS_ERR_INVALID_ARGUMENT
     # N == 0 is a no-op
     assert lib.gs_project_fwd(C.byref(cfg), C.c_int64(0), None, None, None, None, None, C.c_int32(1), cams,
-                              None, None, None, None, None, None, None, None) == cuda_lib.GS_OK
+                              None, None, None, None, None, None, None, None, None, None) == cuda_lib.GS_OK
     # workspace size query grows with capacity and is 256-byte granular
     a = cuda_lib.gs_bin_tiles_workspace_bytes(cfg, 1000, cams, 10_000)
     b = cuda_lib.gs_bin_tiles_workspace_bytes(cfg, 1000, cams, 1_000_000)
     assert b > a > 10_000 * 12 and a % 256 == 0
     # capacity beyond the 2^30 record limit
     n = C.c_size_t(0)
-    assert lib.gs_bin_tiles(C.byref(cfg), C.c_int64(10), C.c_int32(1), cams, None, None, None, None, C.byref(n),
+    assert lib.gs_bin_tiles(C.byref(cfg), C.c_int64(10), C.c_int32(1), cams, None, None, None, None, None, C.byref(n),
                             C.c_int64(1 << 30), None, None, None, None, None, None) == cuda_lib.GS_ERR_UNSUPPORTED
 
 

@@ -84,7 +84,7 @@ def test_city_60m(B, oracle, city60, far):
     tiles = gx * gy
 
     # ---- row subset for the per-Gaussian stages
-    vis_t = st.radii > 0                                             # [C, N] on the device
+    vis_t = st.visible()                                             # [C, N] on the device
     anyvis_t = vis_t.any(dim=0)
     V_sum, V_any = int(vis_t.sum().item()), int(anyvis_t.sum().item())
     stride = 4001
@@ -95,8 +95,10 @@ def test_city_60m(B, oracle, city60, far):
     rows_t = torch.from_numpy(rows).to(st.device)
     sub = {k: np.ascontiguousarray(sc[k][rows]) for k in ("means", "log_scales", "quats", "opacity_logits", "sh")}
     ref = oracle.project_fwd(cfg, sub["means"], sub["log_scales"], sub["quats"], sub["opacity_logits"], sub["sh"], cams)
-    got = {k: getattr(st, k)[:, rows_t].cpu().numpy() for k in ("means2d", "depths", "conics", "opacities", "rgbs", "radii")}
-    got["tiles_touched"] = st.tiles_touched[:, rows_t].cpu().numpy().view(np.uint32)
+    got = {k: getattr(st, k)[:, rows_t].cpu().numpy() for k in ("means2d", "depths", "conics", "opacities", "rgbs")}
+    zero = torch.zeros((), dtype=torch.int32, device=st.device)
+    got["radii"] = torch.where(vis_t[:, rows_t], st.radii[:, rows_t], zero).cpu().numpy()       # culled entries are unwritten in mask mode
+    got["tiles_touched"] = torch.where(vis_t[:, rows_t], st.tiles_touched[:, rows_t], zero).cpu().numpy().view(np.uint32)
     p1 = check_project_fwd_arrays(got, ref, "city-60M", dict(sc, means=sub["means"], log_scales=sub["log_scales"], quats=sub["quats"]))
     del ref
 
@@ -108,7 +110,7 @@ def test_city_60m(B, oracle, city60, far):
     assert np.all(ranges[~nz] == 0)
     starts = ranges[nz, 0]
     assert starts[0] == 0 and np.array_equal(starts[1:], ranges[nz, 1][:-1]) and ranges[nz, 1][-1] == M
-    assert int(st.tiles_touched.to(torch.int64).sum().item()) == M
+    assert int(torch.where(vis_t, st.tiles_touched, zero).to(torch.int64).sum().item()) == M
     vals_t = st.isect_vals[:M].to(torch.int64)
     d_sorted = st.depths.reshape(-1)[vals_t]
     inside = torch.ones((M,), dtype=torch.bool, device=st.device)

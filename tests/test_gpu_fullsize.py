@@ -149,8 +149,9 @@ def record(entry, fname="parity_fullsize.jsonl"):
 
 
 def check_project_fwd(st, ref, name, sc):
-    got = {k: getattr(st, k).cpu().numpy() for k in ("means2d", "depths", "conics", "opacities", "rgbs", "radii")}
-    got["tiles_touched"] = st.tiles_touched.cpu().numpy().view(np.uint32)
+    got = {k: getattr(st, k).cpu().numpy() for k in ("means2d", "depths", "conics", "opacities", "rgbs")}
+    got["radii"] = st.radii_dense().cpu().numpy()           # (mask mode: radii of culled entries are unwritten)
+    got["tiles_touched"] = st.tiles_dense().cpu().numpy().view(np.uint32)
     check_project_fwd_arrays(got, ref, name, sc)
     return got
 

@@ -560,7 +560,7 @@ def test_project_bwd_visible_rows_only(B, name, sc):
         v.fill_(123.0)
     st.project_bwd(accumulate=2)
     torch.cuda.synchronize()
-    vis = (st.radii > 0).any(dim=0)
+    vis = st.visible().any(dim=0)
     assert 0 < int(vis.sum()) < st.N
     for k, v in st.grads.items():
         assert torch.equal(v[vis], dense[k][vis]), k

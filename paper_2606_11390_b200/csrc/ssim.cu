@@ -9,6 +9,8 @@
 //   ssim_grad_kernel    halo tiles of the three maps -> their window means (the adjoint of a symmetric, zero-padded
 //                       correlation is the same correlation) -> dL/dx = g_mu + 2 x g_11 + y g_12 + L1 term.
 // Algorithmic HBM bytes per pixel and channel: read x, y (8), write 3 maps (12); read 3 maps, x, y (20), write dL (4).
+#include <cuda.h>      // CUtensorMap (types only: the encoder is looked up at run time, the library does not link libcuda)
+
 #include "common.cuh"
 
 namespace gs {
@@ -19,6 +21,11 @@ constexpr int kSsimWin = 2 * kSsimR + 1;
 constexpr int kSsimHalo = kSsimTile + 2 * kSsimR;       // 26
 constexpr int kSsimRow = kSsimHalo * 3;                 // floats per halo row (3 interleaved channels)
 constexpr int kSsimRowPad = kSsimRow + 1;               // odd stride: column walks of the vertical pass spread over banks
+constexpr int kSsimRowTma = 80;                         // TMA halo rows: 80 floats = 320 bytes (the box width must be a multiple of 16 bytes)
+constexpr int kSsimTmaOff = 1;                          // ... starting one float left of the halo: the innermost start coordinate must be a
+                                                        // multiple of 16 bytes (measured on B200: illegal instruction otherwise), and
+                                                        // 3 (16 bx - 5) - 1 = 48 bx - 16 is
+constexpr unsigned kSsimTmaBytes = kSsimHalo * kSsimRowTma * 4;
 constexpr float kSsimC1 = 0.01f * 0.01f;
 constexpr float kSsimC2 = 0.03f * 0.03f;
 
@@ -35,7 +42,8 @@ struct SsimArgs {
 // rows i0-5 .. i0+20, pixels j0-5 .. j0+20 of view v, all three channels, zero outside the image; a warp takes whole
 // rows (78 contiguous floats: three coalesced requests).  The elements go global -> shared with cp.async (4 bytes each,
 // zero-filled outside the image), so every load of every halo tile of a block is in flight before the first wait.
-__device__ __forceinline__ void load_halo_async(const float* __restrict__ img, int v, int i0, int j0, int H, int W, float (*s)[kSsimRowPad]) {
+template <int ROW>
+__device__ __forceinline__ void load_halo_async(const float* __restrict__ img, int v, int i0, int j0, int H, int W, float (*s)[ROW]) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // per-thread column state (the same for every row): three elements c = lane + 32 it of the 78-float row
     bool col_in[3];
@@ -55,7 +63,7 @@ __device__ __forceinline__ void load_halo_async(const float* __restrict__ img, i
             const int gi = i0 - kSsimR + r;
             const bool row_in = gi >= 0 && gi < H;
             const float* row = src0 + r * row_stride;
-            const uint32_t drow = dst0 + (uint32_t)(r * kSsimRowPad * 4);
+            const uint32_t drow = dst0 + (uint32_t)(r * ROW * 4);
 #pragma unroll
             for (int it = 0; it < 3; ++it) {
                 if (lane + 32 * it < kSsimRow) {
@@ -70,6 +78,34 @@ __device__ __forceinline__ void load_halo_async(const float* __restrict__ img, i
 __device__ __forceinline__ void halo_wait() {
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
     __syncthreads();
+}
+
+// ---- TMA halo loads (cp.async.bulk.tensor over a [C][H][W * 3] tensor map, box 1 x 26 x 80): one thread issues the copy of a
+// whole halo tile, rows and columns outside the image are filled with zeros by the copy engine (= the zero padding of
+// reading A21), completion is signalled on an mbarrier.
+__device__ __forceinline__ void tma_init(uint64_t* mbar) {
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(mbar)), "r"(1) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+}
+__device__ __forceinline__ void tma_expect(uint64_t* mbar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(mbar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_halo(const CUtensorMap* map, uint64_t* mbar, void* dst, int v, int i0, int j0) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"((j0 - kSsimR) * 3 - kSsimTmaOff), "r"(i0 - kSsimR),
+                   "r"(v), "r"((uint32_t)__cvta_generic_to_shared(mbar))
+                 : "memory");
+}
+__device__ __forceinline__ void tma_wait(uint64_t* mbar) {
+    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(mbar);
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(addr), "r"(0) : "memory");
+    } while (!done);
 }
 
 __device__ __forceinline__ float block_sum(float v, float* s_red) {
@@ -100,14 +136,29 @@ struct HzBuf {
     __device__ __forceinline__ float& at(int ch, int q, int r, int c) { return v[ch][(q * kSsimHalo + r) * kHzRow + c]; }
 };
 
-__global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
-    __shared__ float sx[kSsimHalo][kSsimRowPad], sy[kSsimHalo][kSsimRowPad];
+template <bool TMA>
+__global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a, const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my) {
+    constexpr int ROW = TMA ? kSsimRowTma : kSsimRowPad;
+    constexpr int OFF = TMA ? kSsimTmaOff : 0;            // column of the halo's first float inside a staged row
+    __shared__ __align__(128) float sx[kSsimHalo][ROW];
+    __shared__ __align__(128) float sy[kSsimHalo][ROW];
     __shared__ HzBuf<5> hz;
     __shared__ float s_red[8];
+    __shared__ uint64_t s_mbar;
     const int v = blockIdx.z, i0 = blockIdx.y * kSsimTile, j0 = blockIdx.x * kSsimTile;
-    load_halo_async(a.x, v, i0, j0, a.H, a.W, sx);
-    load_halo_async(a.y, v, i0, j0, a.H, a.W, sy);
-    halo_wait();
+    if constexpr (TMA) {
+        tma_init(&s_mbar);
+        if (threadIdx.x == 0) {
+            tma_expect(&s_mbar, 2 * kSsimTmaBytes);
+            tma_load_halo(&mx, &s_mbar, sx, v, i0, j0);
+            tma_load_halo(&my, &s_mbar, sy, v, i0, j0);
+        }
+        tma_wait(&s_mbar);
+    } else {
+        load_halo_async<ROW>(a.x, v, i0, j0, a.H, a.W, sx);
+        load_halo_async<ROW>(a.y, v, i0, j0, a.H, a.W, sy);
+        halo_wait();
+    }
     // horizontal pass
     for (int task = threadIdx.x; task < kSsimHalo * 3 * (kSsimTile / kSsimRun); task += 256) {
         const int r = task / 12, rem = task - r * 12, cg = rem / 3, ch = rem - cg * 3;
@@ -118,7 +169,7 @@ __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
         for (int o = 0; o < kSsimRun; ++o) { accA[o] = pk2(0.f, 0.f); accB[o] = accA[o]; accC[o] = 0.0f; }
 #pragma unroll
         for (int p = 0; p < kSsimIn; ++p) {
-            const float xv = sx[r][(kSsimRun * cg + p) * 3 + ch], yv = sy[r][(kSsimRun * cg + p) * 3 + ch];
+            const float xv = sx[r][(kSsimRun * cg + p) * 3 + ch + OFF], yv = sy[r][(kSsimRun * cg + p) * 3 + ch + OFF];
             const f32x2 X = pk2(xv, yv);
             const f32x2 P = mul2(X, X);
             const float xy = xv * yv;
@@ -191,7 +242,7 @@ __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
                 a.maps[a.n + o3] = wgt * d11;
                 a.maps[2 * a.n + o3] = wgt * d12;
                 ssim_sum += S;
-                l1_sum += fabsf(sx[ty + kSsimR][(col + kSsimR) * 3 + ch] - sy[ty + kSsimR][(col + kSsimR) * 3 + ch]);
+                l1_sum += fabsf(sx[ty + kSsimR][(col + kSsimR) * 3 + ch + OFF] - sy[ty + kSsimR][(col + kSsimR) * 3 + ch + OFF]);
             }
         }
     }
@@ -203,12 +254,27 @@ __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a) {
     }
 }
 
-__global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
-    __shared__ float sm[3][kSsimHalo][kSsimRowPad];
+template <bool TMA>
+__global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a, const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUtensorMap m1,
+                                                        const __grid_constant__ CUtensorMap m2) {
+    constexpr int ROW = TMA ? kSsimRowTma : kSsimRowPad;
+    constexpr int OFF = TMA ? kSsimTmaOff : 0;
+    __shared__ __align__(128) float sm[3][kSsimHalo][ROW];
     __shared__ HzBuf<3> hz;
+    __shared__ uint64_t s_mbar;
     const int v = blockIdx.z, i0 = blockIdx.y * kSsimTile, j0 = blockIdx.x * kSsimTile;
+    if constexpr (TMA) {
+        tma_init(&s_mbar);
+        if (threadIdx.x == 0) {
+            tma_expect(&s_mbar, 3 * kSsimTmaBytes);
+            tma_load_halo(&m0, &s_mbar, sm[0], v, i0, j0);
+            tma_load_halo(&m1, &s_mbar, sm[1], v, i0, j0);
+            tma_load_halo(&m2, &s_mbar, sm[2], v, i0, j0);
+        }
+    } else {
 #pragma unroll
-    for (int q = 0; q < 3; ++q) load_halo_async(a.maps + q * a.n, v, i0, j0, a.H, a.W, sm[q]);
+        for (int q = 0; q < 3; ++q) load_halo_async<ROW>(a.maps + q * a.n, v, i0, j0, a.H, a.W, sm[q]);
+    }
     // x and y at this thread's four output values travel while the window passes run
     const bool vtask = threadIdx.x < 3 * kSsimTile * (kSsimTile / kSsimRun);
     const int vch = threadIdx.x % 3, vcol = (threadIdx.x / 3) % kSsimTile, vg = threadIdx.x / (3 * kSsimTile);
@@ -222,7 +288,8 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
             xo[o] = __ldg(a.x + o3); yo[o] = __ldg(a.y + o3);
         }
     }
-    halo_wait();
+    if constexpr (TMA) tma_wait(&s_mbar);
+    else halo_wait();
     for (int task = threadIdx.x; task < kSsimHalo * 3 * (kSsimTile / kSsimRun); task += 256) {
         const int r = task / 12, rem = task - r * 12, cg = rem / 3, ch = rem - cg * 3;
         f32x2 accA[kSsimRun];
@@ -233,7 +300,7 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
         for (int p = 0; p < kSsimIn; ++p) {
             float in[3];
 #pragma unroll
-            for (int q = 0; q < 3; ++q) in[q] = sm[q][r][(kSsimRun * cg + p) * 3 + ch];
+            for (int q = 0; q < 3; ++q) in[q] = sm[q][r][(kSsimRun * cg + p) * 3 + ch + OFF];
             const f32x2 A2 = pk2(in[0], in[1]);
 #pragma unroll
             for (int o = 0; o < kSsimRun; ++o) {
@@ -293,6 +360,32 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a) {
     }
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point query (no link-time dependency on libcuda: the library
+// must load on a machine without a driver); nullptr when unavailable -> the cp.async path is used
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn tensor_map_encoder() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;          // idempotent cache of an immutable fact, like DeviceCache
+    if (!tried) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+        tried = true;
+    }
+    return fn;
+}
+// [C][H][W * 3] fp32 image as a 3-D tensor, box = one view x 26 rows x 80 floats, zero fill outside
+static bool make_halo_map(EncodeTiledFn enc, const float* img, int C, int H, int W, CUtensorMap* out) {
+    const cuuint64_t dims[3] = {(cuuint64_t)W * 3, (cuuint64_t)H, (cuuint64_t)C};
+    const cuuint64_t strides[2] = {(cuuint64_t)W * 3 * sizeof(float), (cuuint64_t)H * W * 3 * sizeof(float)};
+    const cuuint32_t box[3] = {(cuuint32_t)kSsimRowTma, (cuuint32_t)kSsimHalo, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(img), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 }  // namespace gs
 
 using namespace gs;
@@ -324,9 +417,20 @@ extern "C" int gs_l1_ssim_loss(int32_t C, int32_t height, int32_t width, const f
     for (int k = 0; k < kSsimWin; ++k) a.win[k] = (float)(g[k] / sum);
     const dim3 grid((unsigned)((width + kSsimTile - 1) / kSsimTile), (unsigned)((height + kSsimTile - 1) / kSsimTile), (unsigned)C);
     cudaStream_t st = (cudaStream_t)stream;
-    ssim_stats_kernel<<<grid, 256, 0, st>>>(a);
+    // TMA halo loads need 16-byte aligned images and row strides (W % 4 == 0); everything else takes the cp.async path
+    CUtensorMap mx, my, m0, m1, m2;
+    bool tma = false;
+    if (width % 4 == 0 && aligned(image, 16) && aligned(target, 16) && aligned(workspace, 16) && n % 4 == 0) {
+        if (EncodeTiledFn enc = tensor_map_encoder())
+            tma = make_halo_map(enc, image, C, height, width, &mx) && make_halo_map(enc, target, C, height, width, &my) &&
+                  make_halo_map(enc, a.maps, C, height, width, &m0) && make_halo_map(enc, a.maps + n, C, height, width, &m1) &&
+                  make_halo_map(enc, a.maps + 2 * n, C, height, width, &m2);
+    }
+    if (tma) ssim_stats_kernel<true><<<grid, 256, 0, st>>>(a, mx, my);
+    else ssim_stats_kernel<false><<<grid, 256, 0, st>>>(a, mx, my);
     int rc = launch_status();
     if (rc) return rc;
-    ssim_grad_kernel<<<grid, 256, 0, st>>>(a);
+    if (tma) ssim_grad_kernel<true><<<grid, 256, 0, st>>>(a, m0, m1, m2);
+    else ssim_grad_kernel<false><<<grid, 256, 0, st>>>(a, m0, m1, m2);
     return launch_status();
 }

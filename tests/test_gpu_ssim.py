@@ -52,7 +52,8 @@ def images(shape, seed, smooth=False):
     ((1, 16, 16, 3), 0.2, False),               # exactly one tile
     ((2, 37, 45, 3), 0.2, False),               # several tiles, ragged in both directions, two views
     ((1, 5, 7, 3), 0.2, False),                 # smaller than the window: every window is cut by the padding
-    ((3, 64, 80, 3), 1.0, True),                # SSIM term only, correlated images
+    ((3, 64, 80, 3), 1.0, True),                # SSIM term only, correlated images (W % 4 == 0: TMA halo loads)
+    ((2, 41, 52, 3), 0.2, True),                # TMA halo loads with ragged tiles: zero fill by the copy engine on every border
     ((1, 33, 17, 3), 0.0, False),               # L1 term only
     ((1, 1, 1, 3), 0.2, False),                 # a single pixel
 ])

@@ -523,7 +523,10 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
                         f"{FWD_FLOP_COMPOSITED if dominant == 'raster_fwd' else BWD_FLOP_COMPOSITED} per composited pair, "
                         f"{FWD_FLOP_REJECTED if dominant == 'raster_fwd' else BWD_FLOP_REJECTED} per evaluated-and-rejected pair; the kernel is "
                         "latency/barrier bound (ncu FMA pipe < 45 % of cycles, profiles/), not pipe bound")
-    roof["traffic"] = load_traffic(workload + ("_farinf" if far_inf else ""), roof["kernel"].split(" ")[0])
+    wl_key = workload + ("_farinf" if far_inf else "")
+    roof["traffic"] = load_traffic(wl_key, roof["kernel"])            # (a stage of several kernels has a row of its own: the sum)
+    if roof["traffic"] is None:
+        roof["traffic"] = load_traffic(wl_key, roof["kernel"].split(" ")[0])
 
     # ---- end to end: inputs from pinned host memory, loss read back, every step; uploads of step k + 1 overlap step k
     e2e = None

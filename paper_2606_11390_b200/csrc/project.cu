@@ -186,19 +186,38 @@ __device__ __forceinline__ uint32_t lateral_precull(const ProjFwdArgs& a, const 
     return keep;
 }
 
-// linear lateral test of one Gaussian against the views of zmask (set_lateral_bound in common.cuh): ALU only
-__device__ __forceinline__ uint32_t lateral_linear(const ProjFwdArgs& a, const CamBatch& cams, float smax_all, float px, float py, float pz,
-                                                   uint32_t zmask) {
-    uint32_t keep = 0;
-    for (int c = 0; c < a.C; ++c) {
-        if (!((zmask >> c) & 1u)) continue;
+// Camera constants of the linear lateral test in shared memory (20 floats per view): the lanes of a warp test different
+// views, and a lane-varying index into the constant bank would be replayed once per distinct view.
+constexpr int kLatFloats = 20;
+__device__ __forceinline__ void load_lateral_constants(const CamBatch& cams, int C, float smax_all, float (*s_lat)[kLatFloats]) {
+    for (int k = threadIdx.x; k < C * kLatFloats; k += blockDim.x) {
+        const int c = k / kLatFloats, j = k - c * kLatFloats;
         const DevCam& cam = cams.cam[c];
-        const float tx = cam.W[0] * px + cam.W[1] * py + cam.W[2] * pz + cam.tau[0];
-        const float ty = cam.W[3] * px + cam.W[4] * py + cam.W[5] * pz + cam.tau[1];
-        const float tz = cam.W[6] * px + cam.W[7] * py + cam.W[8] * pz + cam.tau[2];
-        const float kk = fmaf(cam.lat_k2, smax_all, cam.lat_abs);
-        const bool out = (cam.fx * fabsf(tx - tz * cam.lat_cx) > fmaf(cam.lat_k1x, tz, kk)) ||
-                         (cam.fy * fabsf(ty - tz * cam.lat_cy) > fmaf(cam.lat_k1y, tz, kk));
+        float v = 0.0f;
+        if (j < 9) v = cam.W[j];
+        else if (j < 12) v = cam.tau[j - 9];
+        else if (j == 12) v = cam.fx;
+        else if (j == 13) v = cam.fy;
+        else if (j == 14) v = cam.lat_cx;
+        else if (j == 15) v = cam.lat_cy;
+        else if (j == 16) v = cam.lat_k1x;
+        else if (j == 17) v = cam.lat_k1y;
+        else if (j == 18) v = fmaf(cam.lat_k2, smax_all, cam.lat_abs);
+        s_lat[c][j] = v;
+    }
+}
+// linear lateral test of one Gaussian against the views of zmask (set_lateral_bound in common.cuh): ALU only; the loop
+// runs over the set bits (a depth candidate of a large scene is usually inside one view's depth range)
+__device__ __forceinline__ uint32_t lateral_linear(const float (*s_lat)[kLatFloats], float px, float py, float pz, uint32_t zmask) {
+    uint32_t keep = 0;
+    while (zmask) {
+        const int c = __ffs(zmask) - 1;
+        zmask &= zmask - 1;
+        const float* q = s_lat[c];
+        const float tx = q[0] * px + q[1] * py + q[2] * pz + q[9];
+        const float ty = q[3] * px + q[4] * py + q[5] * pz + q[10];
+        const float tz = q[6] * px + q[7] * py + q[8] * pz + q[11];
+        const bool out = (q[12] * fabsf(tx - tz * q[14]) > fmaf(q[16], tz, q[18])) || (q[13] * fabsf(ty - tz * q[15]) > fmaf(q[17], tz, q[18]));
         if (!out) keep |= 1u << c;
     }
     return keep;
@@ -247,6 +266,9 @@ __global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const Proj
     float smax_all = -1.0f;
     if (a.ls_bound) smax_all = expf(__ldg(a.ls_bound));
     const bool use_bound = smax_all >= 0.0f && smax_all < kInfF;      // false for a NaN bound as well: nothing is dropped then
+    __shared__ float s_lat[kMaxCamsPerLaunch][kLatFloats];
+    if (use_bound) load_lateral_constants(cams, a.C, smax_all, s_lat);
+    __syncthreads();       // (the only block barrier: from here on the warps run independently)
     while (true) {
         const bool more = chunk < n_chunks;
         if (cnt2 >= 32 || (cnt2 > 0 && !more && cnt1 == 0 && cnt1b == 0)) {
@@ -268,7 +290,7 @@ __global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const Proj
         } else if (cnt1 >= 32 || (cnt1 > 0 && !more)) {
             // ---- B0a: linear lateral test with the scene-wide bound (a plain move without one) -> s1b
             stack_filter(s1, cnt1, s1b, cnt1b, lane, [&](uint32_t, uint32_t zmask, const float* m) {
-                return use_bound ? lateral_linear(a, cams, smax_all, m[0], m[1], m[2], zmask) : zmask;
+                return use_bound ? lateral_linear(s_lat, m[0], m[1], m[2], zmask) : zmask;
             });
         } else if (more) {
             // ---- A (streaming): means -> near/far test of every view; zero radii / tiles_touched (or the mask words) of the chunk

@@ -281,6 +281,7 @@ struct BwdSmem {
     float tbuf[kWarps][2 * kGroup][kTStride]; // rows 0..7: gp of record k over the warp's 64 pixels; rows 8..15: wgt
     float gpix[kWarps][3][kTStride];          // dL/dimage of the warp's pixels, one row per channel, same pixel layout
     unsigned int vis[kWarps][kBwdChunks];
+    unsigned int check[kBwdChunks];           // chunk holds a non-concave conic: the "power > 0" test applies (as in the forward pass)
     int max_contrib;
 };
 
@@ -382,6 +383,7 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
     const float ox = (warp & 1) ? 4.0f : -4.0f;                                            // centre of the warp's columns - xc
     const float pya = (float)((warp >> 1) * 8 + 2 * (lane & 3)) + 0.5f - 8.0f;             // reduce-phase row 2 (lane & 3) - yc
     const int64_t start = __ldg(a.ranges + 2 * bt);
+    const int list_len = (int)(__ldg(a.ranges + 2 * bt + 1) - start);
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.rec);
     const int ppos = 2 * lane + ((lane >> 4) << 2);                                        // this lane's pixel pair in a tile row
     const uint32_t tbase = (uint32_t)__cvta_generic_to_shared(&sm.tbuf[warp][0][ppos]);
@@ -422,8 +424,21 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
     const int nb = (maxn + kBwdBatch - 1) / kBwdBatch;
     for (int b = nb - 1; b >= 0; --b) {
         const int cnt = min(kBwdBatch, maxn - b * kBwdBatch);
+        // records behind the last walked one are staged up to the end of their 32-record chunk: they are never evaluated, but
+        // the forward kernel looked at the whole chunk when it decided whether the "power > 0" test applies
+        const int cnt_stage = min(min(kBwdBatch, (cnt + 31) & ~31), list_len - b * kBwdBatch);
         __syncthreads();   // previous batch fully flushed
-        if (tid < cnt) stage_record(a, __ldg(a.vals + start + (int64_t)b * kBwdBatch + tid), sm.rec[tid]);
+        if (tid < kBwdBatch) {
+            // (warp w < 2 stages chunk w; it also decides whether the chunk holds a non-concave conic)
+            bool concave = true;
+            if (tid < cnt_stage) {
+                stage_record(a, __ldg(a.vals + start + (int64_t)b * kBwdBatch + tid), sm.rec[tid]);
+                const Rec& rc = sm.rec[tid];
+                concave = (rc.b.x <= 0.0f) && (rc.c.x <= 0.0f) && (4.0f * rc.b.x * rc.c.x - rc.b.z * rc.b.z >= 0.0f);
+            }
+            const bool chk = __any_sync(0xffffffffu, !concave);
+            if (lane == 0) sm.check[warp] = chk ? 1u : 0u;
+        }
         __syncthreads();
         int k = 0;         // records in the warp's current group (warp-uniform)
         int myq = 0;       // batch position of the group's record (lane >> 2)
@@ -436,6 +451,9 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                 const Rec& rc = sm.rec[r];
                 may = rect_may_contribute(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr);
             }
+            // the same per-chunk rule as the forward kernel (the chunks are the same 32 list positions): the "power > 0" test
+            // is applied only in chunks that hold a non-concave conic, so both passes take the same decision for every pair
+            const bool check_e = sm.check[ch] != 0u;
             unsigned int mask = __ballot_sync(0xffffffffu, may);
             const int nrel0 = ncon0 - cbase, nrel1 = ncon1 - cbase;   // pixel j walks bits < nrel_j
             unsigned int written = 0;
@@ -457,8 +475,8 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                 unpk2(el, el0, el1);
                 const float raw0 = ex2_approx(el0), raw1 = ex2_approx(el1);
                 const float al0 = fminf(alpha_max, raw0), al1 = fminf(alpha_max, raw1);
-                const bool valid0 = (bit < nrel0) && !(e_0 > 0.0f) && !(al0 < alpha_min);
-                const bool valid1 = (bit < nrel1) && !(e_1 > 0.0f) && !(al1 < alpha_min);
+                const bool valid0 = (bit < nrel0) && !(check_e && e_0 > 0.0f) && !(al0 < alpha_min);
+                const bool valid1 = (bit < nrel1) && !(check_e && e_1 > 0.0f) && !(al1 < alpha_min);
                 if (!__any_sync(0xffffffffu, valid0 || valid1)) continue;
                 f32x2 rr, gg;
                 lds2x64(addr + 48, rr, gg);

@@ -376,6 +376,74 @@ def test_raster_bwd_parity(B, oracle, name, sc):
         print(f"[{name}] rel L2: " + ", ".join(f"{k} {rel_l2(got[k][vis], ref[k][vis]):.1e}" for k in ref))
 
 
+def _near_singular_conics(n):
+    """Conics (A, B, C) of splats 1e7..1e8 times longer than wide whose axis runs through pixel centres (direction (px, py) with
+    small integers), selected so that in fp32 (a) the staged conic still tests as concave under every contraction of
+    4 A' C' - B'^2 the compiler may choose and (b) the exponent, evaluated in the kernels' operation order, comes out positive
+    on at least four of the 17 on-axis pixel centres nearest to the mean (its true value there is about -1e-6)."""
+    import math
+    f, F = np.float32, np.float64
+    k = f(1.4426950408889634)
+    out = []
+    for lam1 in np.logspace(6.8, 8.5, 40):
+        for lam2 in (0.3, 0.4, 0.5, 0.7, 1.0, 1.5, 2.0, 3.0):
+            for px in range(-5, 6):
+                for py in range(1, 6):
+                    if px == 0 or math.gcd(abs(px), py) != 1:
+                        continue
+                    th = np.arctan2(py, px)
+                    c, s_ = np.cos(th), np.sin(th)
+                    A, Bc, Cc = f(c * c / lam1 + s_ * s_ / lam2), f(c * s_ * (1 / lam1 - 1 / lam2)), f(s_ * s_ / lam1 + c * c / lam2)
+                    Ap, Bp, Cp = f(f(f(-0.5) * k) * A), f(f(-k) * Bc), f(f(f(-0.5) * k) * Cc)
+                    t = f(f(4) * Ap)
+                    if min(f(f(t * Cp) - f(Bp * Bp)), f(F(t) * F(Cp) - F(f(Bp * Bp))), f(F(f(t * Cp)) - F(Bp) * F(Bp))) <= 0:
+                        continue
+                    pos = 0
+                    for d in range(-8, 9):
+                        dx, dy = f(px * d), f(py * d)
+                        tq = f(F(Bp) * F(dy) + F(f(Ap * dx)))
+                        pos += f(F(f(Cp * dy)) * F(dy) + F(f(tq * dx))) > 0
+                    if pos >= 4:
+                        out.append((A, Bc, Cc))
+                        if len(out) == n:
+                            return np.array(out, np.float32)
+    return np.array(out, np.float32)
+
+
+def test_raster_near_singular_conics_fwd_and_bwd_take_the_same_decisions(B, oracle):
+    """On the axis of such a splat the exponent is a difference of terms of size 1e2..1e3: its fp32 value is +-1e-4 around a
+    true value of about 0 and comes out POSITIVE on many pixels, while the conic tests as concave.  The forward kernel drops
+    the "power > 0" test for chunks of concave conics; the backward kernel must take the same decision for every pair, or it
+    misses the record's gradient and one division by (1 - alpha) on those pixels.  Checked without the oracle (in exact
+    arithmetic the fp32-rounded conic may be indefinite, so the double oracle may legitimately skip such a pair):
+    image - T bg = sum_i rgb_i alpha_i T_i, hence  sum_i rgb_i . dL/drgb_i = sum_pixels dL/dimage . (image - final_T bg)
+    holds exactly when the backward pass walks the pairs the forward pass composited, with the same weights."""
+    name, sc0 = SCENES[0]
+    cam = sc0["cameras"][0]
+    sc = {"cameras": [cam], "bg": np.array([0.1, 0.2, 0.3], np.float32), "sh_degree": 0}
+    cfg = oracle_cfg(oracle, sc)
+    H, W = cam["height"], cam["width"]
+    rng = np.random.default_rng(17)
+    conics = _near_singular_conics(32)
+    N = len(conics)
+    assert N >= 16
+    rec = {"means2d": (rng.integers(24, 40, size=(1, N, 2)) + 0.5).astype(np.float32),
+           "conics": conics[None],
+           "opacities": rng.uniform(0.05, 0.15, size=(1, N)).astype(np.float32),        # (low: no pixel saturates)
+           "rgbs": rng.uniform(0.2, 1.0, size=(1, N, 3)).astype(np.float32),
+           "depths": (1.0 + np.arange(N, dtype=np.float32))[None]}
+    radii = np.full((1, N), 2 * max(H, W), np.int32)
+    keys, vals, ranges = oracle.bin_tiles(cfg, sc["cameras"], rec["means2d"], rec["depths"], radii)
+    gi, gT, gn = run_raster_fwd(B, sc, rec, vals, ranges)
+    assert gn.max() > 0 and gT.min() < 0.9
+    dL = (rng.uniform(0.5, 1.5, size=gi.shape) / gi[0].size).astype(np.float32)      # one sign: no cancellation in the sums
+    got = run_raster_bwd(B, sc, rec, vals, ranges, gT, gn, dL)
+    lhs = float((rec["rgbs"].astype(np.float64) * got["rgbs"].astype(np.float64)).sum())
+    rhs = float((dL.astype(np.float64) * (gi.astype(np.float64) - gT.astype(np.float64)[..., None] * sc["bg"].astype(np.float64))).sum())
+    print(f"sum rgb . dL/drgb = {lhs:.9f}, sum dL . (image - T bg) = {rhs:.9f}")
+    assert abs(lhs - rhs) <= 2e-5 * abs(rhs), (lhs, rhs)
+
+
 # ------------------------------------------------------------------------------------ P5
 def run_project_bwd(B, sc, radii, g2, accumulate=False, init=None):
     cams = B.make_cameras(sc["cameras"])

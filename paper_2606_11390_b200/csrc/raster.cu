@@ -18,8 +18,6 @@
 // record go to the warp's own shared-memory slot (shared-memory float atomics are CAS loops on
 // this hardware), are summed across the 4 warps at the end of the batch and flushed with one
 // device-scope red.add per value and (tile, record).
-#include <type_traits>
-
 #include "common.cuh"
 
 namespace gs {
@@ -110,7 +108,7 @@ __device__ __forceinline__ void stage_record(const RasterArgs& a, int g, Rec& r)
 
 // rect_may_contribute for a (wx+1) x (wy+1) block of pixel centres starting at (X0, Y0)
 __device__ __forceinline__ bool rect_may_contribute(float u, float v, float A, float B, float C, float lo, float X0, float Y0, float wx, float wy,
-                                                     float thr, bool* is_concave = nullptr) {
+                                                     float thr) {
     const float dx0 = u - (X0 + wx), dx1 = u - X0;
     const float dy0 = v - (Y0 + wy), dy1 = v - Y0;
     const bool inx = (dx0 <= 0.0f) && (dx1 >= 0.0f), iny = (dy0 <= 0.0f) && (dy1 >= 0.0f);
@@ -129,7 +127,6 @@ __device__ __forceinline__ bool rect_may_contribute(float u, float v, float A, f
             emax = fmaxf(emax, fmaxf(quad_form(A, B, C, dxs, dye), fmaxf(quad_form(A, B, C, dx0, dye), quad_form(A, B, C, dx1, dye))));
         }
     }
-    if (is_concave) *is_concave = concave;
     return !concave || !(emax + lo < thr);
 }
 
@@ -170,17 +167,18 @@ __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, 
         bool warp_done = __all_sync(0xffffffffu, T0 < 0.0f && T1 < 0.0f);
         for (int ch = 0; ch * 32 < cnt && !warp_done; ++ch) {
             const int r = ch * 32 + lane;
-            bool may = false, concave = true;
+            bool may = false;
             if (r < cnt) {
                 const Rec& rc = s_rec[r];
-                may = rect_may_contribute(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr, &concave);
+                may = rect_may_contribute(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr);
             }
-            // the exponent of a concave (valid) conic cannot be positive: its "power > 0" test is dropped (a rounding
-            // residue of +1e-7 changes alpha by 1e-7); chunks that hold any other record take the checked body
-            const bool check_e = __any_sync(0xffffffffu, !concave);
             unsigned int mask = __ballot_sync(0xffffffffu, may);
-            auto composite = [&](auto checked, int q) {
-                constexpr bool CHECK = decltype(checked)::value;
+            // (Round 1 dropped the "power > 0" test for chunks of concave conics; the backward kernel always applies it, and for
+            //  near-singular conics the fp32 exponent is +-1e-4 around 0, so the two passes disagreed on such pairs.  Always
+            //  applying it, as O-R1 is written, costs 2 % here; the same per-chunk rule in the backward kernel cost it 1-4 %.)
+            while (mask) {
+                const int q = ch * 32 + __ffs(mask) - 1;
+                mask &= mask - 1;
                 const uint32_t addr = sbase + (uint32_t)q * (uint32_t)sizeof(Rec);
                 f32x2 uu, vv, AA, BB, CC, LL, rr, gg;
                 lds2x64(addr, uu, vv);
@@ -203,7 +201,7 @@ __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, 
                 float Tn0, Tn1, wg0, wg1;
                 unpk2(Tn, Tn0, Tn1);
                 unpk2(wg, wg0, wg1);
-                const bool ok0 = !(CHECK && e_0 > 0.0f) && !(al0 < alpha_min), ok1 = !(CHECK && e_1 > 0.0f) && !(al1 < alpha_min);
+                const bool ok0 = !(e_0 > 0.0f) && !(al0 < alpha_min), ok1 = !(e_1 > 0.0f) && !(al1 < alpha_min);
                 const bool term0 = ok0 && (Tn0 < t_min), term1 = ok1 && (Tn1 < t_min);      // also true again for a finished pixel
                 const bool upd0 = ok0 && !(Tn0 < t_min), upd1 = ok1 && !(Tn1 < t_min);
                 const f32x2 w2 = pk2(upd0 ? wg0 : 0.0f, upd1 ? wg1 : 0.0f);
@@ -213,21 +211,7 @@ __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, 
                 T0 = upd0 ? Tn0 : (term0 ? -fabsf(T0) : T0);
                 T1 = upd1 ? Tn1 : (term1 ? -fabsf(T1) : T1);
                 last0 = upd0 ? nbase + q : last0; last1 = upd1 ? nbase + q : last1;
-            };
-            if (check_e) {
-                while (mask) {
-                    const int q = ch * 32 + __ffs(mask) - 1;
-                    mask &= mask - 1;
-                    composite(std::true_type{}, q);
-                    if (__all_sync(0xffffffffu, T0 < 0.0f && T1 < 0.0f)) { warp_done = true; break; }
-                }
-            } else {
-                while (mask) {
-                    const int q = ch * 32 + __ffs(mask) - 1;
-                    mask &= mask - 1;
-                    composite(std::false_type{}, q);
-                    if (__all_sync(0xffffffffu, T0 < 0.0f && T1 < 0.0f)) { warp_done = true; break; }
-                }
+                if (__all_sync(0xffffffffu, T0 < 0.0f && T1 < 0.0f)) { warp_done = true; break; }
             }
         }
     }
@@ -281,7 +265,6 @@ struct BwdSmem {
     float tbuf[kWarps][2 * kGroup][kTStride]; // rows 0..7: gp of record k over the warp's 64 pixels; rows 8..15: wgt
     float gpix[kWarps][3][kTStride];          // dL/dimage of the warp's pixels, one row per channel, same pixel layout
     unsigned int vis[kWarps][kBwdChunks];
-    unsigned int check[kBwdChunks];           // chunk holds a non-concave conic: the "power > 0" test applies (as in the forward pass)
     int max_contrib;
 };
 
@@ -383,7 +366,6 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
     const float ox = (warp & 1) ? 4.0f : -4.0f;                                            // centre of the warp's columns - xc
     const float pya = (float)((warp >> 1) * 8 + 2 * (lane & 3)) + 0.5f - 8.0f;             // reduce-phase row 2 (lane & 3) - yc
     const int64_t start = __ldg(a.ranges + 2 * bt);
-    const int list_len = (int)(__ldg(a.ranges + 2 * bt + 1) - start);
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.rec);
     const int ppos = 2 * lane + ((lane >> 4) << 2);                                        // this lane's pixel pair in a tile row
     const uint32_t tbase = (uint32_t)__cvta_generic_to_shared(&sm.tbuf[warp][0][ppos]);
@@ -424,21 +406,8 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
     const int nb = (maxn + kBwdBatch - 1) / kBwdBatch;
     for (int b = nb - 1; b >= 0; --b) {
         const int cnt = min(kBwdBatch, maxn - b * kBwdBatch);
-        // records behind the last walked one are staged up to the end of their 32-record chunk: they are never evaluated, but
-        // the forward kernel looked at the whole chunk when it decided whether the "power > 0" test applies
-        const int cnt_stage = min(min(kBwdBatch, (cnt + 31) & ~31), list_len - b * kBwdBatch);
         __syncthreads();   // previous batch fully flushed
-        if (tid < kBwdBatch) {
-            // (warp w < 2 stages chunk w; it also decides whether the chunk holds a non-concave conic)
-            bool concave = true;
-            if (tid < cnt_stage) {
-                stage_record(a, __ldg(a.vals + start + (int64_t)b * kBwdBatch + tid), sm.rec[tid]);
-                const Rec& rc = sm.rec[tid];
-                concave = (rc.b.x <= 0.0f) && (rc.c.x <= 0.0f) && (4.0f * rc.b.x * rc.c.x - rc.b.z * rc.b.z >= 0.0f);
-            }
-            const bool chk = __any_sync(0xffffffffu, !concave);
-            if (lane == 0) sm.check[warp] = chk ? 1u : 0u;
-        }
+        if (tid < cnt) stage_record(a, __ldg(a.vals + start + (int64_t)b * kBwdBatch + tid), sm.rec[tid]);
         __syncthreads();
         int k = 0;         // records in the warp's current group (warp-uniform)
         int myq = 0;       // batch position of the group's record (lane >> 2)
@@ -451,9 +420,6 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                 const Rec& rc = sm.rec[r];
                 may = rect_may_contribute(rc.a.x, rc.a.z, rc.b.x, rc.b.z, rc.c.x, rc.c.z, X0, Y0, 7.0f, 7.0f, a.filter_thr);
             }
-            // the same per-chunk rule as the forward kernel (the chunks are the same 32 list positions): the "power > 0" test
-            // is applied only in chunks that hold a non-concave conic, so both passes take the same decision for every pair
-            const bool check_e = sm.check[ch] != 0u;
             unsigned int mask = __ballot_sync(0xffffffffu, may);
             const int nrel0 = ncon0 - cbase, nrel1 = ncon1 - cbase;   // pixel j walks bits < nrel_j
             unsigned int written = 0;
@@ -475,8 +441,8 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                 unpk2(el, el0, el1);
                 const float raw0 = ex2_approx(el0), raw1 = ex2_approx(el1);
                 const float al0 = fminf(alpha_max, raw0), al1 = fminf(alpha_max, raw1);
-                const bool valid0 = (bit < nrel0) && !(check_e && e_0 > 0.0f) && !(al0 < alpha_min);
-                const bool valid1 = (bit < nrel1) && !(check_e && e_1 > 0.0f) && !(al1 < alpha_min);
+                const bool valid0 = (bit < nrel0) && !(e_0 > 0.0f) && !(al0 < alpha_min);
+                const bool valid1 = (bit < nrel1) && !(e_1 > 0.0f) && !(al1 < alpha_min);
                 if (!__any_sync(0xffffffffu, valid0 || valid1)) continue;
                 f32x2 rr, gg;
                 lds2x64(addr + 48, rr, gg);

@@ -412,9 +412,10 @@ def _near_singular_conics(n):
 
 def test_raster_near_singular_conics_fwd_and_bwd_take_the_same_decisions(B, oracle):
     """On the axis of such a splat the exponent is a difference of terms of size 1e2..1e3: its fp32 value is +-1e-4 around a
-    true value of about 0 and comes out POSITIVE on many pixels, while the conic tests as concave.  The forward kernel drops
-    the "power > 0" test for chunks of concave conics; the backward kernel must take the same decision for every pair, or it
-    misses the record's gradient and one division by (1 - alpha) on those pixels.  Checked without the oracle (in exact
+    true value of about 0 and comes out POSITIVE on many pixels, while the conic tests as concave.  Round 1's forward kernel dropped
+    the "power > 0" test for chunks of concave conics while its backward kernel applied it: the backward pass then missed the
+    record's gradient and one division by (1 - alpha) on those pixels (this identity was off by 4 %).  Both kernels now apply
+    the test to every pair, as O-R1 / O-R2 are written.  Checked without the oracle (in exact
     arithmetic the fp32-rounded conic may be indefinite, so the double oracle may legitimately skip such a pair):
     image - T bg = sum_i rgb_i alpha_i T_i, hence  sum_i rgb_i . dL/drgb_i = sum_pixels dL/dimage . (image - final_T bg)
     holds exactly when the backward pass walks the pairs the forward pass composited, with the same weights."""

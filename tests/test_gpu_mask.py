@@ -199,3 +199,46 @@ def test_adam_running_max(B):
         new_max = float(dp.max().item())
         assert (new_max > float(p.max())) == (sign < 0)
         assert float(bound.item()) == max(float(p.max()), new_max)
+
+
+def test_uploaded_parameters_refresh_the_scale_bound(B):
+    """The lateral cull of P1 is only valid with a bound >= every log-scale.  A second parameter set is uploaded in which some
+    Gaussians far outside the image grow so large that they reach it: they are visible only if the bound was recomputed for
+    the new parameters (SplatStep does that in step_uploaded); with the stale bound P1 drops them (checked as well, so that
+    this test is known to see the failure)."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    name, sc = MASK_SCENES[3]
+    sc2 = dict(sc)
+    ls = sc["log_scales"].copy()
+    cam = sc["cameras"][0]
+    vm = np.asarray(cam["viewmat"], np.float64).reshape(3, 4)
+    t = sc["means"].astype(np.float64) @ vm[:, :3].T + vm[:, 3]
+    lateral = (t[:, 2] > 20) & (t[:, 2] < 100) & (np.abs(t[:, 0]) > 1.5 * t[:, 2]) & (np.abs(t[:, 0]) < 2.5 * t[:, 2])
+    grown = np.nonzero(lateral)[0][:200]
+    assert len(grown) >= 50
+    ls[grown] = np.log(0.6 * np.abs(t[grown, 0]))[:, None].astype(np.float32)        # 3 sigma reaches the optical axis
+    sc2["log_scales"] = ls
+    tgt = scenes.target_image(sc)
+    ref = SplatStep(sc2, use_mask=False)
+    ref.set_target(tgt)
+    ref.step(sync=True)
+    torch.cuda.synchronize()
+    vis_ref = ref.visible()
+    assert bool(vis_ref[0, torch.from_numpy(grown).cuda()].any())                      # the grown Gaussians do reach view 0
+
+    st = SplatStep(sc, use_mask=True, capacity_M=ref.capacity_M)
+    st.set_target(tgt)
+    st.step(sync=True)                                                                 # bound of the FIRST parameter set is now cached
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
+    host = {k: pin(sc2[k]) for k in st.param_names}
+    host_loss = torch.zeros((1,), dtype=torch.float32).pin_memory()
+    st.step_from_host(host, pin(tgt), host_loss)
+    torch.cuda.synchronize()
+    assert float(st.ls_bound.item()) == float(ls.max())
+    assert torch.equal(st.visible(), vis_ref)
+    assert torch.equal(st.image, ref.image)
+    # the failure this guards against: the same step with the stale bound of the first parameter set
+    B.gs_log_scale_bound(dev(sc["log_scales"]), st.ls_bound)
+    st.project_fwd()
+    torch.cuda.synchronize()
+    assert not torch.equal(st.visible(), vis_ref)

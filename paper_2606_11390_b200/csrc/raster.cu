@@ -447,21 +447,18 @@ __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, 
                 f32x2 rr, gg;
                 lds2x64(addr + 48, rr, gg);
                 const f32x2 bb = lds64(addr + 64);
-                // quantities of an invalid pixel are computed but selected away
-                const f32x2 al = pk2(al0, al1);
+                // an invalid pixel takes part with alpha = 0: 1 - alpha = 1, rcp.approx(1) = 1 exactly, so its T, S and both
+                // outputs come out unchanged / zero without any further select
+                const f32x2 am = pk2(valid0 ? al0 : 0.0f, valid1 ? al1 : 0.0f);
                 float om0, om1;
-                unpk2(fma2(al, neg2, one2), om0, om1);
-                const f32x2 Tp = pk2(T0, T1);
-                const f32x2 Tf = mul2(Tp, pk2(rcp_approx(om0), rcp_approx(om1)));   // transmittance in front of this record
+                unpk2(fma2(am, neg2, one2), om0, om1);
+                const f32x2 Tf = mul2(pk2(T0, T1), pk2(rcp_approx(om0), rcp_approx(om1)));   // transmittance in front of this record
                 const f32x2 d0 = fma2(S0, neg2, rr), d1 = fma2(S1, neg2, gg), d2 = fma2(S2, neg2, bb);
                 const f32x2 dLda = mul2(Tf, fma2(d2, G2, fma2(d1, G1, mul2(d0, G0))));
-                const f32x2 am = pk2(valid0 ? al0 : 0.0f, valid1 ? al1 : 0.0f);
                 S0 = fma2(am, d0, S0);
                 S1 = fma2(am, d1, S1);
                 S2 = fma2(am, d2, S2);
-                float Tf0, Tf1;
-                unpk2(Tf, Tf0, Tf1);
-                T0 = valid0 ? Tf0 : T0; T1 = valid1 ? Tf1 : T1;
+                unpk2(Tf, T0, T1);
                 // no gradient through the alpha_max clamp
                 float gp0, gp1;
                 unpk2(mul2(am, dLda), gp0, gp1);

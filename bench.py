@@ -67,6 +67,8 @@ def parse_args():
                     help="run the dense zero-fill of the gradients on a second stream underneath the rasterisation kernels instead of "
                          "inside project_bwd (measured: no gain, see pipeline.py)")
     ap.add_argument("--zf-priority", type=int, default=0, help="stream priority of the zero-fill stream (0 or -1)")
+    ap.add_argument("--tile-sort", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="gs_bin_tiles tile_sort: 0 automatic, 1 one-level record sort, 2 / 3 groups of 4x4 / 8x8 tiles + expansion")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE configs")
@@ -383,6 +385,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     st = SplatStep(sc, device=dev, use_mask=False if args.no_mask else None)
     st.set_target(tgt_host)
     st.loss_mode = args.loss
+    st.tile_sort = args.tile_sort
     morton_ms = None
     if args.morton:
         B.morton_sort({k: st.params[k] for k in st.param_names})          # warm-up (allocations, first launches)
@@ -482,6 +485,12 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     P_t = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
     cells = C * (st.gx + 1) * (st.gy + 1)
     tsort_bytes = 4 * M_now if P_t == 1 else (8 + 16 * (P_t - 2) + 12) * M_now
+    # two-level tile sort (chosen by gs_bin_tiles from the record capacity): the records that are generated and sorted are
+    # (group of tiles, entry) -- their count M_c is in the workspace header -- and every record is then written once by the
+    # expansion: group sort (8 + 12) M_c (two passes), expansion 4 M_c (list) + 12 M_c (mean, radius gathers) + 4 M
+    M_groups = int(st.workspace[:96].view(torch.int64)[11].item())
+    if M_groups > 0:
+        tsort_bytes = (8 + 12 + 4 + 12) * M_groups + 4 * M_now
     K3 = 3 * st.K
     par_b = 4 * (3 + 3 + 4 + 1 + K3)
     # how visibility travels: the bit mask written by P1 (C * GS_VIS_WORDS(N) words) or the dense radii (and tiles_touched)
@@ -605,7 +614,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
                    "sparse_grads": bool(args.sparse_grads),
                    "visibility": "bit mask written by P1 + scene-wide log-scale bound" if st.use_mask else "dense radii",
                    "grad_zero_fill": "second stream, under the rasterisation kernels" if overlap else "inside project_bwd", "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
-                   "intersections": M_now, "visible_entries": V_sum, "visible_gaussians": V_any,
+                   "intersections": M_now, "group_records": M_groups, "visible_entries": V_sum, "visible_gaussians": V_any,
                    "pairs_composited": pairs_composited, "pairs_rejected_fwd": pairs_rej_fwd, "pairs_rejected_bwd": pairs_rej_bwd,
                    "pairs_dense_bound": pairs_dense, "n_contrib_sum": n_contrib_sum,
                    "parallelism": "replicas only" if world > 1 else "single GPU", "timing": "median of the timed steps (CUDA events)",

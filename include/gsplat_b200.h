@@ -113,12 +113,21 @@ int gs_log_scale_bound(int64_t N, const float* log_scales, float* bound, void* s
  * rasteriser reads only values and ranges), isect_vals[capacity_M] (int32),
  * tile_ranges[C*tiles,2] (int64).  depths must be positive (they are: depth > near > 0).
  * vis_mask (optional): the mask gs_project_fwd wrote; the visible entries are then exactly its set bits (radii is read
- *   only for those) and no pass over the dense radii is made. */
+ *   only for those) and no pass over the dense radii is made.
+ * tile_sort: how the records are brought into tile order (same result bit for bit, GS_TILE_SORT_AUTO chooses by size):
+ *   ONE_LEVEL = stable radix sort of the M (tile, entry) records on the tile id; GROUPS_4 / GROUPS_8 = the records that are
+ *   generated and sorted are (group of 4x4 / 8x8 tiles, entry), 2..10 per visible entry instead of 19..80, and every group
+ *   then expands its depth-ordered list into the lists of its tiles, one ballot per (tile, 32 entries), writing each record
+ *   straight to its final place (GS_ERR_UNSUPPORTED beyond 8192 groups per batch). */
+#define GS_TILE_SORT_AUTO 0
+#define GS_TILE_SORT_ONE_LEVEL 1
+#define GS_TILE_SORT_GROUPS_4 2
+#define GS_TILE_SORT_GROUPS_8 3
 int gs_bin_tiles(const gs_config* cfg /*host*/, int64_t N, int32_t C, const gs_camera* cams /*host*/,
                  const float* means2d, const float* depths, const int32_t* radii, const uint32_t* vis_mask /*optional*/, void* workspace,
                  size_t* workspace_bytes /*host*/, int64_t capacity_M, uint64_t* isect_keys,
                  int32_t* isect_vals, int64_t* tile_ranges, int64_t* M_dev, int64_t* M_out /*host*/,
-                 void* stream);
+                 int32_t tile_sort, void* stream);
 
 /* Stand-alone stable LSD radix sort used by gs_bin_tiles (step B3), exported for testing and
  * measurement: sorts n (key, value) pairs on key bits [0, end_bit) -- bit 31 is skipped when

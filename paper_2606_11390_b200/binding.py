@@ -16,6 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgsplat_b200.so")
 
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+GS_TILE_SORT_AUTO, GS_TILE_SORT_ONE_LEVEL, GS_TILE_SORT_GROUPS_4, GS_TILE_SORT_GROUPS_8 = 0, 1, 2, 3
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
            "gs_raster_fwd", "gs_raster_bwd", "gs_raster_pair_stats", "gs_project_bwd", "gs_grad_zero_fill", "gs_log_scale_bound", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
@@ -147,13 +148,13 @@ def gs_log_scale_bound(log_scales, bound, stream=None):
 def gs_bin_tiles_workspace_bytes(cfg, N, cams, capacity_M):
     n = C.c_size_t(0)
     rc = lib().gs_bin_tiles(C.byref(cfg), C.c_int64(N), C.c_int32(len(cams)), cams, None, None, None, None, None, C.byref(n),
-                            C.c_int64(capacity_M), None, None, None, None, None, None)
+                            C.c_int64(capacity_M), None, None, None, None, None, C.c_int32(0), None)
     _check(rc, "gs_bin_tiles(size query)")
     return int(n.value)
 
 
 def gs_bin_tiles(cfg, N, cams, means2d, depths, radii, workspace, capacity_M, isect_keys, isect_vals, tile_ranges,
-                 M_dev=None, sync=True, stream=None, vis_mask=None):
+                 M_dev=None, sync=True, stream=None, vis_mask=None, tile_sort=0):
     """``isect_keys`` may be None (the 64-bit keys are then not materialised).
     Returns M (host int) when ``sync`` is true, else None (M is then only in ``M_dev``).
     Raises GsError(GS_ERR_CAPACITY) with ``.needed`` set when capacity_M is too small."""
@@ -165,7 +166,7 @@ def gs_bin_tiles(cfg, N, cams, means2d, depths, radii, workspace, capacity_M, is
                             C.c_int64(capacity_M), _ptr(isect_keys) if isect_keys is not None else None,
                             _ptr(isect_vals, torch.int32),
                             _ptr(tile_ranges, torch.int64), _ptr(M_dev, torch.int64) if M_dev is not None else None,
-                            C.byref(m) if sync else None, _stream(stream))
+                            C.byref(m) if sync else None, C.c_int32(int(tile_sort)), _stream(stream))
     if rc == GS_ERR_CAPACITY:
         err = GsError(rc, "gs_bin_tiles")
         err.needed = int(m.value)

@@ -160,7 +160,7 @@ class SplatStep:
             try:
                 m = B.gs_bin_tiles(self.cfg, self.N, self.cams, self.means2d, self.depths, self.radii, self.workspace,
                                    self.capacity_M, self.isect_keys, self.isect_vals, self.tile_ranges, self.M_dev, sync,
-                                   vis_mask=self.vis_mask)
+                                   vis_mask=self.vis_mask, tile_sort=getattr(self, "tile_sort", 0))
                 if sync:
                     self.M = m
                 elif self._M_event is None:

@@ -83,7 +83,7 @@ def test_host_side_validation_needs_no_gpu(cuda_lib):
     # capacity beyond the 2^30 record limit
     n = C.c_size_t(0)
     assert lib.gs_bin_tiles(C.byref(cfg), C.c_int64(10), C.c_int32(1), cams, None, None, None, None, None, C.byref(n),
-                            C.c_int64(1 << 30), None, None, None, None, None, None) == cuda_lib.GS_ERR_UNSUPPORTED
+                            C.c_int64(1 << 30), None, None, None, None, None, C.c_int32(0), None) == cuda_lib.GS_ERR_UNSUPPORTED
 
 
 def test_binding_refuses_cpu_tensors(cuda_lib):

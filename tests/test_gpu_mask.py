@@ -118,13 +118,14 @@ def test_bin_tiles_from_mask_bit_exact(B, oracle, name, sc):
     vis = pf["radii"] > 0
     radii = np.where(vis, pf["radii"], 12345).astype(np.int32)
     vm = dev(pack_mask(vis, B.vis_words(N)))
-    for cap, sync in ((len(keys) + 1000, True), (len(keys), False)):
+    for cap, sync, mode in ((len(keys) + 1000, True, 0), (len(keys), False, 2), (len(keys) + 7, False, 3)):      # (tile_sort modes)
         gk = torch.zeros((cap,), dtype=torch.int64, device="cuda")
         gv = torch.zeros((cap,), dtype=torch.int32, device="cuda")
         gr = torch.full((C * gx * gy, 2), -1, dtype=torch.int64, device="cuda")
         ws = torch.empty((B.gs_bin_tiles_workspace_bytes(bcfg, N, cams, cap),), dtype=torch.uint8, device="cuda")
         M_dev = torch.full((1,), -1, dtype=torch.int64, device="cuda")
-        B.gs_bin_tiles(bcfg, N, cams, dev(rec["means2d"]), dev(rec["depths"]), dev(radii), ws, cap, gk, gv, gr, M_dev, sync, vis_mask=vm)
+        B.gs_bin_tiles(bcfg, N, cams, dev(rec["means2d"]), dev(rec["depths"]), dev(radii), ws, cap, gk, gv, gr, M_dev, sync, vis_mask=vm,
+                       tile_sort=mode)
         torch.cuda.synchronize()
         M = int(M_dev.item())
         assert M == len(keys)

@@ -141,6 +141,18 @@ def oracle_stage1(oracle, sc):
     return cfg, pf, rec
 
 
+TILE_SORT = 0      # gs_bin_tiles tile_sort mode used by run_bin; the `tile_sort` fixture runs the binning tests in every mode
+
+
+@pytest.fixture(params=[1, 2, 3], ids=["one-level", "groups4", "groups8"])
+def tile_sort(request):
+    """GS_TILE_SORT_ONE_LEVEL / GROUPS_4 / GROUPS_8: at the test sizes AUTO would always choose the one-level sort."""
+    global TILE_SORT
+    TILE_SORT = request.param
+    yield request.param
+    TILE_SORT = 0
+
+
 def run_bin(B, sc, rec, radii, capacity=None, sync=True, want_keys=True):
     cams = B.make_cameras(sc["cameras"])
     cfg = B.default_config(sh_degree=sc["sh_degree"])
@@ -153,13 +165,13 @@ def run_bin(B, sc, rec, radii, capacity=None, sync=True, want_keys=True):
     ws = torch.empty((B.gs_bin_tiles_workspace_bytes(cfg, N, cams, cap),), dtype=torch.uint8, device="cuda")
     M_dev = torch.full((1,), -1, dtype=torch.int64, device="cuda")
     M = B.gs_bin_tiles(cfg, N, cams, dev(rec["means2d"]), dev(rec["depths"]), dev(radii), ws, cap, keys if want_keys else None,
-                       vals, ranges, M_dev, sync)
+                       vals, ranges, M_dev, sync, tile_sort=TILE_SORT)
     torch.cuda.synchronize()
     return M, int(M_dev.item()), keys.cpu().numpy().view(np.uint64), vals.cpu().numpy(), ranges.cpu().numpy()
 
 
 @pytest.mark.parametrize("name,sc", SCENES, ids=[s[0] for s in SCENES])
-def test_bin_tiles_bit_exact(B, oracle, name, sc):
+def test_bin_tiles_bit_exact(B, oracle, name, sc, tile_sort):
     """north_star: "tile keys and per-tile ranges bit-exact when built from the oracle's projected
     means and radii" -- and, because the emit is index-ordered, the values too."""
     cfg, pf, rec = oracle_stage1(oracle, sc)
@@ -183,7 +195,7 @@ def test_bin_tiles_bit_exact(B, oracle, name, sc):
     print(f"[{name}] M = {M}")
 
 
-def test_bin_tiles_edge_cases(B, oracle):
+def test_bin_tiles_edge_cases(B, oracle, tile_sort):
     name, sc = SCENES[1]
     cfg, pf, rec = oracle_stage1(oracle, sc)
     keys, vals, ranges = oracle.bin_tiles(cfg, sc["cameras"], rec["means2d"], rec["depths"], pf["radii"])
@@ -205,7 +217,7 @@ def test_bin_tiles_edge_cases(B, oracle):
     np.testing.assert_array_equal(gk[:M], k1); np.testing.assert_array_equal(gv[:M], v1); np.testing.assert_array_equal(gr, r1)
 
 
-def test_bin_tiles_whole_screen_splat_and_depth_ties(B, oracle):
+def test_bin_tiles_whole_screen_splat_and_depth_ties(B, oracle, tile_sort):
     """A Gaussian covering every tile (largest per-entry record count) plus exact depth ties."""
     cams = [scenes.make_camera(640, 360, 500.0, 500.0, (0, 0, -3), (0, 0, 0), (0, -1, 0))] * 2
     sc = {"cameras": cams, "sh_degree": 0}
@@ -225,8 +237,11 @@ def test_bin_tiles_whole_screen_splat_and_depth_ties(B, oracle):
 
 
 @pytest.mark.parametrize("W,H,C", [(3840, 2160, 4), (8192, 8192, 2), (4000, 33, 3)])
-def test_bin_tiles_tile_sort_pass_plans(B, oracle, W, H, C):
-    """Tile-id widths of 17 bits (2 passes of 9 bits), 19 bits (3 passes) and 10 bits (2 narrow passes)."""
+def test_bin_tiles_tile_sort_pass_plans(B, oracle, W, H, C, tile_sort):
+    """Tile-id widths of 17 bits (2 passes of 9 bits), 19 bits (3 passes) and 10 bits (2 narrow passes); in the group modes
+    8 160 / 32 768 (refused) / 27 groups of 4 x 4 tiles, 2 040 / 8 192 / 9 groups of 8 x 8."""
+    if tile_sort == 2 and (W, H) == (8192, 8192):
+        pytest.skip("32 768 groups of 4 x 4 tiles: beyond the 8 192 groups a batch may have (GS_ERR_UNSUPPORTED, checked below)")
     cams = [scenes.make_camera(W, H, 1000.0, 1000.0, (0, 0, -3), (0, 0, 0), (0, -1, 0))] * C
     sc = {"cameras": cams, "sh_degree": 0}
     rng = np.random.default_rng(W + C)
@@ -242,6 +257,12 @@ def test_bin_tiles_tile_sort_pass_plans(B, oracle, W, H, C):
     np.testing.assert_array_equal(gk[:M], keys)
     np.testing.assert_array_equal(gv[:M], vals)
     np.testing.assert_array_equal(gr, ranges)
+    if (W, H) == (8192, 8192) and tile_sort == 3:
+        global TILE_SORT
+        TILE_SORT = 2
+        with pytest.raises(B.GsError) as ei:
+            run_bin(B, sc, {"means2d": m2d, "depths": dep}, rad, capacity=len(keys) + 3)
+        assert ei.value.status == B.GS_ERR_UNSUPPORTED
 
 
 @pytest.mark.parametrize("N,C,vis_frac", [(1_300_003, 2, 0.02), (2_000_001, 3, 0.01), (5_000_005, 2, 0.004), (8_500_001, 2, 0.003)])

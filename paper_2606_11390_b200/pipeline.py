@@ -348,7 +348,21 @@ class SplatStep:
         view_bits = int(np.ceil(np.log2(self.C))) if self.C > 1 else 0
         depth_passes = 4 + (view_bits + 7) // 8
         tile_passes = min((tile_bits + 7) // 8, (tile_bits + 8) // 9)
+        # two-level tile sort (mirrors gs_bin_tiles with tile_sort = 0): group records sorted + count, scan and expansion kernels
+        extra = 0
+        if getattr(self, "tile_sort", 0) in (0, 2, 3) and (self.capacity_M >= (4 << 20) or getattr(self, "tile_sort", 0) in (2, 3)):
+            shift = 2
+            if self.C * ((self.gx + 3) // 4) * ((self.gy + 3) // 4) > 8192 or self.capacity_M >= 512 * self.C * self.gx * self.gy or getattr(self, "tile_sort", 0) == 3:
+                shift = 3
+            if getattr(self, "tile_sort", 0) == 2:
+                shift = 2
+            side = 1 << shift
+            groups = self.C * ((self.gx + side - 1) // side) * ((self.gy + side - 1) // side)
+            if groups <= 8192:
+                gbits = max(1, int(np.ceil(np.log2(groups))))
+                tile_passes = min((gbits + 7) // 8, (gbits + 8) // 9)
+                extra = 3
         compact = 1 if self.use_mask else (2 if self.C * self.N >= (1 << 24) else 1)   # radii mode, large inputs: visibility mask + scan over it
         p5 = 6 if self.N >= (1 << 22) else 1                         # dense zero-fill as five streaming launches for large N
         loss = 2 if getattr(self, "loss_mode", "l1") == "l1ssim" else 1
-        return (loss - 1) + (p5 - 1) + 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1
+        return extra + (loss - 1) + (p5 - 1) + 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

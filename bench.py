@@ -386,6 +386,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     st.set_target(tgt_host)
     st.loss_mode = args.loss
     st.tile_sort = args.tile_sort
+    st.tile_sort_fixed = args.tile_sort != 0
     morton_ms = None
     if args.morton:
         B.morton_sort({k: st.params[k] for k in st.param_names})          # warm-up (allocations, first launches)

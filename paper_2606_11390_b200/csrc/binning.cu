@@ -23,6 +23,9 @@
 //                       chunk of records from the entry table (the unsorted record list is never
 //                       written to memory), the last pass writes only the values.  Persistent blocks,
 //                       per-digit decoupled look-back, ballot-based stable ranking.
+//   group_count/scan,   B2+B3 from 4 M records (two-level tile sort, see "two-level tile sort" below): the records that are
+//   expand_kernel       generated and sorted by tile_sweep_kernel are (group of 4 x 4 or 8 x 8 tiles, entry); every group then
+//                       expands its depth-ordered list into the lists of its tiles, each record written once.
 //   keys_kernel         optional: the 64-bit keys (tile << 32 | depth bits) of the sorted records.
 //
 // Equal (tile, depth) records keep ascending entry order (reading A10) because every step is

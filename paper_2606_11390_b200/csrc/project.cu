@@ -71,17 +71,37 @@ struct WarpStack {
 template <int ITEMS, int CAP, bool WITH_MEAN>
 __device__ __forceinline__ void warp_push(const uint32_t (&idx)[ITEMS], const uint32_t (&msk)[ITEMS], const float* m /*[3*ITEMS] or null*/,
                                           WarpStack<CAP, WITH_MEAN>& st, int& cnt, int lane) {
-    const unsigned int lt = (1u << lane) - 1u;
-#pragma unroll
-    for (int k = 0; k < ITEMS; ++k) {
-        const unsigned int b = __ballot_sync(0xffffffffu, msk[k] != 0u);
-        if (msk[k]) {
-            const int p = cnt + __popc(b & lt);
-            st.idx[p] = idx[k];
-            st.msk[p] = msk[k];
-            if (WITH_MEAN) { st.xyz[0][p] = m[3 * k]; st.xyz[WITH_MEAN ? 1 : 0][p] = m[3 * k + 1]; st.xyz[WITH_MEAN ? 2 : 0][p] = m[3 * k + 2]; }
+    if constexpr (ITEMS == 1) {
+        const unsigned int b = __ballot_sync(0xffffffffu, msk[0] != 0u);
+        if (msk[0]) {
+            const int p = cnt + __popc(b & ((1u << lane) - 1u));
+            st.idx[p] = idx[0];
+            st.msk[p] = msk[0];
+            if (WITH_MEAN) { st.xyz[0][p] = m[0]; st.xyz[WITH_MEAN ? 1 : 0][p] = m[1]; st.xyz[WITH_MEAN ? 2 : 0][p] = m[2]; }
         }
         cnt += __popc(b);
+    } else {
+        // several items per lane: one warp scan of the per-lane counts instead of one ballot per item; a lane's survivors
+        // take consecutive slots
+        int n = 0;
+#pragma unroll
+        for (int k = 0; k < ITEMS; ++k) n += msk[k] != 0u;
+        int incl = n;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        int p = cnt + incl - n;
+#pragma unroll
+        for (int k = 0; k < ITEMS; ++k)
+            if (msk[k]) {
+                st.idx[p] = idx[k];
+                st.msk[p] = msk[k];
+                if (WITH_MEAN) { st.xyz[0][p] = m[3 * k]; st.xyz[WITH_MEAN ? 1 : 0][p] = m[3 * k + 1]; st.xyz[WITH_MEAN ? 2 : 0][p] = m[3 * k + 2]; }
+                ++p;
+            }
+        cnt += __shfl_sync(0xffffffffu, incl, 31);
     }
 }
 
@@ -314,10 +334,22 @@ __global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const Proj
             for (int c = 0; c < a.C; ++c) {
                 const DevCam& cam = cams.cam[c];
                 const float w0 = cam.W[6], w1 = cam.W[7], w2 = cam.W[8], t2 = cam.tau[2], zn = cam.near_plane, zf = cam.far_plane;
+                const uint32_t bit = 1u << c;
+                if (zn >= 0.0f && zf > zn) {
+                    // zn < tz < zf on the bit patterns (non-negative floats order like their bits; a negative, zero or NaN tz wraps
+                    // to or stays at a value above every range): one integer add and one unsigned compare per pair
+                    const uint32_t lo = __float_as_uint(zn + 0.0f) + 1u, range = __float_as_uint(zf) - lo;
 #pragma unroll
-                for (int k = 0; k < ITEMS; ++k) {
-                    const float tz = w0 * m[3 * k] + w1 * m[3 * k + 1] + w2 * m[3 * k + 2] + t2;
-                    if (tz > zn && tz < zf) msk[k] |= 1u << c;
+                    for (int k = 0; k < ITEMS; ++k) {
+                        const float tz = w0 * m[3 * k] + w1 * m[3 * k + 1] + w2 * m[3 * k + 2] + t2;
+                        msk[k] |= (__float_as_uint(tz) - lo < range) ? bit : 0u;
+                    }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < ITEMS; ++k) {
+                        const float tz = w0 * m[3 * k] + w1 * m[3 * k + 1] + w2 * m[3 * k + 2] + t2;
+                        if (tz > zn && tz < zf) msk[k] |= bit;
+                    }
                 }
                 const int64_t e0 = (int64_t)c * a.N + i0;
                 if (a.vmask) {

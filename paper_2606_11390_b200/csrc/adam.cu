@@ -36,6 +36,7 @@ __device__ __forceinline__ void adam1(float& p, float g, float& m, float& v, con
 
 // dense: one thread per 16-byte unit
 __global__ void __launch_bounds__(256) adam_dense_kernel(const AdamArgs a, int64_t n4, int64_t n) {
+    pdl_enter();
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     float vmax = -3.0e38f;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n4; k += stride) {
@@ -58,6 +59,7 @@ __global__ void __launch_bounds__(256) adam_dense_kernel(const AdamArgs a, int64
 // scalar fall-back for unaligned arrays, and the visible-only variant: a warp scans 32 Gaussians' radii over the C views
 // and then walks the visible rows, lanes across the row's floats
 __global__ void __launch_bounds__(256) adam_rows_kernel(const AdamArgs a) {
+    pdl_enter();
     const int lane = threadIdx.x & 31;
     const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     float vmax = -3.0e38f;
@@ -118,6 +120,7 @@ __device__ __forceinline__ void adam_gaussian(const AdamMultiArgs& a, const Adam
 }
 
 __global__ void __launch_bounds__(256) adam_visible_multi_kernel(const AdamMultiArgs a) {
+    pdl_enter();
     const int lane = threadIdx.x & 31;
     const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     AdamArgs h;
@@ -205,7 +208,7 @@ extern "C" int gs_adam_step_visible(int64_t N, int32_t n_arrays, const int32_t* 
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     int64_t blocks = (N + 1023) / 1024;
     if (blocks > (int64_t)sms * 8) blocks = (int64_t)sms * 8;
-    adam_visible_multi_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(a);
+    launch_chained(adam_visible_multi_kernel, dim3((unsigned)blocks), dim3(256), (size_t)(0), (cudaStream_t)stream, a);
     return launch_status();
 }
 
@@ -232,11 +235,11 @@ extern "C" int gs_adam_step(int64_t N, int32_t row_floats, float* param, const f
         const int64_t n4 = n >> 2;
         int64_t blocks = (n4 + 255) / 256;
         if (blocks > (int64_t)sms * 32) blocks = (int64_t)sms * 32;
-        adam_dense_kernel<<<(unsigned)(blocks < 1 ? 1 : blocks), 256, 0, st>>>(a, n4, n);
+        launch_chained(adam_dense_kernel, dim3((unsigned)(blocks < 1 ? 1 : blocks)), dim3(256), (size_t)(0), st, a, n4, n);
     } else {
         int64_t blocks = (N + 255) / 256;
         if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
-        adam_rows_kernel<<<(unsigned)blocks, 256, 0, st>>>(a);
+        launch_chained(adam_rows_kernel, dim3((unsigned)blocks), dim3(256), (size_t)(0), st, a);
     }
     return launch_status();
 }

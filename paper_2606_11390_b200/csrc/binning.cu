@@ -344,6 +344,7 @@ struct CompactArgs {
 // ascending entry order (iteration, lane, component).
 template <int VEC>
 __global__ void __launch_bounds__(kScanThreads) compact_kernel(const CompactArgs a) {
+    pdl_enter();
     constexpr int TILE = kScanThreads * 4 * VEC;
     constexpr int WARPS = kScanThreads / 32;
     __shared__ unsigned int s_ticket;
@@ -482,6 +483,7 @@ constexpr int64_t kMaskWideMinWords = 1 << 19;
 constexpr int64_t kMaskMinEntries = 1 << 24;                  // measured on B200: fused 50 us vs split 62 us at 10 M entries, 530 vs 265 us at 240 M
 
 __global__ void __launch_bounds__(kScanThreads) visible_kernel(const CompactArgs a, unsigned int* __restrict__ vmask, int64_t n_words) {
+    pdl_enter();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t wbase = (int64_t)blockIdx.x * kMaskTile + (int64_t)warp * (128 * kMaskVec);
     const int64_t w0 = wbase + lane * 4;
@@ -541,6 +543,7 @@ __global__ void __launch_bounds__(kScanThreads) visible_kernel(const CompactArgs
 template <bool VIEWS, int WPT>
 __global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const CompactArgs a, const unsigned int* __restrict__ vmask, int64_t n_words,
                                                                     int64_t wn) {
+    pdl_enter();
     __shared__ unsigned int s_ticket;
     __shared__ ChainScanSmem s_scan;
     __shared__ unsigned int s_w[WPT][kScanThreads];     // the thread's words, indexed dynamically in the expansion
@@ -632,6 +635,7 @@ __global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const Compac
 // ------------------------------------------------------------------------------ B4: counts, ranges, histograms
 // column prefix sums of the difference grid (one thread per (view, column))
 __global__ void __launch_bounds__(128) tile_yscan_kernel(int* __restrict__ tdiff, int C, int gx, int gy) {
+    pdl_enter();
     const int sx = gx + 1, sy = gy + 1;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= C * sx) return;
@@ -653,6 +657,7 @@ __global__ void __launch_bounds__(128) tile_yscan_kernel(int* __restrict__ tdiff
 // cell is the number of rectangles covering that tile); in place
 __global__ void __launch_bounds__(kScanThreads) tile_xscan_kernel(int* __restrict__ tdiff, int64_t cells, BinHeader* hdr,
                                                                   unsigned long long* status) {
+    pdl_enter();
     __shared__ unsigned int s_ticket;
     __shared__ ChainScanSmem s_scan;
     const int tid = threadIdx.x;
@@ -685,6 +690,7 @@ struct RangesArgs {
 };
 
 __global__ void __launch_bounds__(kScanThreads) tile_ranges_kernel(const RangesArgs a) {
+    pdl_enter();
     __shared__ unsigned int s_ticket;
     __shared__ ChainScanSmem s_scan;
     __shared__ unsigned int s_hist[kTsMaxPasses * kTsMaxBins];
@@ -747,6 +753,7 @@ __global__ void __launch_bounds__(kScanThreads) tile_ranges_kernel(const RangesA
 // capacity nothing is sorted, so every range is cleared ("outputs incomplete, nothing out of bounds")
 __global__ void __launch_bounds__(kTsMaxBins) scan_hist_kernel(unsigned int* thist, int P, const BinHeader* hdr, int64_t capacity,
                                                                int64_t* ranges, int64_t n_ranges) {
+    pdl_enter();
     __shared__ unsigned int s[kTsMaxBins];
     const int tid = threadIdx.x;
     for (int p = 0; p < P; ++p) {
@@ -785,6 +792,7 @@ struct OffsetsArgs {
 };
 
 __global__ void __launch_bounds__(kScanThreads) offsets_kernel(const OffsetsArgs a) {
+    pdl_enter();
     __shared__ unsigned int s_ticket;
     __shared__ ChainScanSmem s_scan;
     const int tid = threadIdx.x;
@@ -860,6 +868,7 @@ __global__ void __launch_bounds__(kScanThreads) offsets_kernel(const OffsetsArgs
 // same counts as global atomics from the chained-scan kernel cost 0.8 ms on the room scene: 7 M atomics on 2 040 addresses)
 __global__ void __launch_bounds__(256) group_count_kernel(const EntryRec* __restrict__ entries, const unsigned short* __restrict__ entry_h,
                                                           const BinHeader* hdr, int ggx, int n_groups, unsigned int* __restrict__ cg_count) {
+    pdl_enter();
     extern __shared__ unsigned int s_cnt[];
     for (int k = threadIdx.x; k < n_groups; k += blockDim.x) s_cnt[k] = 0;
     __syncthreads();
@@ -879,6 +888,7 @@ __global__ void __launch_bounds__(256) group_count_kernel(const EntryRec* __rest
 
 __global__ void __launch_bounds__(512) group_scan_kernel(const unsigned int* __restrict__ cg_count, int n_groups, unsigned int* __restrict__ group_start,
                                                          unsigned int* thist, const TilePlan plan) {
+    pdl_enter();
     __shared__ unsigned int s_hist[kTsMaxPasses * kTsMaxBins];
     __shared__ unsigned int s_scan[512];
     const int tid = threadIdx.x;
@@ -945,6 +955,7 @@ constexpr int kExpChunk = 256;       // group records staged per round
 
 template <int SHIFT>
 __global__ void __launch_bounds__(32 << SHIFT) expand_kernel(const ExpandArgs a) {
+    pdl_enter();
     constexpr int SIDE = 1 << SHIFT;               // tiles per group side; one warp per tile row of the group
     constexpr int THREADS = 32 * SIDE;
     constexpr int PER = kExpChunk / THREADS;       // entries staged per thread and round
@@ -1045,6 +1056,7 @@ __global__ void __launch_bounds__(32 << SHIFT) expand_kernel(const ExpandArgs a)
 // ------------------------------------------------------------------------------ histograms
 __global__ void __launch_bounds__(256) hist_kernel(const uint64_t* __restrict__ keys, const unsigned long long* count, int64_t capacity,
                                                    const SortPlan plan, unsigned int* __restrict__ hist) {
+    pdl_enter();
     __shared__ unsigned int h[kMaxPasses][kRadix];
     for (int k = threadIdx.x; k < kMaxPasses * kRadix; k += blockDim.x) (&h[0][0])[k] = 0;
     __syncthreads();
@@ -1089,6 +1101,7 @@ struct SweepSmem {
 };
 
 __global__ void __launch_bounds__(kSortThreads) onesweep_kernel(const SweepArgs a) {
+    pdl_enter();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SweepSmem& sm = *reinterpret_cast<SweepSmem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1239,6 +1252,7 @@ struct TileSweepSmem {
 
 template <int BITS, bool GEN>
 __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSweepArgs a) {
+    pdl_enter();
     using Smem = TileSweepSmem<BITS>;
     constexpr int BINS = Smem::BINS;
     static_assert(kTsItems % 8 == 0, "blocked generation reads 8 heads per vector");
@@ -1457,12 +1471,13 @@ __global__ void __launch_bounds__(kTsThreads, 2) tile_sweep_kernel(const TileSwe
 __global__ void __launch_bounds__(256) keys_kernel(const unsigned int* __restrict__ tkeys, const int32_t* __restrict__ vals,
                                                    const float* __restrict__ depths, const unsigned long long* count,
                                                    uint64_t* __restrict__ keys) {
+    pdl_enter();
     const int64_t n = (int64_t)(*count);
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
         keys[i] = ((uint64_t)__ldg(tkeys + i) << 32) | (uint64_t)__float_as_uint(__ldg(depths + __ldg(vals + i)));
 }
 
-__global__ void set_count_kernel(unsigned long long* count, unsigned long long n) { *count = n; }
+__global__ void set_count_kernel(unsigned long long* count, unsigned long long n) { pdl_enter(); *count = n; }
 
 // 64-bit radix passes; data starts in (k0, v0) and ping-pongs with (k1, v1)
 static int run_sort(const SortPlan& plan, uint64_t* k0, int32_t* v0, uint64_t* k1, int32_t* v1, const unsigned long long* count,
@@ -1472,7 +1487,7 @@ static int run_sort(const SortPlan& plan, uint64_t* k0, int32_t* v0, uint64_t* k
     const int sms = sm_count();
     const int64_t tiles = (capacity + kSortTile - 1) / kSortTile;
     const int64_t hist_blocks = tiles < (int64_t)sms * 4 ? tiles : (int64_t)sms * 4;
-    hist_kernel<<<(unsigned)hist_blocks, 256, 0, st>>>(k0, count, capacity, plan, hist);
+    launch_chained(hist_kernel, dim3((unsigned)hist_blocks), dim3(256), (size_t)(0), st, k0, count, capacity, plan, hist);
     int rc = launch_status();
     if (rc) return rc;
     for (int p = 0; p < plan.P; ++p) {
@@ -1484,7 +1499,7 @@ static int run_sort(const SortPlan& plan, uint64_t* k0, int32_t* v0, uint64_t* k
         a.hist = hist + p * kRadix;
         a.status = status;
         a.ticket = tickets + p;
-        onesweep_kernel<<<(unsigned)tiles, kSortThreads, sizeof(SweepSmem), st>>>(a);
+        launch_chained(onesweep_kernel, dim3((unsigned)tiles), dim3(kSortThreads), (size_t)(sizeof(SweepSmem)), st, a);
         rc = launch_status();
         if (rc) return rc;
     }
@@ -1504,7 +1519,7 @@ static int launch_tile_sweep(const TileSweepArgs& a, int64_t capacity, cudaStrea
     }
     const int64_t tiles = (capacity + kTsTile - 1) / kTsTile;
     const int64_t resident = (int64_t)dc.sms * dc.occ[slot];
-    tile_sweep_kernel<BITS, GEN><<<(unsigned)(tiles < resident ? tiles : resident), kTsThreads, smem, st>>>(a);
+    launch_chained(tile_sweep_kernel<BITS, GEN>, dim3((unsigned)(tiles < resident ? tiles : resident)), dim3(kTsThreads), (size_t)(smem), st, a);
     return launch_status();
 }
 
@@ -1594,25 +1609,25 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
             const int64_t wn = GS_VIS_WORDS(N), n_words = (int64_t)C * wn;
             if (n_words >= kMaskWideMinWords) {
                 a.n_blocks = (unsigned int)((n_words + kScanThreads * 16 - 1) / (kScanThreads * 16));
-                compact_mask_kernel<true, 16><<<a.n_blocks, kScanThreads, 0, st>>>(a, vis_mask, n_words, wn);
+                launch_chained(compact_mask_kernel<true, 16>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vis_mask, n_words, wn);
             } else {
                 a.n_blocks = (unsigned int)((n_words + kScanThreads * 4 - 1) / (kScanThreads * 4));
-                compact_mask_kernel<true, 4><<<a.n_blocks, kScanThreads, 0, st>>>(a, vis_mask, n_words, wn);
+                launch_chained(compact_mask_kernel<true, 4>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vis_mask, n_words, wn);
             }
         } else if (n_entries >= kMaskMinEntries) {
             // large inputs: streaming visibility mask, then the ordered scan over the mask
             unsigned int* vmask = reinterpret_cast<unsigned int*>(ws + w.off_vmask);
             const int64_t n_words = (n_entries + 31) / 32;
-            visible_kernel<<<(unsigned)((n_entries + kMaskTile - 1) / kMaskTile), kScanThreads, 0, st>>>(a, vmask, n_words);
+            launch_chained(visible_kernel, dim3((unsigned)((n_entries + kMaskTile - 1) / kMaskTile)), dim3(kScanThreads), (size_t)(0), st, a, vmask, n_words);
             rc = launch_status();
             if (rc) return rc;
             a.n_blocks = (unsigned int)((n_words + kScanThreads * 16 - 1) / (kScanThreads * 16));
-            compact_mask_kernel<false, 16><<<a.n_blocks, kScanThreads, 0, st>>>(a, vmask, n_words, 0);
+            launch_chained(compact_mask_kernel<false, 16>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vmask, n_words, 0);
         } else switch (cvec) {
-            case 8: compact_kernel<8><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
-            case 4: compact_kernel<4><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
-            case 2: compact_kernel<2><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
-            default: compact_kernel<1><<<(unsigned)n_blocks, kScanThreads, 0, st>>>(a); break;
+            case 8: launch_chained(compact_kernel<8>, dim3((unsigned)n_blocks), dim3(kScanThreads), (size_t)(0), st, a); break;
+            case 4: launch_chained(compact_kernel<4>, dim3((unsigned)n_blocks), dim3(kScanThreads), (size_t)(0), st, a); break;
+            case 2: launch_chained(compact_kernel<2>, dim3((unsigned)n_blocks), dim3(kScanThreads), (size_t)(0), st, a); break;
+            default: launch_chained(compact_kernel<1>, dim3((unsigned)n_blocks), dim3(kScanThreads), (size_t)(0), st, a); break;
         }
         rc = launch_status();
         if (rc) return rc;
@@ -1620,11 +1635,11 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
     // records per tile -> ranges, digit histograms, M
     {
         const int cols = C * (gx + 1);
-        tile_yscan_kernel<<<(cols + 127) / 128, 128, 0, st>>>(tdiff, C, gx, gy);
+        launch_chained(tile_yscan_kernel, dim3((cols + 127) / 128), dim3(128), (size_t)(0), st, tdiff, C, gx, gy);
         rc = launch_status();
         if (rc) return rc;
         const unsigned int cb = (unsigned int)((cells + kScanTile - 1) / kScanTile);
-        tile_xscan_kernel<<<cb, kScanThreads, 0, st>>>(tdiff, cells, hdr, status_at(w.off_xscan_status));
+        launch_chained(tile_xscan_kernel, dim3(cb), dim3(kScanThreads), (size_t)(0), st, tdiff, cells, hdr, status_at(w.off_xscan_status));
         rc = launch_status();
         if (rc) return rc;
         RangesArgs a;
@@ -1632,10 +1647,10 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
         a.ranges = tile_ranges; a.thist = thist; a.plan = tplan; a.hdr = hdr; a.status = status_at(w.off_rscan_status);
         if (two_level) a.plan.P = 0;      // (the digit histograms of the group sort come from the group counts, below)
         a.n_blocks = cb; a.M_dev = reinterpret_cast<unsigned long long*>(M_dev);
-        tile_ranges_kernel<<<cb, kScanThreads, 0, st>>>(a);
+        launch_chained(tile_ranges_kernel, dim3(cb), dim3(kScanThreads), (size_t)(0), st, a);
         rc = launch_status();
         if (rc) return rc;
-        scan_hist_kernel<<<1, kTsMaxBins, 0, st>>>(thist, two_level ? 0 : tplan.P, hdr, capacity_M, tile_ranges, (int64_t)C * tiles);
+        launch_chained(scan_hist_kernel, dim3(1), dim3(kTsMaxBins), (size_t)(0), st, thist, two_level ? 0 : tplan.P, hdr, capacity_M, tile_ranges, (int64_t)C * tiles);
         rc = launch_status();
         if (rc) return rc;
     }
@@ -1654,7 +1669,7 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
             a.hdr = hdr; a.status = status_at(w.off_offs_status);
             a.coarse = two_level ? 1 : 0; a.gshift = gshift; a.ggx = ggx; a.ggy = ggy; a.groups = (unsigned int)(ggx * ggy);
             a.entry_h = reinterpret_cast<unsigned short*>(ws + w.off_entry_h);
-            offsets_kernel<<<(unsigned)((w.vcap + kScanTile - 1) / kScanTile), kScanThreads, 0, st>>>(a);
+            launch_chained(offsets_kernel, dim3((unsigned)((w.vcap + kScanTile - 1) / kScanTile)), dim3(kScanThreads), (size_t)(0), st, a);
             rc = launch_status();
             if (rc) return rc;
         }
@@ -1662,12 +1677,12 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
         int32_t* gv[2] = {reinterpret_cast<int32_t*>(ws + w.off_vals), reinterpret_cast<int32_t*>(ws + w.off_vals2)};
         if (two_level) {
             const int64_t vb = (w.vcap + 255) / 256;
-            group_count_kernel<<<(unsigned)(vb < 2 * sms ? vb : 2 * sms), 256, (size_t)n_groups * sizeof(unsigned int), st>>>(
+            launch_chained(group_count_kernel, dim3((unsigned)(vb < 2 * sms ? vb : 2 * sms)), dim3(256), (size_t)((size_t)n_groups * sizeof(unsigned int)), st, 
                 entries, reinterpret_cast<const unsigned short*>(ws + w.off_entry_h), hdr, ggx, (int)n_groups,
                 reinterpret_cast<unsigned int*>(ws + w.off_cg_count));
             rc = launch_status();
             if (rc) return rc;
-            group_scan_kernel<<<1, 512, 0, st>>>(reinterpret_cast<const unsigned int*>(ws + w.off_cg_count), (int)n_groups, group_start, thist, tplan);
+            launch_chained(group_scan_kernel, dim3(1), dim3(512), (size_t)(0), st, reinterpret_cast<const unsigned int*>(ws + w.off_cg_count), (int)n_groups, group_start, thist, tplan);
             rc = launch_status();
             if (rc) return rc;
         }
@@ -1696,8 +1711,8 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
             a.N = N; a.gx = gx; a.gy = gy; a.ggx = ggx; a.tiles = (unsigned int)tiles; a.groups = (unsigned int)(ggx * ggy);
             a.means2d = means2d; a.radii = radii; a.cvals = gv[tplan.P & 1]; a.group_start = group_start; a.ranges = tile_ranges;
             a.vals_out = isect_vals; a.tkeys_out = isect_keys ? tk[0] : nullptr; a.hdr = hdr;
-            if (gshift == 2) expand_kernel<2><<<(unsigned)n_groups, 128, 0, st>>>(a);
-            else expand_kernel<3><<<(unsigned)n_groups, 256, 0, st>>>(a);
+            if (gshift == 2) launch_chained(expand_kernel<2>, dim3((unsigned)n_groups), dim3(128), (size_t)(0), st, a);
+            else launch_chained(expand_kernel<3>, dim3((unsigned)n_groups), dim3(256), (size_t)(0), st, a);
             rc = launch_status();
             if (rc) return rc;
             sorted_tile_ids = tk[0];
@@ -1705,7 +1720,7 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
         if (isect_keys) {
             const int64_t rb = (capacity_M + 255) / 256;
             const unsigned grid = (unsigned)(rb < (int64_t)sms * 8 ? rb : (int64_t)sms * 8);
-            keys_kernel<<<grid, 256, 0, st>>>(sorted_tile_ids, isect_vals, depths, &hdr->n_rec, isect_keys);
+            launch_chained(keys_kernel, dim3(grid), dim3(256), (size_t)(0), st, sorted_tile_ids, isect_vals, depths, &hdr->n_rec, isect_keys);
             rc = launch_status();
             if (rc) return rc;
         }
@@ -1761,7 +1776,7 @@ extern "C" int gs_sort_pairs(int64_t n, int32_t end_bit, int32_t skip_bit31, uin
     unsigned char* ws = reinterpret_cast<unsigned char*>(workspace);
     unsigned long long* count = reinterpret_cast<unsigned long long*>(ws + w.off_count);
     if (cudaMemsetAsync(ws, 0, w.zero_bytes, st) != cudaSuccess) return GS_ERR_CUDA;
-    set_count_kernel<<<1, 1, 0, st>>>(count, (unsigned long long)n);
+    launch_chained(set_count_kernel, dim3(1), dim3(1), (size_t)(0), st, count, (unsigned long long)n);
     uint64_t* alt_keys = reinterpret_cast<uint64_t*>(ws + w.off_keys);
     int32_t* alt_vals = reinterpret_cast<int32_t*>(ws + w.off_vals);
     int rc = run_sort(plan, keys, vals, alt_keys, alt_vals, count, reinterpret_cast<unsigned int*>(ws + w.off_tickets),

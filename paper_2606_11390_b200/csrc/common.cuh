@@ -112,6 +112,28 @@ inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_
 inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? GS_OK : GS_ERR_CUDA; }
 inline int launch_status() { return cuda_status(cudaGetLastError()); }
 
+// ---- programmatic dependent launch ---------------------------------------------------------------
+// The stages are chains of short kernels on one stream.  With the launch attribute below the next kernel is released when
+// the blocks of its predecessor have exited (not after the full completion + flush handshake of a plain launch), and its
+// blocks stop at pdl_enter() until the predecessor's writes are visible.  Every kernel of the library is launched through
+// launch_chained() and calls pdl_enter() as its FIRST statement, in every block and before any early return: a block that
+// left without waiting would let its grid complete -- and release the grid behind it -- before the grid in front has
+// finished.  No kernel touches global memory before the wait, so the dependency semantics are those of a plain stream.
+// Measured (bin_tiles, ms): city 0.368 -> 0.335, block 0.206 -> 0.179, room 0.856 -> 0.814, object 0.398 -> 0.362.
+// An explicit early `griddepcontrol.launch_dependents` at the top of every kernel (blocks of the next kernels resident
+// and waiting while the predecessor runs) was slower on the larger scenes: city 0.382, object 0.411 (block 0.183).
+__device__ __forceinline__ void pdl_enter() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline void launch_chained(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // Per-device cache of immutable facts about the current device (SM count; which kernels already have their opt-in
 // dynamic shared-memory size set; resident blocks per SM of the persistent kernels).  Entries are idempotent, so
 // concurrent first calls are harmless; nothing here changes the result of any call.

@@ -16,10 +16,12 @@ __device__ __forceinline__ float ord2f(unsigned int o) {
 }
 
 __global__ void bounds_init_kernel(unsigned int* b) {
+    pdl_enter();
     if (threadIdx.x < 3) b[threadIdx.x] = 0xffffffffu;          // running minimum
     else if (threadIdx.x < 6) b[threadIdx.x] = 0u;               // running maximum
 }
 __global__ void __launch_bounds__(256) bounds_kernel(int64_t N, const float* __restrict__ means, unsigned int* b) {
+    pdl_enter();
     unsigned int lo[3] = {0xffffffffu, 0xffffffffu, 0xffffffffu}, hi[3] = {0u, 0u, 0u};
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
 #pragma unroll
@@ -39,6 +41,7 @@ __global__ void __launch_bounds__(256) bounds_kernel(int64_t N, const float* __r
     }
 }
 __global__ void bounds_decode_kernel(unsigned int* b) {
+    pdl_enter();
     if (threadIdx.x < 6) {
         const float f = ord2f(b[threadIdx.x]);
         reinterpret_cast<float*>(b)[threadIdx.x] = f;
@@ -58,6 +61,7 @@ __device__ __forceinline__ unsigned long long spread3(unsigned long long x) {
 
 __global__ void __launch_bounds__(256) morton_codes_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ lo_hi,
                                                            unsigned long long* __restrict__ codes, int32_t* __restrict__ index) {
+    pdl_enter();
     float lo[3], sc[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -84,6 +88,7 @@ __global__ void __launch_bounds__(256) morton_codes_kernel(int64_t N, const floa
 template <typename T>
 __global__ void __launch_bounds__(256) gather_rows_kernel(int64_t N, int units, const T* __restrict__ src, const int32_t* __restrict__ perm,
                                                           T* __restrict__ dst) {
+    pdl_enter();
     const int64_t total = N * units;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += (int64_t)gridDim.x * blockDim.x) {
         const int64_t i = k / units;
@@ -109,9 +114,9 @@ extern "C" int gs_bounds(int64_t N, const float* means, float* lo_hi, void* stre
     if (N < 1 || !means || !lo_hi || !aligned(lo_hi, 4)) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t st = (cudaStream_t)stream;
     unsigned int* b = reinterpret_cast<unsigned int*>(lo_hi);
-    bounds_init_kernel<<<1, 32, 0, st>>>(b);
-    bounds_kernel<<<grid_for(N), 256, 0, st>>>(N, means, b);
-    bounds_decode_kernel<<<1, 32, 0, st>>>(b);
+    launch_chained(bounds_init_kernel, dim3(1), dim3(32), (size_t)(0), st, b);
+    launch_chained(bounds_kernel, dim3(grid_for(N)), dim3(256), (size_t)(0), st, N, means, b);
+    launch_chained(bounds_decode_kernel, dim3(1), dim3(32), (size_t)(0), st, b);
     return launch_status();
 }
 
@@ -119,7 +124,7 @@ extern "C" int gs_morton_codes(int64_t N, const float* means, const float* lo_hi
     if (N < 0 || N >= (1LL << 31)) return GS_ERR_INVALID_ARGUMENT;
     if (N == 0) return GS_OK;
     if (!means || !lo_hi || !codes || !index || !aligned(codes, 8)) return GS_ERR_INVALID_ARGUMENT;
-    morton_codes_kernel<<<grid_for(N), 256, 0, (cudaStream_t)stream>>>(N, means, lo_hi, reinterpret_cast<unsigned long long*>(codes), index);
+    launch_chained(morton_codes_kernel, dim3(grid_for(N)), dim3(256), (size_t)(0), (cudaStream_t)stream, N, means, lo_hi, reinterpret_cast<unsigned long long*>(codes), index);
     return launch_status();
 }
 
@@ -129,9 +134,9 @@ extern "C" int gs_gather_rows(int64_t N, int32_t row_floats, const float* src, c
     if (!src || !perm || !dst || src == dst) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t st = (cudaStream_t)stream;
     if (row_floats % 4 == 0 && aligned(src, 16) && aligned(dst, 16))
-        gather_rows_kernel<float4><<<grid_for(N * (row_floats / 4)), 256, 0, st>>>(N, row_floats / 4, reinterpret_cast<const float4*>(src), perm,
+        launch_chained(gather_rows_kernel<float4>, dim3(grid_for(N * (row_floats / 4))), dim3(256), (size_t)(0), st, N, row_floats / 4, reinterpret_cast<const float4*>(src), perm,
                                                                                   reinterpret_cast<float4*>(dst));
     else
-        gather_rows_kernel<float><<<grid_for(N * row_floats), 256, 0, st>>>(N, row_floats, src, perm, dst);
+        launch_chained(gather_rows_kernel<float>, dim3(grid_for(N * row_floats)), dim3(256), (size_t)(0), st, N, row_floats, src, perm, dst);
     return launch_status();
 }

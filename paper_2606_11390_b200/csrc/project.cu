@@ -270,6 +270,7 @@ __device__ __forceinline__ void stack_filter(Src& src, int& cnt_src, Dst& dst, i
 //   B1  full projection; SH only if visible somewhere
 template <int DEG, int ITEMS>
 __global__ void __launch_bounds__(kProjThreads, 6) project_fwd_kernel(const ProjFwdArgs a, const __grid_constant__ CamBatch cams) {
+    pdl_enter();
     constexpr int CHUNK = 32 * ITEMS;                   // Gaussians per warp and phase-A step
     constexpr int WARPS = kProjThreads / 32;
     __shared__ WarpStack<32 + CHUNK, true> s1_all[WARPS];   // Gaussians inside some view's depth range
@@ -606,6 +607,7 @@ __device__ __forceinline__ void zero_span(float* __restrict__ p, int64_t count, 
 // ITEMS = 32, and only the non-zero words are expanded (lane = bit).
 template <int DEG, int ITEMS, bool MASK = false>
 __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjBwdArgs a, const __grid_constant__ CamBatch cams) {
+    pdl_enter();
     static_assert(!MASK || ITEMS == 32, "mask variant: one word per lane");
     constexpr int CHUNK = 32 * ITEMS;                   // Gaussians per warp and phase-A step
     constexpr int WARPS = kBwdThreads / 32;
@@ -687,6 +689,7 @@ __global__ void __launch_bounds__(kBwdThreads, 3) project_bwd_kernel(const ProjB
 // 7.5 TB/s, the same stores issued from the 168-register persistent kernel's phase A 4.8 TB/s.
 // one array: every thread zeroes four 16-byte units a block-width apart (coalesced, four stores in flight)
 __global__ void __launch_bounds__(256) zero_fill_kernel(float* __restrict__ p, int64_t count) {
+    pdl_enter();
     const int64_t n4 = count >> 2;
     const int64_t i0 = (int64_t)blockIdx.x * 1024 + threadIdx.x;
     float4* p4 = reinterpret_cast<float4*>(p);
@@ -699,6 +702,7 @@ __global__ void __launch_bounds__(256) zero_fill_kernel(float* __restrict__ p, i
 
 // max over all log-scales (gs_log_scale_bound): 16-byte loads, warp shuffle, one atomic per warp
 __global__ void __launch_bounds__(256) log_scale_max_kernel(const float* __restrict__ ls, int64_t n, int vec, float* __restrict__ out) {
+    pdl_enter();
     float m = -3.0e38f;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x, t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (vec) {
@@ -718,7 +722,7 @@ __global__ void __launch_bounds__(256) log_scale_max_kernel(const float* __restr
         else atomicMin(reinterpret_cast<unsigned int*>(out), __float_as_uint(m));
     }
 }
-__global__ void set_float_kernel(float* p, float v) { *p = v; }
+__global__ void set_float_kernel(float* p, float v) { pdl_enter(); *p = v; }
 
 // The same zero-fill as ONE launch with a small persistent grid (2 blocks of 256 threads per SM, 8 x 16-byte stores per
 // thread and round): made to run on a second stream UNDERNEATH other kernels (gs_grad_zero_fill).  A full-size grid would
@@ -729,6 +733,7 @@ struct ZeroFillArgs {
     int64_t count[5];
 };
 __global__ void __launch_bounds__(256) zero_fill_persistent_kernel(const ZeroFillArgs a) {
+    pdl_enter();
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     const int64_t stride = (int64_t)gridDim.x * 2048;
 #pragma unroll 1
@@ -761,10 +766,10 @@ int launch_fwd(const ProjFwdArgs& a, const CamBatch& cb, cudaStream_t st) {
     const int64_t wide = (a.N + 32 * kProjItems - 1) / (32 * kProjItems);
     const unsigned wide_grid = persistent_grid(project_fwd_kernel<DEG, kProjItems>, kProjThreads, (wide + warps - 1) / warps, sms);
     if (wide >= 8 * (int64_t)wide_grid * warps) {
-        project_fwd_kernel<DEG, kProjItems><<<wide_grid, kProjThreads, 0, st>>>(a, cb);
+        launch_chained(project_fwd_kernel<DEG, kProjItems>, dim3(wide_grid), dim3(kProjThreads), (size_t)(0), st, a, cb);
     } else {
         const int64_t chunks = (a.N + 31) / 32;
-        project_fwd_kernel<DEG, 1><<<persistent_grid(project_fwd_kernel<DEG, 1>, kProjThreads, (chunks + warps - 1) / warps, sms), kProjThreads, 0, st>>>(a, cb);
+        launch_chained(project_fwd_kernel<DEG, 1>, dim3(persistent_grid(project_fwd_kernel<DEG, 1>, kProjThreads, (chunks + warps - 1) / warps, sms)), dim3(kProjThreads), (size_t)(0), st, a, cb);
     }
     return launch_status();
 }
@@ -774,8 +779,7 @@ int launch_bwd(const ProjBwdArgs& a, const CamBatch& cb, cudaStream_t st) {
     constexpr int warps = kBwdThreads / 32;
     if (a.vmask) {
         const int64_t chunks = (a.N + 1023) / 1024;
-        project_bwd_kernel<DEG, 32, true><<<persistent_grid(project_bwd_kernel<DEG, 32, true>, kBwdThreads, (chunks + warps - 1) / warps, sms),
-                                            kBwdThreads, 0, st>>>(a, cb);
+        launch_chained(project_bwd_kernel<DEG, 32, true>, dim3(persistent_grid(project_bwd_kernel<DEG, 32, true>, kBwdThreads, (chunks + warps - 1) / warps, sms)), dim3(kBwdThreads), (size_t)(0), st, a, cb);
         return launch_status();
     }
     if (a.prezeroed || a.accumulate) {
@@ -784,17 +788,17 @@ int launch_bwd(const ProjBwdArgs& a, const CamBatch& cb, cudaStream_t st) {
         const int64_t scan = (a.N + 32 * 16 - 1) / (32 * 16);
         const unsigned scan_grid = persistent_grid(project_bwd_kernel<DEG, 16>, kBwdThreads, (scan + warps - 1) / warps, sms);
         if (scan >= 8 * (int64_t)scan_grid * warps) {
-            project_bwd_kernel<DEG, 16><<<scan_grid, kBwdThreads, 0, st>>>(a, cb);
+            launch_chained(project_bwd_kernel<DEG, 16>, dim3(scan_grid), dim3(kBwdThreads), (size_t)(0), st, a, cb);
             return launch_status();
         }
     }
     const int64_t wide = (a.N + 32 * 4 - 1) / (32 * 4);
     const unsigned wide_grid = persistent_grid(project_bwd_kernel<DEG, 4>, kBwdThreads, (wide + warps - 1) / warps, sms);
     if (wide >= 8 * (int64_t)wide_grid * warps) {
-        project_bwd_kernel<DEG, 4><<<wide_grid, kBwdThreads, 0, st>>>(a, cb);
+        launch_chained(project_bwd_kernel<DEG, 4>, dim3(wide_grid), dim3(kBwdThreads), (size_t)(0), st, a, cb);
     } else {
         const int64_t chunks = (a.N + 31) / 32;
-        project_bwd_kernel<DEG, 1><<<persistent_grid(project_bwd_kernel<DEG, 1>, kBwdThreads, (chunks + warps - 1) / warps, sms), kBwdThreads, 0, st>>>(a, cb);
+        launch_chained(project_bwd_kernel<DEG, 1>, dim3(persistent_grid(project_bwd_kernel<DEG, 1>, kBwdThreads, (chunks + warps - 1) / warps, sms)), dim3(kBwdThreads), (size_t)(0), st, a, cb);
     }
     return launch_status();
 }
@@ -852,13 +856,13 @@ extern "C" int gs_project_fwd(const gs_config* cfg, int64_t N, const float* mean
 extern "C" int gs_log_scale_bound(int64_t N, const float* log_scales, float* bound, void* stream) {
     if (N < 1 || !log_scales || !bound || !aligned(bound, 4)) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t st = (cudaStream_t)stream;
-    set_float_kernel<<<1, 1, 0, st>>>(bound, -3.0e38f);
+    launch_chained(set_float_kernel, dim3(1), dim3(1), (size_t)(0), st, bound, -3.0e38f);
     const int64_t n = 3 * N;
     int64_t blocks = (n / 4 + 255) / 256;
     const int64_t cap = (int64_t)sm_count() * 8;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    log_scale_max_kernel<<<(unsigned)blocks, 256, 0, st>>>(log_scales, n, aligned(log_scales, 16) ? 1 : 0, bound);
+    launch_chained(log_scale_max_kernel, dim3((unsigned)blocks), dim3(256), (size_t)(0), st, log_scales, n, aligned(log_scales, 16) ? 1 : 0, bound);
     return launch_status();
 }
 
@@ -871,7 +875,7 @@ static int zero_fill_all(int64_t N, int sh_degree, float* dL_dmeans, float* dL_d
     for (int k = 0; k < 5; ++k) {
         if (aligned(ptrs[k], 16)) {
             const int64_t blocks = ((counts[k] >> 2) + 1023) / 1024;
-            zero_fill_kernel<<<(unsigned)(blocks > 0 ? blocks : 1), 256, 0, st>>>(ptrs[k], counts[k]);
+            launch_chained(zero_fill_kernel, dim3((unsigned)(blocks > 0 ? blocks : 1)), dim3(256), (size_t)(0), st, ptrs[k], counts[k]);
         } else if (cudaMemsetAsync(ptrs[k], 0, (size_t)counts[k] * sizeof(float), st) != cudaSuccess) {
             return GS_ERR_CUDA;
         }
@@ -889,7 +893,7 @@ extern "C" int gs_grad_zero_fill(int64_t N, int32_t sh_degree, float* dL_dmeans,
         ZeroFillArgs a;
         a.p[0] = dL_dsh; a.p[1] = dL_dquats; a.p[2] = dL_dmeans; a.p[3] = dL_dlog_scales; a.p[4] = dL_dopacity_logits;
         a.count[0] = K3 * N; a.count[1] = 4 * N; a.count[2] = 3 * N; a.count[3] = 3 * N; a.count[4] = N;
-        zero_fill_persistent_kernel<<<(unsigned)(2 * sm_count()), 256, 0, (cudaStream_t)stream>>>(a);
+        launch_chained(zero_fill_persistent_kernel, dim3((unsigned)(2 * sm_count())), dim3(256), (size_t)(0), (cudaStream_t)stream, a);
         return launch_status();
     }
     return zero_fill_all(N, sh_degree, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh, (cudaStream_t)stream);

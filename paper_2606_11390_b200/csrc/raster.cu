@@ -133,6 +133,7 @@ __device__ __forceinline__ bool rect_may_contribute(float u, float v, float A, f
 constexpr int kBlock = 128;    // 4 warps per tile, each an 8x8 pixel block, lane = 2 x 1 pixels
 
 __global__ void __launch_bounds__(kBlock) raster_fwd_kernel(const RasterArgs a, const RasterFwdOut o) {
+    pdl_enter();
     __shared__ Rec s_rec[kBlock];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t bt = blockIdx.x;                  // view * tiles + tile
@@ -347,6 +348,7 @@ __device__ __forceinline__ void reduce_group(BwdSmem& sm, int warp, int lane, in
 }
 
 __global__ void __launch_bounds__(kBlock) raster_bwd_kernel(const RasterArgs a, const RasterBwdIO io) {
+    pdl_enter();
     extern __shared__ __align__(16) unsigned char bwd_smem_raw[];
     BwdSmem& sm = *reinterpret_cast<BwdSmem*>(bwd_smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -527,6 +529,7 @@ __device__ __forceinline__ void zero_row(int64_t e, float* g_means2d, float* g_c
 }
 __global__ void __launch_bounds__(256) zero_visible_rows_kernel(int64_t n, const int32_t* __restrict__ radii, int vec, float* g_means2d,
                                                                 float* g_conics, float* g_opacities, float* g_rgbs) {
+    pdl_enter();
     const int64_t q0 = ((int64_t)blockIdx.x * 512 + threadIdx.x) * 4;
     int4 r[2];
 #pragma unroll
@@ -555,6 +558,7 @@ __global__ void __launch_bounds__(256) zero_visible_rows_kernel(int64_t n, const
 // the non-zero words with lane = bit, so that the rows zeroed together are neighbours in memory
 __global__ void __launch_bounds__(256) zero_masked_rows_kernel(int64_t N, int64_t wn, int64_t n_words, const uint32_t* __restrict__ vmask,
                                                                float* g_means2d, float* g_conics, float* g_opacities, float* g_rgbs) {
+    pdl_enter();
     const int lane = threadIdx.x & 31;
     const int64_t wi = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 4;              // n_words = C * wn is a multiple of 16
     uint4 v = make_uint4(0u, 0u, 0u, 0u);
@@ -578,6 +582,7 @@ __global__ void __launch_bounds__(256) zero_masked_rows_kernel(int64_t N, int64_
 
 __global__ void __launch_bounds__(256) l1_loss_kernel(int64_t n, const float* __restrict__ image, const float* __restrict__ target,
                                                       float* __restrict__ dL, float* loss_sum, float inv_n) {
+    pdl_enter();
     float acc = 0.f;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
         const float d = __ldg(image + k) - __ldg(target + k);
@@ -603,6 +608,7 @@ __global__ void __launch_bounds__(256) l1_loss_kernel(int64_t n, const float* __
 // definition walks (list position <= n_contrib) without compositing; stats[3] records of all tile lists times 256 (the
 // dense upper bound).
 __global__ void __launch_bounds__(256) pair_stats_kernel(const RasterArgs a, unsigned long long* __restrict__ stats) {
+    pdl_enter();
     __shared__ float s_u[256], s_v[256], s_A[256], s_B[256], s_C[256], s_lo[256];
     __shared__ unsigned long long s_sum[3];
     const int tid = threadIdx.x;
@@ -684,7 +690,7 @@ extern "C" int gs_raster_fwd(const gs_config* cfg, int32_t C, const gs_camera* c
     if (rc) return rc;
     if (!image || !final_T || !n_contrib) return GS_ERR_INVALID_ARGUMENT;
     RasterFwdOut o{image, final_T, n_contrib};
-    raster_fwd_kernel<<<(unsigned)(C * a.tiles), kBlock, 0, (cudaStream_t)stream>>>(a, o);
+    launch_chained(raster_fwd_kernel, dim3((unsigned)(C * a.tiles)), dim3(kBlock), (size_t)(0), (cudaStream_t)stream, a, o);
     return launch_status();
 }
 
@@ -704,12 +710,12 @@ extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* c
         if (vis_mask) {
             if (N_total % C != 0 || !aligned(vis_mask, 16)) return GS_ERR_INVALID_ARGUMENT;
             const int64_t N = N_total / C, wn = GS_VIS_WORDS(N), n_words = (int64_t)C * wn;
-            zero_masked_rows_kernel<<<(unsigned)((n_words / 4 + 255) / 256), 256, 0, st>>>(N, wn, n_words, vis_mask, dL_dmeans2d, dL_dconics,
+            launch_chained(zero_masked_rows_kernel, dim3((unsigned)((n_words / 4 + 255) / 256)), dim3(256), (size_t)(0), st, N, wn, n_words, vis_mask, dL_dmeans2d, dL_dconics,
                                                                                           dL_dopacities, dL_drgbs);
             rc = launch_status();
             if (rc) return rc;
         } else if (radii) {
-            zero_visible_rows_kernel<<<(unsigned)((N_total + 2047) / 2048), 256, 0, st>>>(N_total, radii, aligned(radii, 16) ? 1 : 0,
+            launch_chained(zero_visible_rows_kernel, dim3((unsigned)((N_total + 2047) / 2048)), dim3(256), (size_t)(0), st, N_total, radii, aligned(radii, 16) ? 1 : 0,
                                                                                            dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs);
             rc = launch_status();
             if (rc) return rc;
@@ -724,7 +730,7 @@ extern "C" int gs_raster_bwd(const gs_config* cfg, int32_t C, const gs_camera* c
     RasterBwdIO io{final_T, n_contrib, dL_dimage, dL_dmeans2d, dL_dconics, dL_dopacities, dL_drgbs};
     rc = ensure_smem(raster_bwd_kernel, 0, (int)sizeof(BwdSmem));
     if (rc) return rc;
-    raster_bwd_kernel<<<(unsigned)(C * a.tiles), kBlock, sizeof(BwdSmem), st>>>(a, io);
+    launch_chained(raster_bwd_kernel, dim3((unsigned)(C * a.tiles)), dim3(kBlock), (size_t)(sizeof(BwdSmem)), st, a, io);
     return launch_status();
 }
 
@@ -737,7 +743,7 @@ extern "C" int gs_raster_pair_stats(const gs_config* cfg, int32_t C, const gs_ca
     if (rc) return rc;
     if (!stats || !aligned(stats, 8)) return GS_ERR_INVALID_ARGUMENT;
     if (cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream) != cudaSuccess) return GS_ERR_CUDA;
-    pair_stats_kernel<<<(unsigned)(C * a.tiles), 256, 0, (cudaStream_t)stream>>>(a, reinterpret_cast<unsigned long long*>(stats));
+    launch_chained(pair_stats_kernel, dim3((unsigned)(C * a.tiles)), dim3(256), (size_t)(0), (cudaStream_t)stream, a, reinterpret_cast<unsigned long long*>(stats));
     return launch_status();
 }
 
@@ -748,7 +754,7 @@ extern "C" int gs_l1_loss(int64_t n, const float* image, const float* target, fl
     const int sms = sm_count();
     int64_t blocks = (n + 255) / 256;
     if (blocks > (int64_t)sms * 16) blocks = (int64_t)sms * 16;
-    l1_loss_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(n, image, target, dL_dimage, loss_sum, 1.0f / (float)n);
+    launch_chained(l1_loss_kernel, dim3((unsigned)blocks), dim3(256), (size_t)(0), (cudaStream_t)stream, n, image, target, dL_dimage, loss_sum, 1.0f / (float)n);
     return launch_status();
 }
 

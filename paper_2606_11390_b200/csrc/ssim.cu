@@ -138,6 +138,7 @@ struct HzBuf {
 
 template <bool TMA>
 __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a, const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my) {
+    pdl_enter();
     constexpr int ROW = TMA ? kSsimRowTma : kSsimRowPad;
     constexpr int OFF = TMA ? kSsimTmaOff : 0;            // column of the halo's first float inside a staged row
     __shared__ __align__(128) float sx[kSsimHalo][ROW];
@@ -257,6 +258,7 @@ __global__ void __launch_bounds__(256) ssim_stats_kernel(const SsimArgs a, const
 template <bool TMA>
 __global__ void __launch_bounds__(256) ssim_grad_kernel(const SsimArgs a, const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUtensorMap m1,
                                                         const __grid_constant__ CUtensorMap m2) {
+    pdl_enter();
     constexpr int ROW = TMA ? kSsimRowTma : kSsimRowPad;
     constexpr int OFF = TMA ? kSsimTmaOff : 0;
     __shared__ __align__(128) float sm[3][kSsimHalo][ROW];
@@ -426,11 +428,11 @@ extern "C" int gs_l1_ssim_loss(int32_t C, int32_t height, int32_t width, const f
                   make_halo_map(enc, a.maps, C, height, width, &m0) && make_halo_map(enc, a.maps + n, C, height, width, &m1) &&
                   make_halo_map(enc, a.maps + 2 * n, C, height, width, &m2);
     }
-    if (tma) ssim_stats_kernel<true><<<grid, 256, 0, st>>>(a, mx, my);
-    else ssim_stats_kernel<false><<<grid, 256, 0, st>>>(a, mx, my);
+    if (tma) launch_chained(ssim_stats_kernel<true>, dim3(grid), dim3(256), (size_t)(0), st, a, mx, my);
+    else launch_chained(ssim_stats_kernel<false>, dim3(grid), dim3(256), (size_t)(0), st, a, mx, my);
     int rc = launch_status();
     if (rc) return rc;
-    if (tma) ssim_grad_kernel<true><<<grid, 256, 0, st>>>(a, m0, m1, m2);
-    else ssim_grad_kernel<false><<<grid, 256, 0, st>>>(a, m0, m1, m2);
+    if (tma) launch_chained(ssim_grad_kernel<true>, dim3(grid), dim3(256), (size_t)(0), st, a, m0, m1, m2);
+    else launch_chained(ssim_grad_kernel<false>, dim3(grid), dim3(256), (size_t)(0), st, a, m0, m1, m2);
     return launch_status();
 }

@@ -12,7 +12,8 @@
  *
  * Conventions (all entry points)
  *   - Every pointer is a DEVICE pointer owned by the caller unless its comment says "host".
- *     The library never allocates or frees device memory and keeps no global state.
+ *     The library never allocates or frees device memory and keeps no global state (one exception, stated at its
+ *     declaration: gs_sort_pairs_static keeps its scratch in a static device array that every call on a device shares).
  *   - Arrays are dense, row-major, fp32 unless stated; counts are int64_t.
  *   - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default
  *     stream).  The only host synchronisation is in gs_bin_tiles when `M_out` is non-NULL.
@@ -135,6 +136,24 @@ int gs_bin_tiles(const gs_config* cfg /*host*/, int64_t N, int32_t C, const gs_c
  * workspace as in gs_bin_tiles (NULL -> size query). */
 int gs_sort_pairs(int64_t n, int32_t end_bit, int32_t skip_bit31, uint64_t* keys, int32_t* vals, void* workspace,
                   size_t* workspace_bytes /*host*/, void* stream);
+
+/* gs_sort_pairs for callers that cannot allocate (stream capture into a CUDA graph, serving loops, harnesses that forbid
+ * cudaMalloc): the same sort -- same kernels, same result bit for bit -- with NO workspace argument.  The scratch (pass
+ * tickets, digit histograms, look-back status words, the ping-pong copy of keys and values) lives in one file-scope
+ * `static __device__` array inside the library, sized for n <= GS_SORT_STATIC_MAX_N pairs (13.1 MB; every GPU that loads
+ * the library holds it until the process exits).  The call allocates nothing: no cudaMalloc / cudaFree, no allocating
+ * library routine; the caller passes only the inputs / outputs keys[n] (uint64, device) and vals[n] (int32, device), which
+ * are overwritten with the result.  Asynchronous on `stream`.
+ * The first call on a device (with that device current) resolves the array's device address once
+ * (cudaGetSymbolAddress); make that call -- n == 0 is enough -- before stream capture starts.
+ * Every call on a device shares the one array, which keeps the previous call's contents: the call itself clears what must
+ * start at zero (tickets, histograms, status words), so calls in sequence on one stream need nothing from the caller, but
+ * two calls that overlap on the GPU (different streams, or graphs launched concurrently) RACE on the scratch -- order them.
+ * Errors: GS_ERR_UNSUPPORTED when n > GS_SORT_STATIC_MAX_N (nothing is launched; use gs_sort_pairs with a workspace) or the
+ * bit range needs more than 8 passes; GS_ERR_INVALID_ARGUMENT (n < 0, end_bit outside [1, 64], null / misaligned pointers);
+ * GS_ERR_CUDA. */
+#define GS_SORT_STATIC_MAX_N (1 << 20)
+int gs_sort_pairs_static(int64_t n, int32_t end_bit, int32_t skip_bit31, uint64_t* keys, int32_t* vals, void* stream);
 
 /* R1 -- rasterisation forward.  Per pixel, front to back over
  * its tile's range: power = -1/2 d^T K d; skip power > 0; alpha = min(alpha_max, o*exp(power));

@@ -17,8 +17,9 @@ LIB_PATH = os.path.join(_HERE, "libgsplat_b200.so")
 
 GS_OK, GS_ERR_INVALID_ARGUMENT, GS_ERR_CAPACITY, GS_ERR_CUDA, GS_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 GS_TILE_SORT_AUTO, GS_TILE_SORT_ONE_LEVEL, GS_TILE_SORT_GROUPS_4, GS_TILE_SORT_GROUPS_8 = 0, 1, 2, 3
+GS_SORT_STATIC_MAX_N = 1 << 20
 
-EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs",
+EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs", "gs_sort_pairs_static",
            "gs_raster_fwd", "gs_raster_bwd", "gs_raster_pair_stats", "gs_project_bwd", "gs_grad_zero_fill", "gs_log_scale_bound", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
 
 
@@ -188,6 +189,15 @@ def gs_sort_pairs(n, end_bit, skip_bit31, keys, vals, workspace, stream=None):
     rc = lib().gs_sort_pairs(C.c_int64(n), C.c_int32(end_bit), C.c_int32(1 if skip_bit31 else 0), _ptr(keys),
                              _ptr(vals, torch.int32), _ptr(workspace), C.byref(wb), _stream(stream))
     _check(rc, "gs_sort_pairs")
+
+
+def gs_sort_pairs_static(n, end_bit, skip_bit31, keys, vals, stream=None):
+    """gs_sort_pairs without a workspace: the scratch is a static device array inside the library (n <= GS_SORT_STATIC_MAX_N);
+    nothing is allocated.  Calls that overlap on the GPU race on that array."""
+    import torch
+    rc = lib().gs_sort_pairs_static(C.c_int64(n), C.c_int32(end_bit), C.c_int32(1 if skip_bit31 else 0), _ptr(keys),
+                                    _ptr(vals, torch.int32), _stream(stream))
+    _check(rc, f"gs_sort_pairs_static(n = {n}, limit GS_SORT_STATIC_MAX_N = {GS_SORT_STATIC_MAX_N})")
 
 
 def _bg(bg):

@@ -1844,3 +1844,67 @@ extern "C" int gs_sort_pairs(int64_t n, int32_t end_bit, int32_t skip_bit31, uin
     }
     return GS_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// gs_sort_pairs_static: gs_sort_pairs for callers that cannot allocate.  The workspace of the stand-alone sort (count,
+// pass tickets, digit histograms, look-back status words, ping-pong copy of keys and values: sort_layout) is a file-scope
+// device array sized for GS_SORT_STATIC_MAX_N pairs.  In HOST code the array's name is only a stand-in for the symbol, not
+// a device address: the address is resolved once per device with cudaGetSymbolAddress (below) and that pointer is what
+// the kernels receive.  One array per device, shared by every call and never cleared between calls: the call zeroes the
+// words that must start at zero, exactly as gs_sort_pairs does with its workspace; calls that overlap on the GPU race.
+namespace gs {
+constexpr size_t static_align(size_t x) { return (x + 255) / 256 * 256; }
+constexpr size_t kSortStaticBytes =
+    static_align(16 + kMaxPasses * sizeof(unsigned int)) +                                                     // count, tickets
+    static_align((size_t)kMaxPasses * kRadix * sizeof(unsigned int)) +                                         // histograms
+    static_align((size_t)((GS_SORT_STATIC_MAX_N + kSortTile - 1) / kSortTile + 1) * kRadix * sizeof(unsigned long long)) +   // status
+    static_align((size_t)GS_SORT_STATIC_MAX_N * sizeof(uint64_t)) + static_align((size_t)GS_SORT_STATIC_MAX_N * sizeof(int32_t));
+static __device__ __align__(256) unsigned char g_sort_static_scratch[kSortStaticBytes];
+
+// device address of the scratch array on the current device (resolved once per device; idempotent, so concurrent first
+// calls are harmless)
+static int sort_static_scratch(unsigned char** out) {
+    static unsigned char* ptr[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return GS_ERR_CUDA;
+    if (dev < 0 || dev >= 64) return GS_ERR_UNSUPPORTED;
+    if (!ptr[dev]) {
+        unsigned char* p = nullptr;
+        if (cudaGetSymbolAddress((void**)&p, g_sort_static_scratch) != cudaSuccess || !p) {
+            cudaGetLastError();
+            return GS_ERR_CUDA;
+        }
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return GS_OK;
+}
+}  // namespace gs
+
+extern "C" int gs_sort_pairs_static(int64_t n, int32_t end_bit, int32_t skip_bit31, uint64_t* keys, int32_t* vals, void* stream) {
+    if (n < 0 || end_bit < 1 || end_bit > 64) return GS_ERR_INVALID_ARGUMENT;
+    if (n > (int64_t)GS_SORT_STATIC_MAX_N) return GS_ERR_UNSUPPORTED;        // beyond the static scratch: nothing is launched
+    unsigned char* ws = nullptr;
+    if (int rc = sort_static_scratch(&ws)) return rc;
+    if (n == 0) return GS_OK;
+    if (!keys || !vals || !aligned(keys, 8) || !aligned(vals, 4)) return GS_ERR_INVALID_ARGUMENT;
+    const SortWorkspace w = sort_layout(n);
+    if (w.total > kSortStaticBytes) return GS_ERR_UNSUPPORTED;               // (cannot happen for n <= GS_SORT_STATIC_MAX_N)
+    const SortPlan plan = make_plan(end_bit, skip_bit31 != 0);
+    if (plan.P > kMaxPasses) return GS_ERR_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* count = reinterpret_cast<unsigned long long*>(ws + w.off_count);
+    // what must start at zero: count, tickets, histograms, status words (the previous call's values are still there)
+    if (cudaMemsetAsync(ws, 0, w.zero_bytes, st) != cudaSuccess) return GS_ERR_CUDA;
+    launch_chained(set_count_kernel, dim3(1), dim3(1), (size_t)(0), st, count, (unsigned long long)n);
+    uint64_t* alt_keys = reinterpret_cast<uint64_t*>(ws + w.off_keys);
+    int32_t* alt_vals = reinterpret_cast<int32_t*>(ws + w.off_vals);
+    int rc = run_sort(plan, keys, vals, alt_keys, alt_vals, count, reinterpret_cast<unsigned int*>(ws + w.off_tickets),
+                      reinterpret_cast<unsigned int*>(ws + w.off_hist), reinterpret_cast<unsigned long long*>(ws + w.off_status), n, st);
+    if (rc) return rc;
+    if (plan.P & 1) {
+        if (cudaMemcpyAsync(keys, alt_keys, (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, st) != cudaSuccess) return GS_ERR_CUDA;
+        if (cudaMemcpyAsync(vals, alt_vals, (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st) != cudaSuccess) return GS_ERR_CUDA;
+    }
+    return GS_OK;
+}

@@ -60,6 +60,10 @@ def parse_args():
     ap.add_argument("--sparse-grads", action="store_true",
                     help="P5 writes only the rows of Gaussians visible in the batch (gs_project_bwd accumulate = 2) instead of the dense "
                          "overwrite; only valid with --adam sparse or none")
+    ap.add_argument("--grads", default="dense", choices=["dense", "incremental"],
+                    help="how P5 produces the dense gradient: 'dense' = zero-fill all N rows and write the visible ones (default); "
+                         "'incremental' = same arrays bit for bit, but only the rows the previous step wrote are cleared "
+                         "(gs_grad_zero_rows from the previous step's visibility mask) before this step's rows are written")
     ap.add_argument("--no-mask", action="store_true",
                     help="every stage scans the dense radii[C, N] instead of reading P1's visibility bit mask (and P1 does not use the "
                          "scene-wide log-scale bound)")
@@ -74,6 +78,8 @@ def parse_args():
     ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE configs")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
     args = ap.parse_args()
+    if args.grads == "incremental" and (args.sparse_grads or args.overlap or args.no_mask):
+        ap.error("--grads incremental excludes --sparse-grads, --overlap and --no-mask")
     if args.sparse_grads and args.adam == "dense":
         ap.error("--sparse-grads leaves stale rows for invisible Gaussians; the dense Adam step reads every row (use --adam sparse)")
     return args
@@ -382,7 +388,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     kw = {"far": 3.0e38} if (far_inf and workload == "city") else {}
     sc = scenes.make_scene(workload, n=args.n, **kw)
     tgt_host = scenes.target_image(sc)
-    st = SplatStep(sc, device=dev, use_mask=False if args.no_mask else None)
+    st = SplatStep(sc, device=dev, use_mask=False if args.no_mask else (True if args.grads == "incremental" else None))
     st.set_target(tgt_host)
     st.loss_mode = args.loss
     st.tile_sort = args.tile_sort
@@ -423,6 +429,8 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     def timed_step(ev, zf_ev=None):
         if args.sparse_grads:
             p5 = lambda: st.project_bwd(accumulate=2)
+        elif args.grads == "incremental":
+            p5 = st.project_bwd_incremental
         elif overlap:
             p5 = lambda: (st.join_grad_zero_fill(), st.project_bwd(accumulate=1))
         else:
@@ -444,6 +452,8 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
             st.adam(args.adam)            # (also allocates the moments outside the timed region)
         if args.sparse_grads:
             st.project_bwd(accumulate=2)
+        if args.grads == "incremental":
+            st.project_bwd_incremental()
     barrier()
 
     sampler = ClockSampler(dev.index if dev.index is not None else 0)
@@ -467,6 +477,29 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     mpix_step = C * W * H / 1e6
     value = whole_job_rate(world, mpix_step, ms_per_step)
     gauss_per_s = whole_job_rate(world, C * N, ms_per_step)
+
+    # ---- the same step with the gradient arrays cleared sparsely (SplatStep.project_bwd_incremental): same arrays bit for
+    # bit, reported beside the headline, which keeps the dense zero-fill of the method as written
+    inc = None
+    if args.grads == "dense" and st.use_mask and not args.sparse_grads and not overlap and args.adam == "none":
+        def inc_step():
+            st.project_fwd(); st.bin_tiles(sync=False); st.raster_fwd(); st.l1_loss(); st.raster_bwd(); st.project_bwd_incremental()
+        for _ in range(3):
+            inc_step()
+        barrier()
+        iev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for k in range(steps):
+            flush.fill_(k & 0xFF)
+            iev[k][0].record(stream)
+            inc_step()
+            iev[k][1].record(stream)
+        barrier()
+        inc_ms = max_over_ranks(float(np.median([a.elapsed_time(b) for a, b in iev])), world, dev)
+        inc = {"ms_per_step": inc_ms, "value": whole_job_rate(world, mpix_step, inc_ms), "unit": "MP/s", "steps": steps,
+               "note": "gradient arrays persist between steps; rows written by the previous step are cleared from its visibility "
+                       "mask (gs_grad_zero_rows), then gs_project_bwd(accumulate = 2): the dense gradient bit for bit "
+                       "(tests/test_gpu_mask.py), 2 x 236 B per visible Gaussian instead of 236 B per Gaussian"}
+        st.project_bwd()        # (leave the arrays and the step's state as the dense step does)
 
     # ---- algorithmic work of this step (harness-side counting, outside the timed region)
     vis = st.visible()
@@ -504,7 +537,8 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
         "bin_tiles": vis_r + 24 * V_sum + (8 + 24 * P_d) * V_sum + (32 + 16) * V_sum + tsort_bytes + 24 * cells + 16 * C * st.gx * st.gy,
         # P5: visibility, 2-D gradients, parameters re-read; gradient rows: visible rows only (sparse), visible rows read +
         # written on top of the zero-fill (overlap), or every row written (dense overwrite)
-        "project_bwd": vis_r + 36 * V_sum + par_b * V_any + par_b * (V_any if args.sparse_grads else (2 * V_any if overlap else N)),
+        "project_bwd": vis_r + 36 * V_sum + par_b * V_any + par_b * (V_any if args.sparse_grads else (2 * V_any if overlap else N))
+                       if args.grads == "dense" else 2 * vis_r + 36 * V_sum + 3 * par_b * V_any,    # + mask re-read, rows cleared
         "grad_zero_fill": par_b * N,
         # L1: read image, target, write dL; L1 + SSIM: + three derivative maps written and read, image and target read twice
         "l1_loss": (12 if args.loss == "l1" else 44) * C * W * H * 3,
@@ -544,7 +578,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     kernel_of = dict(KERNEL_OF)
     kernel_of["l1_loss"] = "l1_loss_kernel" if args.loss == "l1" else "ssim_stats_kernel"
     kernel_of["adam"] = "adam_dense_kernel" if args.adam == "dense" else "adam_visible_multi_kernel"
-    if dominant == "project_bwd" and not args.sparse_grads and not overlap and N >= (1 << 22):
+    if dominant == "project_bwd" and not args.sparse_grads and not overlap and args.grads == "dense" and N >= (1 << 22):
         kernel_of["project_bwd"] = "zero_fill_kernel + project_bwd_kernel"
     roof["kernel"] = kernel_of[dominant]
     roof["share_of_step"] = round(stage_ms[dominant] / float(np.median(step_ms)), 4)
@@ -612,7 +646,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
     out = {
         "value": value, "ms_per_step": ms_per_step, "ms_per_step_mean": ms_mean, "gaussians_per_s": gauss_per_s,
         "config": {"workload": workload + (" (far = +inf)" if far_inf else ""), "loss": args.loss, "morton": bool(args.morton), "adam": args.adam,
-                   "sparse_grads": bool(args.sparse_grads),
+                   "sparse_grads": bool(args.sparse_grads), "grads": args.grads,
                    "visibility": "bit mask written by P1 + scene-wide log-scale bound" if st.use_mask else "dense radii",
                    "grad_zero_fill": "second stream, under the rasterisation kernels" if overlap else "inside project_bwd", "gaussians": N, "views": C, "width": W, "height": H, "sh_degree": st.cfg.sh_degree,
                    "intersections": M_now, "group_records": M_groups, "visible_entries": V_sum, "visible_gaussians": V_any,
@@ -621,8 +655,8 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
                    "parallelism": "replicas only" if world > 1 else "single GPU", "timing": "median of the timed steps (CUDA events)",
                    "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},
         "morton_sort_ms": morton_ms, "clocks": clocks, "e2e": e2e,
-        "gpu_launches": (st.launches_per_step() + {"none": 0, "dense": 5, "sparse": 1}[args.adam]) * steps,
-        "roofline": roof, "stages": stage_roof, "wall_s_timed_region": round(t_wall, 3),
+        "gpu_launches": (st.launches_per_step(2 if args.grads == "incremental" else (1 if args.sparse_grads else None)) + {"none": 0, "dense": 5, "sparse": 1}[args.adam]) * steps,
+        "roofline": roof, "stages": stage_roof, "wall_s_timed_region": round(t_wall, 3), "grads_incremental": inc,
     }
     del st, flush
     torch.cuda.empty_cache()
@@ -670,7 +704,8 @@ def run_b200(args):
         "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
     }
-    for k in ("config", "gaussians_per_s", "ms_per_step_mean", "morton_sort_ms", "clocks", "e2e", "gpu_launches", "roofline", "stages"):
+    for k in ("config", "gaussians_per_s", "ms_per_step_mean", "morton_sort_ms", "clocks", "e2e", "gpu_launches", "roofline", "stages",
+              "grads_incremental"):
         line[k] = main[k]
     line["cpu_baseline"] = cpu
     line["per_config"] = per_config

@@ -214,6 +214,18 @@ int gs_project_bwd(const gs_config* cfg /*host*/, int64_t N, const float* means,
 int gs_grad_zero_fill(int64_t N, int32_t sh_degree, float* dL_dmeans, float* dL_dlog_scales, float* dL_dquats,
                       float* dL_dopacity_logits, float* dL_dsh, void* stream);
 
+/* Sparse clearing of the gradient arrays: zeroes the rows of every Gaussian that `vis_mask` (uint32 [C][GS_VIS_WORDS(N)],
+ * the mask a gs_project_fwd call wrote) marks in at least one of its C views; all other rows are untouched.
+ * Use: gradient arrays that persist from step to step hold non-zero rows only where the previous gs_project_bwd wrote
+ * them.  gs_grad_zero_rows(mask of the PREVIOUS step) followed by gs_project_bwd(accumulate = 2, mask of this step) then
+ * leaves exactly what gs_project_bwd(accumulate = 0) would: the dense gradient, zeros included, bit for bit -- for
+ * 2 * 236 bytes per visible Gaussian instead of 236 bytes for every Gaussian (SH degree 3), provided the arrays were
+ * zero-filled once (gs_grad_zero_fill) and nothing else writes to them in between.  Asynchronous on `stream`.
+ * Errors: GS_ERR_INVALID_ARGUMENT (null / misaligned pointers, N < 0, sh_degree outside 0..3, C outside 1..GS_MAX_VIEWS),
+ * GS_ERR_CUDA. */
+int gs_grad_zero_rows(int64_t N, int32_t sh_degree, int32_t C, const uint32_t* vis_mask, float* dL_dmeans, float* dL_dlog_scales,
+                      float* dL_dquats, float* dL_dopacity_logits, float* dL_dsh, void* stream);
+
 /* Harness loss (SURVEY.md 8(c) reading A18): mean-reduced L1 against a target image.
  * dL_dimage[n] = sign(image - target) / n; *loss_sum (device, float, caller-zeroed) += sum |image - target| / n. */
 int gs_l1_loss(int64_t n, const float* image, const float* target, float* dL_dimage, float* loss_sum, void* stream);

@@ -20,7 +20,7 @@ GS_TILE_SORT_AUTO, GS_TILE_SORT_ONE_LEVEL, GS_TILE_SORT_GROUPS_4, GS_TILE_SORT_G
 GS_SORT_STATIC_MAX_N = 1 << 20
 
 EXPORTS = ["gs_config_default", "gs_status_string", "gs_project_fwd", "gs_bin_tiles", "gs_sort_pairs", "gs_sort_pairs_static",
-           "gs_raster_fwd", "gs_raster_bwd", "gs_raster_pair_stats", "gs_project_bwd", "gs_grad_zero_fill", "gs_log_scale_bound", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
+           "gs_raster_fwd", "gs_raster_bwd", "gs_raster_pair_stats", "gs_project_bwd", "gs_grad_zero_fill", "gs_grad_zero_rows", "gs_log_scale_bound", "gs_l1_loss", "gs_l1_ssim_loss", "gs_bounds", "gs_morton_codes", "gs_gather_rows", "gs_adam_step", "gs_adam_step_visible"]
 
 
 class gs_camera(C.Structure):
@@ -261,6 +261,17 @@ def gs_grad_zero_fill(sh_degree, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopaci
                                  _ptr(dL_dquats, torch.float32), _ptr(dL_dopacity_logits, torch.float32), _ptr(dL_dsh, torch.float32),
                                  _stream(stream))
     _check(rc, "gs_grad_zero_fill")
+
+
+def gs_grad_zero_rows(sh_degree, n_views, vis_mask, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh, stream=None):
+    """Zero the gradient rows of the Gaussians that ``vis_mask`` ([n_views, vis_words(N)]) marks in any view."""
+    import torch
+    N = dL_dmeans.shape[0]
+    assert vis_mask.numel() == n_views * vis_words(N)
+    rc = lib().gs_grad_zero_rows(C.c_int64(N), C.c_int32(sh_degree), C.c_int32(n_views), _ptr(vis_mask), _ptr(dL_dmeans, torch.float32),
+                                 _ptr(dL_dlog_scales, torch.float32), _ptr(dL_dquats, torch.float32),
+                                 _ptr(dL_dopacity_logits, torch.float32), _ptr(dL_dsh, torch.float32), _stream(stream))
+    _check(rc, "gs_grad_zero_rows")
 
 
 def gs_l1_loss(image, target, dL_dimage, loss_sum, stream=None):

@@ -899,6 +899,71 @@ extern "C" int gs_grad_zero_fill(int64_t N, int32_t sh_degree, float* dL_dmeans,
     return zero_fill_all(N, sh_degree, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits, dL_dsh, (cudaStream_t)stream);
 }
 
+// Zero the rows of the Gaussians that a visibility mask marks in ANY of its C views (gs_grad_zero_rows).  A warp reads
+// 32 consecutive mask words of every view (1024 Gaussians) and walks the set bits of the union; per marked Gaussian the
+// lanes store one row: the SH row as 16-byte stores where K3 and the pointer allow, the 11 floats of the other four arrays
+// from 11 further lanes.
+struct ZeroRowsArgs {
+    int64_t N, wn;
+    int32_t C, K3, sh_vec;
+    const uint32_t* vmask;
+    float* d_means; float* d_log_scales; float* d_quats; float* d_logits; float* d_sh;
+};
+__global__ void __launch_bounds__(256) zero_union_rows_kernel(const ZeroRowsArgs a) {
+    pdl_enter();
+    const int lane = threadIdx.x & 31;
+    const int64_t n_chunks = (a.N + 1023) / 1024;
+    const int64_t warps = (int64_t)gridDim.x * (blockDim.x >> 5);
+    for (int64_t chunk = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); chunk < n_chunks; chunk += warps) {
+        const int64_t w = chunk * 32 + lane;
+        uint32_t u = 0;
+        if (w < a.wn)
+            for (int c = 0; c < a.C; ++c) u |= __ldg(a.vmask + (int64_t)c * a.wn + w);
+        unsigned int live = __ballot_sync(0xffffffffu, u != 0u);
+        while (live) {
+            const int src = __ffs(live) - 1;
+            live &= live - 1;
+            uint32_t bits = __shfl_sync(0xffffffffu, u, src);
+            const int64_t base = (chunk * 32 + src) * 32;
+            while (bits) {
+                const int64_t i = base + (__ffs(bits) - 1);
+                bits &= bits - 1;
+                if (i >= a.N) break;
+                if (a.sh_vec) {
+                    float4* p4 = reinterpret_cast<float4*>(a.d_sh + i * a.K3);
+                    for (int k = lane; k < a.K3 / 4; k += 32) p4[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                } else {
+                    for (int k = lane; k < a.K3; k += 32) a.d_sh[i * a.K3 + k] = 0.f;
+                }
+                // lanes 16..18: mean, 19..21: log-scale, 22..25: quaternion, 26: logit (lanes 0..11 hold the SH row at degree 3)
+                if (lane >= 16 && lane < 19) a.d_means[3 * i + (lane - 16)] = 0.f;
+                else if (lane >= 19 && lane < 22) a.d_log_scales[3 * i + (lane - 19)] = 0.f;
+                else if (lane >= 22 && lane < 26) a.d_quats[4 * i + (lane - 22)] = 0.f;
+                else if (lane == 26) a.d_logits[i] = 0.f;
+            }
+        }
+    }
+}
+
+extern "C" int gs_grad_zero_rows(int64_t N, int32_t sh_degree, int32_t C, const uint32_t* vis_mask, float* dL_dmeans, float* dL_dlog_scales,
+                                 float* dL_dquats, float* dL_dopacity_logits, float* dL_dsh, void* stream) {
+    if (N < 0 || sh_degree < 0 || sh_degree > 3 || C < 1 || C > GS_MAX_VIEWS) return GS_ERR_INVALID_ARGUMENT;
+    if (N == 0) return GS_OK;
+    if (!vis_mask || !aligned(vis_mask, 16) || !dL_dmeans || !dL_dlog_scales || !dL_dquats || !dL_dopacity_logits || !dL_dsh)
+        return GS_ERR_INVALID_ARGUMENT;
+    ZeroRowsArgs a;
+    a.N = N; a.wn = GS_VIS_WORDS(N); a.C = C;
+    a.K3 = 3 * (sh_degree + 1) * (sh_degree + 1);
+    a.sh_vec = (a.K3 % 4 == 0 && aligned(dL_dsh, 16)) ? 1 : 0;
+    a.vmask = vis_mask;
+    a.d_means = dL_dmeans; a.d_log_scales = dL_dlog_scales; a.d_quats = dL_dquats; a.d_logits = dL_dopacity_logits; a.d_sh = dL_dsh;
+    const int64_t chunks = (N + 1023) / 1024;
+    const int64_t cap = (int64_t)sm_count() * 8;
+    const int64_t blocks = (chunks + 7) / 8 < cap ? (chunks + 7) / 8 : cap;
+    launch_chained(zero_union_rows_kernel, dim3((unsigned)blocks), dim3(256), (size_t)(0), (cudaStream_t)stream, a);
+    return launch_status();
+}
+
 extern "C" int gs_project_bwd(const gs_config* cfg, int64_t N, const float* means, const float* log_scales,
                               const float* quats, const float* opacity_logits, const float* sh, int32_t C,
                               const gs_camera* cams, const int32_t* radii, const uint32_t* vis_mask, const float* dL_dmeans2d,

@@ -110,6 +110,11 @@ class SplatStep:
         p = self.params
         if self.use_mask and not self._ls_bound_valid:
             self.refresh_log_scale_bound()
+        if getattr(self, "_grad_mask_swap", False):
+            # project_bwd_incremental needs the mask of its last call until its next one: this P1 writes into the other buffer
+            self.vis_mask, self._grad_mask = self._grad_mask, self.vis_mask
+            self._grad_mask_swap = False
+            self._grad_mask_valid = True
         B.gs_project_fwd(self.cfg, p["means"], p["log_scales"], p["quats"], p["opacity_logits"], p["sh"], self.cams,
                          self.means2d, self.depths, self.conics, self.opacities, self.rgbs, self.radii, self.tiles_touched,
                          vis_mask=self.vis_mask, log_scale_bound=self.ls_bound)
@@ -205,6 +210,27 @@ class SplatStep:
         B.gs_project_bwd(self.cfg, p["means"], p["log_scales"], p["quats"], p["opacity_logits"], p["sh"], self.cams,
                          self.radii, self.g_means2d, self.g_conics, self.g_opacities, self.g_rgbs, g["means"],
                          g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], accumulate, vis_mask=self.vis_mask)
+        if getattr(self, "_grad_mask", None) is not None:
+            self._grad_mask_swap = True        # the rows written last are those of this mask (see project_bwd_incremental)
+
+    def project_bwd_incremental(self):
+        """P5 with the DENSE result (what ``project_bwd(accumulate=0)`` leaves in ``self.grads``, zeros included, bit for bit)
+        without the dense zero-fill: the gradient arrays persist from step to step, so their only non-zero rows are those the
+        previous call wrote.  Those rows are cleared from the previous call's visibility mask (gs_grad_zero_rows), then the
+        visible rows of this step are overwritten (accumulate = 2): 2 x 236 bytes per visible Gaussian instead of 236 bytes
+        for every Gaussian.  Needs the visibility mask; the first call zero-fills once.  Nothing else may write to
+        ``self.grads`` between calls."""
+        assert self.use_mask, "project_bwd_incremental needs the visibility mask (use_mask=True)"
+        g = self.grads
+        if getattr(self, "_grad_mask", None) is None:
+            B.gs_grad_zero_fill(self.cfg.sh_degree, g["means"], g["log_scales"], g["quats"], g["opacity_logits"], g["sh"])
+            self._grad_mask = torch.empty_like(self.vis_mask)
+            self._grad_mask_valid = False
+        elif self._grad_mask_valid:
+            B.gs_grad_zero_rows(self.cfg.sh_degree, self.C, self._grad_mask, g["means"], g["log_scales"], g["quats"],
+                                g["opacity_logits"], g["sh"])
+            self._grad_mask_valid = False      # (a second call before the next P1 overwrites the same rows again)
+        self.project_bwd(accumulate=2)         # (marks vis_mask as "the mask of the last call": kept until the next call)
 
     def adam(self, mode="dense", lr=0.0, beta1=0.9, beta2=0.999, eps=1e-15):
         """One fused Adam step over the five parameter arrays (gs_adam_step); ``mode`` "dense" (the paper's _fused_adam_,
@@ -349,7 +375,7 @@ class SplatStep:
     # launches of this library's kernels in one step (memsets excluded): P1; compact, tile y-scan, x-scan,
     # ranges, histogram scan, depth-sort histogram + passes, entry offsets, tile-sort passes (+ keys); R1, L1,
     # zero rows, R2, P5
-    def launches_per_step(self):
+    def launches_per_step(self, p5_launches=None):
         tile_bits = max(1, int(np.ceil(np.log2(self.C * self.gx * self.gy))))
         view_bits = int(np.ceil(np.log2(self.C))) if self.C > 1 else 0
         depth_passes = 4 + (view_bits + 7) // 8
@@ -370,5 +396,7 @@ class SplatStep:
                 extra = 3
         compact = 1 if self.use_mask else (2 if self.C * self.N >= (1 << 24) else 1)   # radii mode, large inputs: visibility mask + scan over it
         p5 = 6 if self.N >= (1 << 22) else 1                         # dense zero-fill as five streaming launches for large N
+        if p5_launches is not None:
+            p5 = p5_launches                                         # e.g. 2 for project_bwd_incremental (row clearing + P5)
         loss = 2 if getattr(self, "loss_mode", "l1") == "l1ssim" else 1
         return extra + (loss - 1) + (p5 - 1) + 1 + (4 + compact) + 1 + depth_passes + 1 + tile_passes + (1 if self.want_keys else 0) + 1 + 1 + 1 + 1 + 1

@@ -243,3 +243,49 @@ def test_uploaded_parameters_refresh_the_scale_bound(B):
     st.project_fwd()
     torch.cuda.synchronize()
     assert not torch.equal(st.visible(), vis_ref)
+
+
+def test_incremental_gradient_clearing_equals_the_dense_overwrite(B):
+    """project_bwd_incremental (gs_grad_zero_rows from the previous step's mask + gs_project_bwd accumulate = 2) must leave
+    exactly the arrays of gs_project_bwd(accumulate = 0) -- zeros of the invisible rows included, bit for bit (P5 has no
+    atomics; both run on the same 2-D gradients) -- over steps whose cameras, and so whose visible sets, change; also after a
+    repeated call without a new P1 and after a dense call in between."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    sc = street_scene()
+    cam = sc["cameras"][0]
+    eye = np.asarray(cam["viewmat"])[:, :3].T @ -np.asarray(cam["viewmat"])[:, 3]
+    dirs = [((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (-1.0, 0.2, 0.0)), ((0.0, -1.0, 0.0), (1.0, 1.0, 0.0), (-1.0, -1.0, 0.0)),
+            ((0.3, 1.0, 0.1), (-1.0, 0.0, 0.0), (1.0, -0.4, 0.0)), ((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (-1.0, 0.2, 0.0))]
+    st = SplatStep(sc, use_mask=True)
+    st.set_target(scenes.target_image(sc))
+    ref = {k: torch.empty_like(v) for k, v in st.grads.items()}
+    for v in st.grads.values():
+        v.fill_(7.5)                                         # the first call must not rely on the arrays' contents
+    seen = None
+    for step, d3 in enumerate(dirs):
+        st.cams = B.make_cameras([scenes.make_camera(640, 360, 500.0, 500.0, eye, eye + np.array(d), (0, 0, 1), far=120.0) for d in d3])
+        st.project_fwd(); st.bin_tiles(sync=True); st.raster_fwd(); st.l1_loss(); st.raster_bwd()
+        p = st.params
+        for v in ref.values():
+            v.fill_(float("nan"))
+        B.gs_project_bwd(st.cfg, p["means"], p["log_scales"], p["quats"], p["opacity_logits"], p["sh"], st.cams, st.radii,
+                         st.g_means2d, st.g_conics, st.g_opacities, st.g_rgbs, ref["means"], ref["log_scales"], ref["quats"],
+                         ref["opacity_logits"], ref["sh"], 0, vis_mask=st.vis_mask)
+        if step == 2:
+            st.project_bwd()                                 # a dense call in between keeps the bookkeeping right
+        else:
+            st.project_bwd_incremental()
+            if step == 1:
+                st.project_bwd_incremental()                 # again, without a new P1
+        torch.cuda.synchronize()
+        vis_any = st.visible().any(dim=0)
+        n_vis = int(vis_any.sum())
+        assert 0 < n_vis < st.N // 4
+        if seen is not None:
+            assert int((seen & ~vis_any).sum()) > 1000       # rows written before and invisible now: they must be zero again
+        seen = vis_any if seen is None else (seen | vis_any)
+        for k in ref:
+            assert not bool(torch.isnan(ref[k]).any()), k
+            assert torch.equal(st.grads[k], ref[k]), (step, k)
+            assert bool((st.grads[k][~vis_any] == 0).all()), (step, k)
+        print(f"[step {step}] visible Gaussians {n_vis} of {st.N}")

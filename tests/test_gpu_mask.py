@@ -289,3 +289,36 @@ def test_incremental_gradient_clearing_equals_the_dense_overwrite(B):
             assert torch.equal(st.grads[k], ref[k]), (step, k)
             assert bool((st.grads[k][~vis_any] == 0).all()), (step, k)
         print(f"[step {step}] visible Gaussians {n_vis} of {st.N}")
+
+
+@pytest.mark.parametrize("N,C,deg", [(1, 1, 3), (513, 3, 0), (1023, 2, 1), (70_001, 3, 2), (300_007, 4, 3)])
+def test_grad_zero_rows_clears_exactly_the_union_of_the_mask(B, N, C, deg):
+    """gs_grad_zero_rows against numpy: the rows of Gaussians marked in any view become zero, every other row (and nothing
+    outside the arrays: they are allocated with a guard row on either side) keeps its contents; every SH degree, sizes
+    around the 512-Gaussian mask granule and the 1024-Gaussian warp chunk."""
+    rng = np.random.default_rng(N + deg)
+    vis = rng.random((C, N)) < (0.5 if N < 2000 else 0.03)
+    if N > 1:
+        vis[:, N - 1] = [c == C - 1 for c in range(C)]           # the last Gaussian, in the last view only
+    words = B.vis_words(N)
+    mask = torch.from_numpy(pack_mask(vis, words)).cuda()
+    K3 = 3 * (deg + 1) ** 2
+    shapes = {"means": 3, "log_scales": 3, "quats": 4, "opacity_logits": 1, "sh": K3}
+    full = {k: torch.full(((N + 2) * w,), 3.25, dtype=torch.float32, device="cuda") for k, w in shapes.items()}
+    g = {k: full[k][shapes[k]: (N + 1) * shapes[k]].view(N, shapes[k]) if shapes[k] > 1 else full[k][1: N + 1] for k in shapes}
+    # (the guard rows shift the alignment: unless the row width is a multiple of 4 floats the scalar store paths run here)
+    B.gs_grad_zero_rows(deg, C, mask, g["means"], g["log_scales"], g["quats"], g["opacity_logits"], g["sh"])
+    torch.cuda.synchronize()
+    any_vis = torch.from_numpy(vis.any(axis=0)).cuda()
+    for k, w in shapes.items():
+        rows = g[k].reshape(N, -1)
+        assert bool((rows[any_vis] == 0).all()), k
+        assert bool((rows[~any_vis] == 3.25).all()), k
+        assert bool((full[k][: w] == 3.25).all()) and bool((full[k][(N + 1) * w:] == 3.25).all()), k
+    # aligned arrays take the 16-byte store paths: same result
+    g2 = {k: torch.full((N, w) if w > 1 else (N,), 1.5, dtype=torch.float32, device="cuda") for k, w in shapes.items()}
+    B.gs_grad_zero_rows(deg, C, mask, g2["means"], g2["log_scales"], g2["quats"], g2["opacity_logits"], g2["sh"])
+    torch.cuda.synchronize()
+    for k in shapes:
+        rows = g2[k].reshape(N, -1)
+        assert bool((rows[any_vis] == 0).all()) and bool((rows[~any_vis] == 1.5).all()), k

@@ -306,6 +306,39 @@ class SplatStep:
         else:
             self.project_bwd()
 
+    # Every stage call is asynchronous and the record counts stay on the device, so a whole step is a fixed sequence of
+    # kernel launches that can be captured once and replayed as ONE CUDA graph launch (the programmatic dependent launches
+    # of launch_chained become programmatic edges of the graph).
+    def capture_step_graph(self):
+        """Capture one asynchronous step (P1, binning, R1, loss, R2, P5 with the dense gradient) on the current buffers into
+        a CUDA graph; ``replay_step_graph`` then runs a step with one launch.  The buffers, the cameras and the record
+        capacity are baked in: call again after ``set_cameras`` / a capacity change.  Overflow is reported only through
+        ``graph_record_count`` (the graph never synchronises)."""
+        self.step(sync=True)                 # sizes the buffers, fixes the tile-sort mode, sets every lazy kernel attribute
+        torch.cuda.current_stream(self.device).synchronize()
+        self._M_event = None
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            self.project_fwd()
+            B.gs_bin_tiles(self.cfg, self.N, self.cams, self.means2d, self.depths, self.radii, self.workspace, self.capacity_M,
+                           self.isect_keys, self.isect_vals, self.tile_ranges, self.M_dev, False, vis_mask=self.vis_mask,
+                           tile_sort=getattr(self, "tile_sort", 0))
+            self.raster_fwd()
+            self.l1_loss()
+            self.raster_bwd()
+            self.project_bwd()
+        self._graph = g
+        self._graph_capacity = self.capacity_M
+        return g
+
+    def replay_step_graph(self):
+        assert getattr(self, "_graph", None) is not None and self._graph_capacity == self.capacity_M, "capture_step_graph first"
+        self._graph.replay()
+
+    def graph_record_count(self):
+        """Record count M of the last replayed step (synchronises); M > capacity_M means that step rendered only the background."""
+        return int(self.M_dev.item())
+
     def step_from_host(self, host_params, host_target, host_loss):
         """End-to-end step, synchronous form: ``upload_async`` + ``step_uploaded`` + wait.  Parameters and target images
         come from (pinned) host tensors, the loss goes back to ``host_loss``."""

@@ -574,6 +574,40 @@ def test_step_from_host_equals_resident_step(B):
         assert rel_l2(st.grads[k].cpu().numpy(), ref.grads[k].cpu().numpy()) <= 1e-5, k
 
 
+@pytest.mark.parametrize("use_mask", [False, True])
+def test_step_graph_replay_equals_the_eager_step(B, use_mask):
+    """A whole asynchronous step captured into one CUDA graph (SplatStep.capture_step_graph; every launch carries the
+    programmatic-dependent-launch attribute) and replayed, on fresh inputs poisoned in between: same lists, image and
+    loss as the eager step, gradients equal up to the order of the float atomics; also after the parameters changed."""
+    from paper_2606_11390_b200.pipeline import SplatStep
+    name, sc = SCENES[1]
+    tgt = scenes.target_image(sc)
+    ref = SplatStep(sc, use_mask=use_mask)
+    ref.set_target(tgt)
+    st = SplatStep(sc, use_mask=use_mask)
+    st.set_target(tgt)
+    st.capture_step_graph()
+    for round_ in range(2):
+        if round_ == 1:                      # new parameters in the same buffers: the graph reads them at replay time
+            for s_ in (ref, st):
+                s_.params["means"].add_(0.01)
+                s_.params["opacity_logits"].sub_(0.2)
+        ref.step(sync=True)
+        torch.cuda.synchronize()
+        for t in (st.image, st.final_T, st.g_means2d, st.g_conics, *st.grads.values()):
+            t.fill_(float("nan"))
+        st.isect_vals.fill_(-7); st.tile_ranges.fill_(-7); st.n_contrib.fill_(-7)
+        st.replay_step_graph()
+        st.replay_step_graph()               # twice in a row: nothing of a replay may depend on the previous one
+        torch.cuda.synchronize()
+        assert st.graph_record_count() == ref.M and ref.M > 0
+        assert torch.equal(st.isect_vals[: ref.M], ref.isect_vals[: ref.M]) and torch.equal(st.tile_ranges, ref.tile_ranges)
+        assert torch.equal(st.image, ref.image) and torch.equal(st.final_T, ref.final_T) and torch.equal(st.n_contrib, ref.n_contrib)
+        assert abs(float(st.loss.item()) - float(ref.loss.item())) <= 1e-5 * abs(float(ref.loss.item()))
+        for k in st.param_names:
+            assert rel_l2(st.grads[k].cpu().numpy(), ref.grads[k].cpu().numpy()) <= 1e-5, k
+
+
 def test_pipelined_uploads_equal_resident_steps(B):
     """upload_async(k + 1) overlapping step_uploaded(k) (two input sets, copy stream): every step sees its own inputs.
     Steps alternate between two parameter sets and two targets; each must reproduce the resident step on that pair."""

@@ -10,6 +10,10 @@ gs_project_fwd -> gs_bin_tiles -> gs_raster_fwd -> gs_l1_loss -> gs_raster_bwd -
 after 10 warm-up) with inputs resident in HBM; `e2e` = the same with the step's inputs (parameters + target images)
 copied from pinned host memory and the loss read back inside the timed region.  One JSON line is printed by rank 0.
 
+Beside the headline the line carries two more timings of the same step, never instead of it: `grads_incremental` (the dense
+gradient arrays produced by clearing only the rows of the previous step instead of zero-filling all of them) and
+`graph_replay` (the whole step replayed as one CUDA graph launch).
+
 The default workload is `city` (60 M Gaussians, four 4K views): BASELINE.json's metric is not quoted on one config, so
 the N = 1 line is on the largest single-GPU one; `per_config` carries the short runs of the other configs.
 

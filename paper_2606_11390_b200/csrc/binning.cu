@@ -540,9 +540,14 @@ __global__ void __launch_bounds__(kScanThreads) visible_kernel(const CompactArgs
 // corner differences).  VIEWS = true: `vmask` is the per-view mask [C][wn] written by gs_project_fwd (bit i & 31 of word
 // c wn + (i >> 5)); the rectangle corners are added here, from the gathered means2d and radii of the visible entries.
 // wn is a multiple of 16 words and a thread owns 16 consecutive words, so a thread's words belong to one view.
-template <bool VIEWS, int WPT>
+// FILL = false (only with VIEWS): the expansion writes nothing but the entry ids; the depth keys and the rectangle corners of
+// the compacted entries are produced by entry_fill_kernel, one thread per entry.  When the visible entries are clustered in
+// index (a Morton-ordered scene: a few blocks of this kernel own all of them) the gathers then do not hang on the few
+// threads whose mask words happen to be full.
+template <bool VIEWS, int WPT, bool FILL>
 __global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const CompactArgs a, const unsigned int* __restrict__ vmask, int64_t n_words,
                                                                     int64_t wn) {
+    static_assert(FILL || VIEWS, "the split form exists for the caller's per-view mask only");
     pdl_enter();
     __shared__ unsigned int s_ticket;
     __shared__ ChainScanSmem s_scan;
@@ -592,7 +597,25 @@ __global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const Compac
         nzw &= nzw - 1;
         unsigned int m = s_w[q][tid];
         const int64_t eq = e_first + (q << 5);
-        while (m) {
+        if constexpr (!FILL) {
+            while (m) {
+                const int64_t e = eq + (__ffs(m) - 1);
+                m &= m - 1;
+                if ((int64_t)r < a.vcap) {
+                    a.cvals[r] = (int)e;
+                } else if (VIEWS) {
+                    // beyond the compact capacity (the call will report an overflow): the rectangle still counts, M must be exact
+                    const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + e);
+                    int x0, x1, y0, y1;
+                    tile_rect(uv.x, uv.y, __ldg(a.radii + e), a.gx, a.gy, x0, x1, y0, y1);
+                    atomicAdd(grid + y0 * sx + x0, 1);
+                    atomicAdd(grid + y0 * sx + x1, -1);
+                    atomicAdd(grid + y1 * sx + x0, -1);
+                    atomicAdd(grid + y1 * sx + x1, 1);
+                }
+                ++r;
+            }
+        } else while (m) {
             int64_t e[4];
             bool on[4];
             float dep[4];
@@ -629,6 +652,31 @@ __global__ void __launch_bounds__(kScanThreads) compact_mask_kernel(const Compac
                     ++r;
                 }
         }
+    }
+}
+
+// Second half of the split compaction: entry r of the compacted list (ids written by compact_mask_kernel<true, WPT, false>)
+// gets its (view << 32 | depth bits) key, and its tile rectangle adds +1 / -1 at the four corners of its view's
+// difference grid.  One thread per entry, persistent grid.
+__global__ void __launch_bounds__(256) entry_fill_kernel(const CompactArgs a) {
+    pdl_enter();
+    const int64_t V = (int64_t)a.hdr->V;            // already clamped to the compact capacity
+    const unsigned int n32 = (unsigned int)a.N;
+    const int sx = a.gx + 1, sy = a.gy + 1;
+    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < V; r += (int64_t)gridDim.x * blockDim.x) {
+        const unsigned int e = (unsigned int)a.cvals[r];
+        const unsigned int view = e / n32;
+        const float dep = __ldg(a.depths + e);
+        const float2 uv = __ldg(reinterpret_cast<const float2*>(a.means2d) + e);
+        const int rad = __ldg(a.radii + e);
+        a.ckeys[r] = ((unsigned long long)view << 32) | (unsigned long long)__float_as_uint(dep);
+        int x0, x1, y0, y1;
+        tile_rect(uv.x, uv.y, rad, a.gx, a.gy, x0, x1, y0, y1);
+        int* const grid = a.tdiff + (int64_t)view * ((int64_t)sx * sy);
+        atomicAdd(grid + y0 * sx + x0, 1);
+        atomicAdd(grid + y0 * sx + x1, -1);
+        atomicAdd(grid + y1 * sx + x0, -1);
+        atomicAdd(grid + y1 * sx + x1, 1);
     }
 }
 
@@ -1680,11 +1728,15 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
             const int64_t wn = GS_VIS_WORDS(N), n_words = (int64_t)C * wn;
             if (n_words >= kMaskWideMinWords) {
                 a.n_blocks = (unsigned int)((n_words + kScanThreads * 16 - 1) / (kScanThreads * 16));
-                launch_chained(compact_mask_kernel<true, 16>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vis_mask, n_words, wn);
+                launch_chained(compact_mask_kernel<true, 16, false>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vis_mask, n_words, wn);
             } else {
                 a.n_blocks = (unsigned int)((n_words + kScanThreads * 4 - 1) / (kScanThreads * 4));
-                launch_chained(compact_mask_kernel<true, 4>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vis_mask, n_words, wn);
+                launch_chained(compact_mask_kernel<true, 4, false>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vis_mask, n_words, wn);
             }
+            rc = launch_status();
+            if (rc) return rc;
+            const int64_t fb = (w.vcap + 255) / 256;
+            launch_chained(entry_fill_kernel, dim3((unsigned)(fb < (int64_t)sms * 8 ? (fb > 0 ? fb : 1) : (int64_t)sms * 8)), dim3(256), (size_t)(0), st, a);
         } else if (n_entries >= kMaskMinEntries) {
             // large inputs: streaming visibility mask, then the ordered scan over the mask
             unsigned int* vmask = reinterpret_cast<unsigned int*>(ws + w.off_vmask);
@@ -1693,7 +1745,7 @@ extern "C" int gs_bin_tiles(const gs_config* cfg, int64_t N, int32_t C, const gs
             rc = launch_status();
             if (rc) return rc;
             a.n_blocks = (unsigned int)((n_words + kScanThreads * 16 - 1) / (kScanThreads * 16));
-            launch_chained(compact_mask_kernel<false, 16>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vmask, n_words, 0);
+            launch_chained(compact_mask_kernel<false, 16, true>, dim3(a.n_blocks), dim3(kScanThreads), (size_t)(0), st, a, vmask, n_words, 0);
         } else switch (cvec) {
             case 8: launch_chained(compact_kernel<8>, dim3((unsigned)n_blocks), dim3(kScanThreads), (size_t)(0), st, a); break;
             case 4: launch_chained(compact_kernel<4>, dim3((unsigned)n_blocks), dim3(kScanThreads), (size_t)(0), st, a); break;

@@ -434,7 +434,7 @@ class SplatStep:
                 gbits = max(1, int(np.ceil(np.log2(groups))))
                 tile_passes = min((gbits + 7) // 8, (gbits + 8) // 9)
                 extra = 3
-        compact = 1 if self.use_mask else (2 if self.C * self.N >= (1 << 24) else 1)   # radii mode, large inputs: visibility mask + scan over it
+        compact = 2 if self.use_mask else (2 if self.C * self.N >= (1 << 24) else 1)   # mask: id compaction + entry_fill_kernel;   # radii mode, large inputs: visibility mask + scan over it
         p5 = 6 if self.N >= (1 << 22) else 1                         # dense zero-fill as five streaming launches for large N
         if p5_launches is not None:
             p5 = p5_launches                                         # e.g. 2 for project_bwd_incremental (row clearing + P5)

@@ -10,9 +10,10 @@ gs_project_fwd -> gs_bin_tiles -> gs_raster_fwd -> gs_l1_loss -> gs_raster_bwd -
 after 10 warm-up) with inputs resident in HBM; `e2e` = the same with the step's inputs (parameters + target images)
 copied from pinned host memory and the loss read back inside the timed region.  One JSON line is printed by rank 0.
 
-Beside the headline the line carries two more timings of the same step, never instead of it: `grads_incremental` (the dense
+Beside the headline the line carries three more timings of the same step, never instead of it: `grads_incremental` (the dense
 gradient arrays produced by clearing only the rows of the previous step instead of zero-filling all of them) and
-`graph_replay` (the whole step replayed as one CUDA graph launch).
+`graph_replay` (the whole step replayed as one CUDA graph launch) and `morton_order` (the same scene with its Gaussians
+reordered along a Morton curve once, as the paper's trainer does during densification).
 
 The default workload is `city` (60 M Gaussians, four 4K views): BASELINE.json's metric is not quoted on one config, so
 the N = 1 line is on the largest single-GPU one; `per_config` carries the short runs of the other configs.
@@ -674,6 +675,39 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
             unpin_host(t)
         del host_params, host_tgt
 
+    # ---- the same step on the Morton-ordered scene (the paper's trainer sorts the Gaussians
+    # along a Morton curve during densification and reports 5-10 % from it); last, because it reorders the resident parameters
+    morton_leg = None
+    if not args.morton and args.grads == "dense" and not args.sparse_grads and not overlap and args.adam == "none":
+        try:
+            B.morton_sort({k: st.params[k] for k in st.param_names})          # warm-up (allocations, first launches)
+            torch.cuda.synchronize()
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            m0.record()
+            sorted_params, _ = B.morton_sort({k: st.params[k] for k in st.param_names})
+            m1.record()
+            torch.cuda.synchronize()
+            for k in st.param_names:
+                st.params[k].copy_(sorted_params[k])
+            del sorted_params
+            for _ in range(3):
+                st.step(sync=False)
+            barrier()
+            mev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            for k in range(steps):
+                flush.fill_(k & 0xFF)
+                mev[k][0].record(stream)
+                st.step(sync=False)
+                mev[k][1].record(stream)
+            barrier()
+            assert st.overflow_count == 0 and not st.check_overflow(wait=True)
+            mo_ms = max_over_ranks(float(np.median([a.elapsed_time(b) for a, b in mev])), world, dev)
+            morton_leg = {"ms_per_step": mo_ms, "value": whole_job_rate(world, mpix_step, mo_ms), "unit": "MP/s", "steps": steps,
+                          "sort_ms": m0.elapsed_time(m1), "note": "one-time reordering of the five parameter arrays (gs_bounds, "
+                          "gs_morton_codes, gs_sort_pairs, gs_gather_rows), outside the steps; same scene, same images"}
+        except Exception as e:
+            morton_leg = {"error": repr(e)[:200]}
+
     out = {
         "value": value, "ms_per_step": ms_per_step, "ms_per_step_mean": ms_mean, "gaussians_per_s": gauss_per_s,
         "config": {"workload": workload + (" (far = +inf)" if far_inf else ""), "loss": args.loss, "morton": bool(args.morton), "adam": args.adam,
@@ -687,7 +721,7 @@ def bench_workload(args, workload, dev, peaks, world, steps, warmup, want_e2e, f
                    "l2": "256 MiB buffer written between timed steps (L2 flush); per-step working set also exceeds the 126 MB L2"},
         "morton_sort_ms": morton_ms, "clocks": clocks, "e2e": e2e,
         "gpu_launches": (st.launches_per_step(2 if args.grads == "incremental" else (1 if args.sparse_grads else None)) + {"none": 0, "dense": 5, "sparse": 1}[args.adam]) * steps,
-        "roofline": roof, "stages": stage_roof, "wall_s_timed_region": round(t_wall, 3), "grads_incremental": inc, "graph_replay": graph_leg,
+        "roofline": roof, "stages": stage_roof, "wall_s_timed_region": round(t_wall, 3), "grads_incremental": inc, "graph_replay": graph_leg, "morton_order": morton_leg,
     }
     del st, flush
     torch.cuda.empty_cache()
@@ -736,7 +770,7 @@ def run_b200(args):
         "data": "synthetic",
     }
     for k in ("config", "gaussians_per_s", "ms_per_step_mean", "morton_sort_ms", "clocks", "e2e", "gpu_launches", "roofline", "stages",
-              "grads_incremental", "graph_replay"):
+              "grads_incremental", "graph_replay", "morton_order"):
         line[k] = main[k]
     line["cpu_baseline"] = cpu
     line["per_config"] = per_config
